@@ -1,0 +1,250 @@
+/*
+ * ge_ref.c -- ORACLE (test infrastructure, NOT the product).
+ *
+ * Plain, slow, scalar fp64 CPU statement of the group-explicit (GE) scheme of
+ * arXiv 1310.3422 for u_t = u_xx (and the 2x2-group 2-D reading for
+ * u_t = u_xx + u_yy).  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code with paper_1310_3422_b200/csrc: the formulas below are
+ * written literally as the paper prints them (with the division), never in
+ * the factored form the CUDA kernels use.
+ *
+ * Notation: N interior nodes 1..N, nodes 0 and N+1 are
+ * the Dirichlet boundary (h = 1/(N+1)); r = tau/h^2
+ * (PAPER.md:73); k = sub-domain length; level = one advance by
+ * tau; phase = level mod 2 (the paper's "first row"/"second row",
+ * PAPER.md:140-148).  Arrays passed to the *_level_* functions carry the
+ * boundary nodes: 1-D length N+2, 2-D (N_y+2) x (N_x+2) row-major.
+ *
+ * Parity pins (tests/test_oracle_*.py): P1 2x2 solve identity, P2 invariants,
+ * P3/P9 exact-rational worked examples (tests/golden), P4 dense A^-1 B brute
+ * force from the implicit statement, P5 spectral radius of the two-level
+ * cycle, P6/P7 convergence to e^{-pi^2 t} sin(pi x), P8 Saul'yev special case.
+ * The 2-D functions follow DESIGN.md reading R-2D (PAPER.md defines no 2-D
+ * scheme; PAPER.md:134, :228 only claim the extension) and are pinned by
+ * P2, P4, P5, P6, P8, P9 only: "parity unpinned by the paper" for 2-D.
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* non-negative remainder */
+static int64_t pmod(int64_t a, int64_t m) {
+    int64_t x = a % m;
+    return x < 0 ? x + m : x;
+}
+
+/*
+ * One level in 1-D for any k >= 1.
+ *
+ * Class of node i: c(i) = (i - phase*k) mod 2k
+ *   c == 2k-1 : left member of the confluence pair (i, i+1)   -> Eq (3)
+ *   c == 0    : right member of the pair (i-1, i)             -> Eq (4)
+ *   1..k-1    : Saul'yev A, Eq (1), ascending i (uses new[i-1])
+ *   k..2k-2   : Saul'yev B, Eq (2), descending i (uses new[i+1])
+ * Prefactor of Eqs (3),(4): 1/(1+2r) (the printed "3" is an extraction
+ * artefact: the four weights sum to 1+2r; reading R-A1).
+ * A pair with a boundary member is not solved as a pair: its interior member
+ * takes Eq (1) (partner node 0) or Eq (2) (partner node N+1) with the boundary
+ * value as the new-level neighbour ("preinitialized").
+ *
+ * old_, new_: length N+2; old_[0], old_[N+1] hold the boundary values, which
+ * are copied to new_ (constant in time).
+ */
+void ge_ref_level_1d(const double *old_, double *new_, int64_t N, double r,
+                     int64_t k, int64_t phase)
+{
+    const int64_t two_k = 2 * k;
+    int64_t i;
+    new_[0] = old_[0];
+    new_[N + 1] = old_[N + 1];
+
+    /* first: confluence pairs, any order */
+    for (i = 0; i <= N; ++i) {
+        if (pmod(i - phase * k, two_k) != two_k - 1) continue;
+        /* i is a left member, i+1 the right member */
+        if (i >= 1 && i + 1 <= N) {
+            new_[i] = ((r + r * r) * old_[i - 1] + (1.0 - r * r) * old_[i]
+                       + (r - r * r) * old_[i + 1] + r * r * old_[i + 2])
+                      / (1.0 + 2.0 * r);                                   /* Eq (3) */
+            new_[i + 1] = (r * r * old_[i - 1] + (r - r * r) * old_[i]
+                           + (1.0 - r * r) * old_[i + 1] + (r + r * r) * old_[i + 2])
+                          / (1.0 + 2.0 * r);                               /* Eq (4) */
+        } else if (i == 0 && N >= 1) {
+            /* pair (0,1): node 0 is boundary -> node 1 by Eq (1) */
+            new_[1] = (r * new_[0] + (1.0 - r) * old_[1] + r * old_[2]) / (1.0 + r);
+        } else if (i == N && N >= 1) {
+            /* pair (N,N+1): node N+1 is boundary -> node N by Eq (2) */
+            new_[N] = (r * new_[N + 1] + (1.0 - r) * old_[N] + r * old_[N - 1]) / (1.0 + r);
+        }
+    }
+    /* second: Eq (1) nodes, ascending */
+    for (i = 1; i <= N; ++i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= 1 && c <= k - 1)
+            new_[i] = (r * new_[i - 1] + (1.0 - r) * old_[i] + r * old_[i + 1]) / (1.0 + r);
+    }
+    /* third: Eq (2) nodes, descending */
+    for (i = N; i >= 1; --i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= k && c <= two_k - 2)
+            new_[i] = (r * new_[i + 1] + (1.0 - r) * old_[i] + r * old_[i - 1]) / (1.0 + r);
+    }
+}
+
+/*
+ * `steps` levels of one rod starting at level counter `level0` (phase =
+ * level mod 2, phase 0 first: DESIGN.md reading R-A3).  u holds the N
+ * interior values and is overwritten by the final level.  Returns 0, or -1 if
+ * out of memory.
+ */
+int ge_ref_run_1d(double *u, int64_t N, double r, int64_t k, double bc_lo,
+                  double bc_hi, int64_t level0, int64_t steps)
+{
+    double *a = (double *)malloc((size_t)(N + 2) * sizeof(double));
+    double *b = (double *)malloc((size_t)(N + 2) * sizeof(double));
+    int64_t s;
+    if (!a || !b) { free(a); free(b); return -1; }
+    a[0] = bc_lo; a[N + 1] = bc_hi;
+    memcpy(a + 1, u, (size_t)N * sizeof(double));
+    for (s = 0; s < steps; ++s) {
+        double *t;
+        ge_ref_level_1d(a, b, N, r, k, pmod(level0 + s, 2));
+        t = a; a = b; b = t;
+    }
+    memcpy(u, a + 1, (size_t)N * sizeof(double));
+    free(a); free(b);
+    return 0;
+}
+
+/*
+ * Batched rods (BASELINE.json configs[2]): rod b has its own r[b], bc_lo[b],
+ * bc_hi[b]; u is [batch][N] row-major, interior values only.
+ */
+int ge_ref_run_batched_1d(double *u, int64_t batch, int64_t N, const double *r,
+                          int64_t k, const double *bc_lo, const double *bc_hi,
+                          int64_t level0, int64_t steps)
+{
+    int64_t b;
+    for (b = 0; b < batch; ++b) {
+        int rc = ge_ref_run_1d(u + b * N, N, r[b], k, bc_lo[b], bc_hi[b], level0, steps);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+/*
+ * One level in 2-D, 2x2 four-point groups (reading R-2D).
+ *
+ * Nodes (i,j), i = 0..Nx+1 along x (fastest), j = 0..Ny+1 along y; interior
+ * 1..N; edges Dirichlet; corner nodes are never read.  Group anchors
+ * (lower-left member) at i == 1+phase, j == 1+phase (mod 2): phase 0 anchors
+ * 1,3,5,...; phase 1 anchors 0,2,4,... (diagonal shift), groups sticking out
+ * over an edge keep only their interior members.
+ *
+ * For an interior member P with in-group neighbours G (new level) and
+ * out-of-group neighbours O (old level):
+ *     (1+2r) new_P - r sum_G new_G = R_P := (1-2r) old_P + r sum_O old_O
+ * where a boundary in-group neighbour contributes r*beta to the right side.
+ *
+ * Full group a=(i,j) b=(i+1,j) c=(i,j+1) d=(i+1,j+1):
+ *   new = M (R_a,R_b,R_c,R_d)^T / ((1+2r)(1+4r)),
+ *   M = [[al,be,be,ga],[be,al,ga,be],[be,ga,al,be],[ga,be,be,al]],
+ *   al = 1+4r+2r^2, be = r(1+2r), ga = 2r^2.
+ * Edge group (two interior members adjacent along the edge):
+ *   new_1 = ((1+2r) R_1 + r R_2) / ((1+r)(1+3r)), symmetric for new_2.
+ * Corner group (one interior member): new = R / (1+2r).
+ */
+#define AT(a, i, j) ((a)[(size_t)(j) * (size_t)sx + (size_t)(i)])
+
+void ge_ref_level_2d(const double *old_, double *new_, int64_t Nx, int64_t Ny,
+                     double r, int64_t phase)
+{
+    const int64_t sx = Nx + 2;
+    const double al = 1.0 + 4.0 * r + 2.0 * r * r;
+    const double be = r * (1.0 + 2.0 * r);
+    const double ga = 2.0 * r * r;
+    const double det4 = (1.0 + 2.0 * r) * (1.0 + 4.0 * r);
+    const double det2 = (1.0 + r) * (1.0 + 3.0 * r);
+    int64_t i, j, gi, gj;
+
+    /* boundary nodes are constant in time */
+    for (i = 0; i <= Nx + 1; ++i) { AT(new_, i, 0) = AT(old_, i, 0); AT(new_, i, Ny + 1) = AT(old_, i, Ny + 1); }
+    for (j = 0; j <= Ny + 1; ++j) { AT(new_, 0, j) = AT(old_, 0, j); AT(new_, Nx + 1, j) = AT(old_, Nx + 1, j); }
+
+    for (gj = 1 - phase; gj <= Ny; gj += 2) {
+        for (gi = 1 - phase; gi <= Nx; gi += 2) {
+            /* members: (gi,gj) (gi+1,gj) (gi,gj+1) (gi+1,gj+1); which are interior? */
+            const int x0 = (gi >= 1), x1 = (gi + 1 <= Nx);
+            const int y0 = (gj >= 1), y1 = (gj + 1 <= Ny);
+            /* right-hand sides: out-of-group neighbours at the old level.  For
+               member (gi+dx, gj+dy) the out-of-group x-neighbour is at
+               gi+dx + (dx ? +1 : -1), likewise in y. */
+            double R[2][2];
+            int dx, dy;
+            for (dy = 0; dy < 2; ++dy)
+                for (dx = 0; dx < 2; ++dx) {
+                    const int64_t pi = gi + dx, pj = gj + dy;
+                    const int inside = (dx ? x1 : x0) && (dy ? y1 : y0);
+                    if (!inside) { R[dy][dx] = 0.0; continue; }
+                    R[dy][dx] = (1.0 - 2.0 * r) * AT(old_, pi, pj)
+                              + r * AT(old_, pi + (dx ? 1 : -1), pj)
+                              + r * AT(old_, pi, pj + (dy ? 1 : -1));
+                    /* in-group neighbour that is a boundary node: known value */
+                    if (!(dx ? x0 : x1)) R[dy][dx] += r * AT(old_, pi + (dx ? -1 : 1), pj);
+                    if (!(dy ? y0 : y1)) R[dy][dx] += r * AT(old_, pi, pj + (dy ? -1 : 1));
+                }
+            if (x0 && x1 && y0 && y1) {
+                const double Ra = R[0][0], Rb = R[0][1], Rc = R[1][0], Rd = R[1][1];
+                AT(new_, gi,     gj)     = (al * Ra + be * Rb + be * Rc + ga * Rd) / det4;
+                AT(new_, gi + 1, gj)     = (be * Ra + al * Rb + ga * Rc + be * Rd) / det4;
+                AT(new_, gi,     gj + 1) = (be * Ra + ga * Rb + al * Rc + be * Rd) / det4;
+                AT(new_, gi + 1, gj + 1) = (ga * Ra + be * Rb + be * Rc + al * Rd) / det4;
+            } else if (x0 && x1) {            /* one interior row: members along x */
+                const int64_t pj = y0 ? gj : gj + 1;
+                const double R1 = R[y0 ? 0 : 1][0], R2 = R[y0 ? 0 : 1][1];
+                if (!(y0 || y1)) continue;
+                AT(new_, gi,     pj) = ((1.0 + 2.0 * r) * R1 + r * R2) / det2;
+                AT(new_, gi + 1, pj) = (r * R1 + (1.0 + 2.0 * r) * R2) / det2;
+            } else if (y0 && y1) {            /* one interior column: members along y */
+                const int64_t pi = x0 ? gi : gi + 1;
+                const double R1 = R[0][x0 ? 0 : 1], R2 = R[1][x0 ? 0 : 1];
+                if (!(x0 || x1)) continue;
+                AT(new_, pi, gj)     = ((1.0 + 2.0 * r) * R1 + r * R2) / det2;
+                AT(new_, pi, gj + 1) = (r * R1 + (1.0 + 2.0 * r) * R2) / det2;
+            } else if ((x0 || x1) && (y0 || y1)) {   /* single interior member */
+                const int64_t pi = x0 ? gi : gi + 1, pj = y0 ? gj : gj + 1;
+                AT(new_, pi, pj) = R[y0 ? 0 : 1][x0 ? 0 : 1] / (1.0 + 2.0 * r);
+            }
+        }
+    }
+}
+
+/*
+ * `steps` levels in 2-D.  u: Ny x Nx interior values, row-major [j][i],
+ * overwritten by the final level.  bc = {x_lo, x_hi, y_lo, y_hi}: the constant
+ * value on the edges i=0, i=Nx+1, j=0, j=Ny+1.
+ */
+int ge_ref_run_2d(double *u, int64_t Nx, int64_t Ny, double r, const double *bc,
+                  int64_t level0, int64_t steps)
+{
+    const int64_t sx = Nx + 2;
+    const size_t tot = (size_t)(Nx + 2) * (size_t)(Ny + 2);
+    double *a = (double *)calloc(tot, sizeof(double));
+    double *b = (double *)calloc(tot, sizeof(double));
+    int64_t i, j, s;
+    if (!a || !b) { free(a); free(b); return -1; }
+    for (j = 0; j <= Ny + 1; ++j) { AT(a, 0, j) = bc[0]; AT(a, Nx + 1, j) = bc[1]; }
+    for (i = 1; i <= Nx; ++i) { AT(a, i, 0) = bc[2]; AT(a, i, Ny + 1) = bc[3]; }
+    for (j = 1; j <= Ny; ++j)
+        memcpy(&AT(a, 1, j), u + (size_t)(j - 1) * (size_t)Nx, (size_t)Nx * sizeof(double));
+    for (s = 0; s < steps; ++s) {
+        double *t;
+        ge_ref_level_2d(a, b, Nx, Ny, r, pmod(level0 + s, 2));
+        t = a; a = b; b = t;
+    }
+    for (j = 1; j <= Ny; ++j)
+        memcpy(u + (size_t)(j - 1) * (size_t)Nx, &AT(a, 1, j), (size_t)Nx * sizeof(double));
+    free(a); free(b);
+    return 0;
+}
