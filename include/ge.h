@@ -1,0 +1,129 @@
+/*
+ * ge.h -- C ABI of libge: the time-marching loop of the group-explicit (GE)
+ * finite-difference scheme of arXiv 1310.3422 for U_t = laplace(U), on one
+ * NVIDIA B200 (sm_100a).  Every step of the path runs in libge's own CUDA
+ * kernels; there is no CPU fallback.
+ *
+ * The method (citations are PAPER.md lines; DESIGN.md lists the readings):
+ *   - grid: N interior nodes 1..N per axis, nodes 0 and N+1 Dirichlet and
+ *     constant in time, h = 1/(N+1), r = tau/h^2
+ *   - one LEVEL advances every node by tau.  phase = level mod 2.
+ *   - 1-D, group_k = 1 ("two-point groups"): the nodes are split into pairs
+ *     (i,i+1), left members at i = 1+phase (mod 2); each pair's 2x2 implicit
+ *     block is solved in closed form from the four previous-level values
+ *     u_{i-1}..u_{i+2} -- Eqs (3),(4), with prefactor 1/(1+2r);
+ *     a pair with a boundary member updates its interior member by Saul'yev's
+ *     Eq (1)/(2) with the boundary value as new-level neighbour
+ *     (PAPER.md:70-78, :142, :148).  The pattern alternates between levels
+ *     (PAPER.md:92, :140-150).
+ *   - 2-D (reading R-2D; the paper only claims the extension,
+ *     PAPER.md:134, :228): 2x2 four-point groups anchored at (1+phase, 1+phase)
+ *     (mod 2) -- diagonal shift --, in-group links implicit, out-of-group links
+ *     explicit, 4x4 block solved in closed form; groups cut by an edge keep
+ *     their interior members.
+ *
+ * Conventions
+ *   - All functions return GE_OK (0) or a negative ge_status.  None throws.
+ *     None synchronises the stream except ge_run_host (see there).
+ *   - "device pointer": memory of the current CUDA device, owned by the
+ *     caller, holding INTERIOR nodes only, contiguous, row-major:
+ *     1-D [batch][nx], 2-D [ny][nx] (x fastest).  16-byte alignment of the
+ *     base pointer selects the vectorised kernels; any alignment is accepted.
+ *   - ge_stream_t is a cudaStream_t (CUstream); 0 = the legacy default stream.
+ *   - A plan is used from one host thread and one stream at a time.
+ *   - Determinism: same inputs and plan settings give bit-identical output.
+ */
+#ifndef GE_H_
+#define GE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ge_plan ge_plan;                 /* opaque, owned by the library */
+typedef struct CUstream_st *ge_stream_t;        /* == cudaStream_t              */
+
+typedef enum { GE_F32 = 0, GE_F64 = 1 } ge_dtype;
+
+typedef enum {
+    GE_KERNEL_AUTO = 0,       /* library picks per shape                  */
+    GE_KERNEL_PER_STEP = 1,   /* A: one launch per level, one HBM round trip per level              */
+    GE_KERNEL_TEMPORAL = 2,   /* B: tb levels per launch in registers/SMEM, halo-redundant tiles    */
+    GE_KERNEL_PERSISTENT = 3  /* C: state stays on chip for the whole run (rod-per-warp, batched 1-D) */
+} ge_kernel;
+
+typedef enum {
+    GE_OK = 0,
+    GE_EINVAL = -1,           /* bad argument; nothing was enqueued                   */
+    GE_ENOMEM = -2,           /* host or device allocation failed                     */
+    GE_ECUDA = -3,            /* a CUDA call failed; ge_strerror appends its message  */
+    GE_EUNSUPPORTED = -4      /* valid request the GPU path does not implement (group_k >= 2) */
+} ge_status;
+
+typedef struct {
+    int32_t   dim;        /* 1 or 2                                                                    */
+    int64_t   nx, ny;     /* interior nodes per axis, >= 1 (ny must be 1 when dim == 1)                */
+    int64_t   batch;      /* independent 1-D rods, >= 1 (must be 1 when dim == 2)                      */
+    int32_t   dtype;      /* ge_dtype: arithmetic and storage type of u                                */
+    int32_t   group_k;    /* 1 = two-point groups (2x2 groups in 2-D); >= 2 = PAPER.md:82 sub-domain
+                             length k: GE_EUNSUPPORTED on the GPU            */
+    const double *r;      /* HOST array, `batch` entries (dim 2: 1 entry), finite, > 0; copied         */
+    const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; copied  */
+    const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; copied  */
+    int32_t   kernel;     /* ge_kernel                                                                 */
+    int32_t   tb;         /* levels per launch for TEMPORAL (0 = auto); ignored otherwise              */
+} ge_desc;
+
+/* Create a plan: validates desc, uploads per-rod coefficients (r, r/(1+2r), r/(1+r), ... computed in
+ * fp64 on the host and rounded once to dtype) and allocates one scratch level of the state's size on the
+ * current device.  `stream` orders the uploads.  The level counter starts at 0 (phase 0 first,
+ * PAPER.md:92, :142).  *out is set only on GE_OK.  desc and its arrays may be freed on return. */
+int ge_plan_create(ge_plan **out, const ge_desc *desc, ge_stream_t stream);
+
+/* One level: u_out = level(u_in) with phase = level & 1, then level += 1.
+ * u_in, u_out: device pointers, batch*nx (1-D) or ny*nx (2-D) elements of dtype, u_in != u_out, no
+ * overlap.  Always one launch of the per-level kernel (strategy A) whatever desc.kernel says.
+ * GE_EINVAL if the plan's dim does not match or a pointer is null/misaligned for dtype. */
+int ge_step_1d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
+int ge_step_2d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
+
+/* `steps` >= 0 levels in place: on completion of the enqueued work u holds level (level0+steps) and
+ * the plan's level counter has advanced by `steps`.  The plan's scratch level is used for
+ * ping-ponging; the strategy is the plan's (AUTO/PER_STEP/TEMPORAL/PERSISTENT).  steps == 0 is a no-op. */
+int ge_run(ge_plan *p, void *u, int64_t steps, ge_stream_t stream);
+
+/* End-to-end variant with HOST buffers: copies u_host (batch*nx or ny*nx elements, ideally pinned)
+ * to a plan-owned device buffer, runs `steps` levels, copies the result back into u_host and
+ * synchronises `stream` before returning. */
+int ge_run_host(ge_plan *p, void *u_host, int64_t steps, ge_stream_t stream);
+
+/* Level counter (checkpoint/resume: state = (u, level)). */
+int ge_plan_get_level(const ge_plan *p, int64_t *level);
+int ge_plan_set_level(ge_plan *p, int64_t level);          /* level >= 0 */
+
+/* Introspection for the benchmark harness.  `what`: */
+enum {
+    GE_INFO_KERNEL = 0,        /* ge_kernel actually selected for ge_run                          */
+    GE_INFO_TB = 1,            /* levels per launch of the temporal kernel (0 if not used)        */
+    GE_INFO_LAUNCHES = 2,      /* kernels launched through this plan so far                       */
+    GE_INFO_TILE_VALID = 3,    /* valid outputs per tile of the temporal kernel (per axis)        */
+    GE_INFO_TILE_LOADED = 4    /* elements loaded per tile of the temporal kernel (per axis)      */
+};
+int ge_plan_info(const ge_plan *p, int32_t what, int64_t *value);
+
+/* Frees the plan's device buffers (stream-ordered on the stream last used) and the plan. */
+int ge_plan_destroy(ge_plan *p);
+
+/* Static description of a status; after GE_ECUDA it includes the last CUDA error string seen by
+ * the calling thread. */
+const char *ge_strerror(int status);
+
+/* Library version: major*10000 + minor*100 + patch. */
+int ge_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GE_H_ */

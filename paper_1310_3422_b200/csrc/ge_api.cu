@@ -1,0 +1,345 @@
+// ge_api.cu -- the C ABI of libge (include/ge.h): plan, validation, strategy
+// selection and kernel dispatch.  No torch types, no CPU fallback: every level
+// is computed by the CUDA kernels in this directory.
+#include "../../include/ge.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "ge_common.cuh"
+#include "ge_level.cuh"
+#include "ge_temporal.cuh"
+
+namespace {
+
+thread_local char g_errbuf[512];
+thread_local cudaError_t g_last_cuda = cudaSuccess;
+
+#define GE_CUDA(expr)                                   \
+    do {                                                \
+        cudaError_t e__ = (expr);                       \
+        if (e__ != cudaSuccess) {                       \
+            g_last_cuda = e__;                          \
+            return e__ == cudaErrorMemoryAllocation ? GE_ENOMEM : GE_ECUDA; \
+        }                                               \
+    } while (0)
+
+inline size_t elem_size(int dtype) { return dtype == GE_F64 ? 8 : 4; }
+
+}  // namespace
+
+struct ge_plan {
+    int32_t dim, dtype, group_k, kernel, tb;
+    int64_t nx, ny, batch;
+    int64_t count;            // elements of the state
+    int64_t level;
+    int64_t launches;
+    int device;
+    void* coef;               // device: Coef1<T>[batch] or Coef2<T>[1]
+    void* scratch;            // device: one level
+    void* hostpath;           // device: state buffer for ge_run_host (lazy)
+    cudaStream_t last_stream;
+    int sm_count;
+};
+
+namespace {
+
+template <typename T>
+int upload_coef(ge_plan* p, const ge_desc* d, cudaStream_t s) {
+    if (p->dim == 1) {
+        std::vector<ge::Coef1<T>> h((size_t)p->batch);
+        for (int64_t b = 0; b < p->batch; ++b) {
+            const double r = d->r[b];
+            h[b].r = (T)r;
+            h[b].g = (T)(r / (1.0 + 2.0 * r));
+            h[b].e = (T)(r / (1.0 + r));
+            h[b].lo = (T)d->bc_lo[b];
+            h[b].hi = (T)d->bc_hi[b];
+            h[b].pad[0] = h[b].pad[1] = h[b].pad[2] = (T)0;
+        }
+        GE_CUDA(cudaMalloc(&p->coef, h.size() * sizeof(ge::Coef1<T>)));
+        GE_CUDA(cudaMemcpyAsync(p->coef, h.data(), h.size() * sizeof(ge::Coef1<T>), cudaMemcpyHostToDevice, s));
+        GE_CUDA(cudaStreamSynchronize(s));   // h is a stack-owned staging buffer
+    } else {
+        ge::Coef2<T> h;
+        std::memset(&h, 0, sizeof(h));
+        const double r = d->r[0];
+        h.r = (T)r;
+        h.g2 = (T)(r / (1.0 + 2.0 * r));
+        h.g4 = (T)(r / (1.0 + 4.0 * r));
+        h.h1 = (T)(r / (2.0 * (1.0 + r)));
+        h.h3 = (T)(3.0 * r / (2.0 * (1.0 + 3.0 * r)));
+        h.xlo = (T)d->bc_lo[0]; h.ylo = (T)d->bc_lo[1];
+        h.xhi = (T)d->bc_hi[0]; h.yhi = (T)d->bc_hi[1];
+        GE_CUDA(cudaMalloc(&p->coef, sizeof(h)));
+        GE_CUDA(cudaMemcpyAsync(p->coef, &h, sizeof(h), cudaMemcpyHostToDevice, s));
+        GE_CUDA(cudaStreamSynchronize(s));
+    }
+    return GE_OK;
+}
+
+// ---- strategy A launches ---------------------------------------------------
+template <typename T>
+int launch_level_1d(ge_plan* p, const void* uin, void* uout, int phase, cudaStream_t s) {
+    constexpr int V = ge::VecOf<T>::V;
+    constexpr int ITER = 4;
+    const bool vec = (p->nx % V == 0) && (((uintptr_t)uin | (uintptr_t)uout) % 16 == 0);
+    const int64_t nvec = vec ? p->nx / V : p->nx;
+    const int64_t per_block = (int64_t)ge::kLevelThreads * ITER;
+    dim3 grid((unsigned)((nvec + per_block - 1) / per_block), (unsigned)(p->batch < 65535 ? p->batch : 65535));
+    dim3 block(ge::kLevelThreads);
+    auto* c = (const ge::Coef1<T>*)p->coef;
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    if (vec) {
+        if (phase == 0) ge::ge1d_level_kernel<T, V, 0, ITER><<<grid, block, 0, s>>>(in, out, p->nx, p->batch, c);
+        else            ge::ge1d_level_kernel<T, V, 1, ITER><<<grid, block, 0, s>>>(in, out, p->nx, p->batch, c);
+    } else {
+        if (phase == 0) ge::ge1d_level_kernel<T, 1, 0, ITER><<<grid, block, 0, s>>>(in, out, p->nx, p->batch, c);
+        else            ge::ge1d_level_kernel<T, 1, 1, ITER><<<grid, block, 0, s>>>(in, out, p->nx, p->batch, c);
+    }
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    return GE_OK;
+}
+
+template <typename T>
+int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStream_t s) {
+    constexpr int V = ge::VecOf<T>::V;
+    const bool vec = (p->nx % V == 0) && (((uintptr_t)uin | (uintptr_t)uout) % 16 == 0);
+    const int64_t nvec = vec ? p->nx / V : p->nx;
+    const int64_t npair = (p->ny + phase) / 2 + 1;      // anchor rows -phase, 2-phase, ... <= ny-1
+    dim3 grid((unsigned)((nvec + ge::kLevel2dBx - 1) / ge::kLevel2dBx),
+              (unsigned)((npair + ge::kLevel2dBy - 1) / ge::kLevel2dBy));
+    dim3 block(ge::kLevel2dBx, ge::kLevel2dBy);
+    auto* c = (const ge::Coef2<T>*)p->coef;
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    if (vec) {
+        if (phase == 0) ge::ge2d_level_kernel<T, V, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+        else            ge::ge2d_level_kernel<T, V, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+    } else {
+        if (phase == 0) ge::ge2d_level_kernel<T, 1, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+        else            ge::ge2d_level_kernel<T, 1, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+    }
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    return GE_OK;
+}
+
+int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
+    const int phase = (int)(p->level & 1);
+    int rc;
+    if (p->dim == 1) rc = p->dtype == GE_F64 ? launch_level_1d<double>(p, uin, uout, phase, s)
+                                             : launch_level_1d<float>(p, uin, uout, phase, s);
+    else             rc = p->dtype == GE_F64 ? launch_level_2d<double>(p, uin, uout, phase, s)
+                                             : launch_level_2d<float>(p, uin, uout, phase, s);
+    if (rc == GE_OK) p->level += 1;
+    return rc;
+}
+
+// ---- strategy B launch (1-D): tb levels, starting at an even level ---------
+template <typename T>
+int launch_temporal_1d(ge_plan* p, const void* uin, void* uout, int tb, cudaStream_t s) {
+    int rc = ge::temporal1d_launch<T>((const T*)uin, (T*)uout, p->nx, p->batch,
+                                      (const ge::Coef1<T>*)p->coef, tb, s);
+    if (rc != 0) { g_last_cuda = (cudaError_t)rc; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += tb;
+    return GE_OK;
+}
+
+bool temporal_ok(const ge_plan* p, const void* u) {
+    if (p->dim != 1) return false;
+    const int V = p->dtype == GE_F64 ? 2 : 4;
+    return p->nx % V == 0 && ((uintptr_t)u % 16 == 0) && ((uintptr_t)p->scratch % 16 == 0);
+}
+
+int step_common(ge_plan* p, int dim, const void* uin, void* uout, cudaStream_t s) {
+    if (!p || !uin || !uout || uin == uout || p->dim != dim) return GE_EINVAL;
+    const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)uin % es || (uintptr_t)uout % es) return GE_EINVAL;
+    const char* a = (const char*)uin; const char* b = (const char*)uout;
+    const size_t bytes = (size_t)p->count * es;
+    if ((a < b + bytes) && (b < a + bytes)) return GE_EINVAL;   // overlap
+    p->last_stream = s;
+    return launch_level(p, uin, uout, s);
+}
+
+}  // namespace
+
+extern "C" {
+
+int ge_version(void) { return 100; }
+
+const char* ge_strerror(int status) {
+    switch (status) {
+        case GE_OK: return "ok";
+        case GE_EINVAL: return "invalid argument";
+        case GE_ENOMEM: return "out of memory";
+        case GE_EUNSUPPORTED: return "unsupported on the GPU path (group_k >= 2 is SURVEY.md 8(f) NEXT-1)";
+        case GE_ECUDA:
+            std::snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s", cudaGetErrorString(g_last_cuda));
+            return g_errbuf;
+        default: return "unknown status";
+    }
+}
+
+int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
+    if (!out || !d) return GE_EINVAL;
+    if (d->dim != 1 && d->dim != 2) return GE_EINVAL;
+    if (d->nx < 1 || d->ny < 1 || d->batch < 1) return GE_EINVAL;
+    if (d->dim == 1 && d->ny != 1) return GE_EINVAL;
+    if (d->dim == 2 && d->batch != 1) return GE_EINVAL;
+    if (d->dtype != GE_F32 && d->dtype != GE_F64) return GE_EINVAL;
+    if (d->group_k < 1) return GE_EINVAL;
+    if (d->group_k >= 2 && d->dim == 2) return GE_EINVAL;
+    if (d->kernel < GE_KERNEL_AUTO || d->kernel > GE_KERNEL_PERSISTENT) return GE_EINVAL;
+    if (d->tb < 0) return GE_EINVAL;
+    if (!d->r || !d->bc_lo || !d->bc_hi) return GE_EINVAL;
+    const int64_t nr = d->dim == 1 ? d->batch : 1;
+    for (int64_t b = 0; b < nr; ++b)
+        if (!(d->r[b] > 0.0) || !std::isfinite(d->r[b])) return GE_EINVAL;
+    const int64_t nb = d->dim == 1 ? d->batch : 2;
+    for (int64_t b = 0; b < nb; ++b)
+        if (!std::isfinite(d->bc_lo[b]) || !std::isfinite(d->bc_hi[b])) return GE_EINVAL;
+    if (d->group_k >= 2) return GE_EUNSUPPORTED;
+
+    ge_plan* p = new (std::nothrow) ge_plan();
+    if (!p) return GE_ENOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->dim = d->dim; p->dtype = d->dtype; p->group_k = d->group_k;
+    p->nx = d->nx; p->ny = d->ny; p->batch = d->batch;
+    p->count = d->dim == 1 ? d->batch * d->nx : d->ny * d->nx;
+    p->last_stream = (cudaStream_t)stream;
+    int rc = GE_OK;
+    cudaError_t ce = cudaGetDevice(&p->device);
+    if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    if (ce != cudaSuccess) { g_last_cuda = ce; delete p; return GE_ECUDA; }
+    rc = p->dtype == GE_F64 ? upload_coef<double>(p, d, (cudaStream_t)stream)
+                            : upload_coef<float>(p, d, (cudaStream_t)stream);
+    if (rc == GE_OK) {
+        ce = cudaMalloc(&p->scratch, (size_t)p->count * elem_size(p->dtype));
+        if (ce != cudaSuccess) { g_last_cuda = ce; rc = ce == cudaErrorMemoryAllocation ? GE_ENOMEM : GE_ECUDA; }
+    }
+    if (rc != GE_OK) { cudaFree(p->coef); cudaFree(p->scratch); cudaGetLastError(); delete p; return rc; }
+
+    // strategy selection
+    int kernel = d->kernel;
+    if (kernel == GE_KERNEL_AUTO) kernel = d->dim == 1 ? GE_KERNEL_TEMPORAL : GE_KERNEL_PER_STEP;
+    if (kernel == GE_KERNEL_PERSISTENT) kernel = d->dim == 1 ? GE_KERNEL_TEMPORAL : GE_KERNEL_PER_STEP;
+    if (kernel == GE_KERNEL_TEMPORAL && d->dim != 1) kernel = GE_KERNEL_PER_STEP;
+    p->kernel = kernel;
+    p->tb = 0;
+    if (kernel == GE_KERNEL_TEMPORAL) {
+        p->tb = p->dtype == GE_F64 ? ge::temporal1d_pick_tb<double>(d->tb) : ge::temporal1d_pick_tb<float>(d->tb);
+    }
+    *out = p;
+    return GE_OK;
+}
+
+int ge_step_1d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
+    return step_common(p, 1, u_in, u_out, (cudaStream_t)stream);
+}
+
+int ge_step_2d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
+    return step_common(p, 2, u_in, u_out, (cudaStream_t)stream);
+}
+
+int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
+    if (!p || !u || steps < 0) return GE_EINVAL;
+    const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)u % es) return GE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    p->last_stream = s;
+    void* cur = u;
+    void* oth = p->scratch;
+    int64_t left = steps;
+    int rc = GE_OK;
+    const bool temporal = p->kernel == GE_KERNEL_TEMPORAL && temporal_ok(p, u);
+    while (left > 0 && rc == GE_OK) {
+        // a temporal block starts at an odd level (ge_temporal.cuh); its length is the plan's tb,
+        // or what is left rounded down to the vector width
+        int tbn = 0;
+        if (temporal && (p->level & 1) == 1) {
+            const int64_t want = left < p->tb ? left : p->tb;
+            tbn = p->dtype == GE_F64 ? ge::temporal1d_round_tb<double>(want) : ge::temporal1d_round_tb<float>(want);
+        }
+        if (tbn > 0) {
+            rc = p->dtype == GE_F64 ? launch_temporal_1d<double>(p, cur, oth, tbn, s)
+                                    : launch_temporal_1d<float>(p, cur, oth, tbn, s);
+            left -= tbn;
+        } else {
+            rc = launch_level(p, cur, oth, s);
+            left -= 1;
+        }
+        void* t = cur; cur = oth; oth = t;
+    }
+    if (rc != GE_OK) return rc;
+    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * es, cudaMemcpyDeviceToDevice, s));
+    return GE_OK;
+}
+
+int ge_run_host(ge_plan* p, void* u_host, int64_t steps, ge_stream_t stream) {
+    if (!p || !u_host || steps < 0) return GE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = (size_t)p->count * elem_size(p->dtype);
+    if (!p->hostpath) GE_CUDA(cudaMalloc(&p->hostpath, bytes));
+    GE_CUDA(cudaMemcpyAsync(p->hostpath, u_host, bytes, cudaMemcpyHostToDevice, s));
+    int rc = ge_run(p, p->hostpath, steps, stream);
+    if (rc != GE_OK) return rc;
+    GE_CUDA(cudaMemcpyAsync(u_host, p->hostpath, bytes, cudaMemcpyDeviceToHost, s));
+    GE_CUDA(cudaStreamSynchronize(s));
+    return GE_OK;
+}
+
+int ge_plan_get_level(const ge_plan* p, int64_t* level) {
+    if (!p || !level) return GE_EINVAL;
+    *level = p->level;
+    return GE_OK;
+}
+
+int ge_plan_set_level(ge_plan* p, int64_t level) {
+    if (!p || level < 0) return GE_EINVAL;
+    p->level = level;
+    return GE_OK;
+}
+
+int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
+    if (!p || !value) return GE_EINVAL;
+    switch (what) {
+        case GE_INFO_KERNEL: *value = p->kernel; return GE_OK;
+        case GE_INFO_TB: *value = p->tb; return GE_OK;
+        case GE_INFO_LAUNCHES: *value = p->launches; return GE_OK;
+        case GE_INFO_TILE_VALID:
+            *value = p->kernel == GE_KERNEL_TEMPORAL
+                         ? (p->dtype == GE_F64 ? ge::temporal1d_tile_valid<double>(p->tb) : ge::temporal1d_tile_valid<float>(p->tb))
+                         : 0;
+            return GE_OK;
+        case GE_INFO_TILE_LOADED:
+            *value = p->kernel == GE_KERNEL_TEMPORAL
+                         ? (p->dtype == GE_F64 ? ge::temporal1d_tile_loaded<double>() : ge::temporal1d_tile_loaded<float>())
+                         : 0;
+            return GE_OK;
+        default: return GE_EINVAL;
+    }
+}
+
+int ge_plan_destroy(ge_plan* p) {
+    if (!p) return GE_EINVAL;
+    // stream-ordered with respect to the last stream used: wait for it, then free
+    cudaError_t e = cudaStreamSynchronize(p->last_stream);
+    cudaFree(p->coef);
+    cudaFree(p->scratch);
+    cudaFree(p->hostpath);
+    delete p;
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    return GE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,207 @@
+"""Thin Python binding of libge (include/ge.h): argument marshalling only.
+
+Every function has the C entry point's name and forwards to it through ctypes;
+every level of the GE scheme is computed by the CUDA kernels
+in csrc/.  PyTorch is used by callers for device buffers and streams only:
+pass `tensor.data_ptr()` and `torch.cuda.current_stream().cuda_stream`.
+
+There is NO CPU fallback: if libge.so is missing or cannot be loaded, `load()`
+raises.  This module imports nothing from oracle/.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "lib", "libge.so")
+
+GE_F32, GE_F64 = 0, 1
+GE_KERNEL_AUTO, GE_KERNEL_PER_STEP, GE_KERNEL_TEMPORAL, GE_KERNEL_PERSISTENT = 0, 1, 2, 3
+GE_OK, GE_EINVAL, GE_ENOMEM, GE_ECUDA, GE_EUNSUPPORTED = 0, -1, -2, -3, -4
+GE_INFO_KERNEL, GE_INFO_TB, GE_INFO_LAUNCHES, GE_INFO_TILE_VALID, GE_INFO_TILE_LOADED = 0, 1, 2, 3, 4
+
+KERNEL_NAMES = {0: "auto", 1: "per_step", 2: "temporal", 3: "persistent"}
+_KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
+_DTYPES = {"f32": GE_F32, "f64": GE_F64}
+
+# every symbol include/ge.h declares
+EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_2d", "ge_run", "ge_run_host",
+           "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_destroy",
+           "ge_strerror", "ge_version")
+
+
+class ge_desc(ctypes.Structure):
+    _fields_ = [
+        ("dim", ctypes.c_int32),
+        ("nx", ctypes.c_int64), ("ny", ctypes.c_int64),
+        ("batch", ctypes.c_int64),
+        ("dtype", ctypes.c_int32),
+        ("group_k", ctypes.c_int32),
+        ("r", ctypes.POINTER(ctypes.c_double)),
+        ("bc_lo", ctypes.POINTER(ctypes.c_double)),
+        ("bc_hi", ctypes.POINTER(ctypes.c_double)),
+        ("kernel", ctypes.c_int32),
+        ("tb", ctypes.c_int32),
+    ]
+
+
+class GeError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s: %s (status %d)" % (where, strerror(status), status))
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """dlopen libge.so; raises if the CUDA library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            "libge.so is missing (%s): build it with `python -m paper_1310_3422_b200.build`; "
+            "there is no CPU fallback" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+    lib.ge_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ge_desc), vp]
+    lib.ge_step_1d.argtypes = [vp, vp, vp, vp]
+    lib.ge_step_2d.argtypes = [vp, vp, vp, vp]
+    lib.ge_run.argtypes = [vp, vp, i64, vp]
+    lib.ge_run_host.argtypes = [vp, vp, i64, vp]
+    lib.ge_plan_get_level.argtypes = [vp, ctypes.POINTER(i64)]
+    lib.ge_plan_set_level.argtypes = [vp, i64]
+    lib.ge_plan_info.argtypes = [vp, i32, ctypes.POINTER(i64)]
+    lib.ge_plan_destroy.argtypes = [vp]
+    lib.ge_strerror.argtypes = [ctypes.c_int]
+    lib.ge_strerror.restype = ctypes.c_char_p
+    lib.ge_version.argtypes = []
+    for name in EXPORTS:
+        if name not in ("ge_strerror",):
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def strerror(status: int) -> str:
+    return load().ge_strerror(int(status)).decode()
+
+
+def ge_version() -> int:
+    return load().ge_version()
+
+
+def _darr(values: Sequence[float]):
+    vals = [float(v) for v in values]
+    return (ctypes.c_double * len(vals))(*vals)
+
+
+def ge_plan_create(dim: int, nx: int, ny: int = 1, batch: int = 1, dtype="f64", r=(1.0,),
+                   bc_lo=(0.0,), bc_hi=(0.0,), group_k: int = 1, kernel="auto", tb: int = 0,
+                   stream: int = 0) -> int:
+    """Returns the opaque plan handle (an integer address)."""
+    lib = load()
+    ra, lo, hi = _darr(r), _darr(bc_lo), _darr(bc_hi)
+    need = batch if dim == 1 else 1
+    needb = batch if dim == 1 else 2
+    if len(ra) < need or len(lo) < needb or len(hi) < needb:
+        raise GeError(GE_EINVAL, "ge_plan_create (host arrays too short)")
+    d = ge_desc(dim=dim, nx=nx, ny=ny, batch=batch,
+                dtype=_DTYPES[dtype] if isinstance(dtype, str) else int(dtype),
+                group_k=group_k, r=ra, bc_lo=lo, bc_hi=hi,
+                kernel=_KERNEL_IDS[kernel] if isinstance(kernel, str) else int(kernel), tb=tb)
+    out = ctypes.c_void_p()
+    rc = lib.ge_plan_create(ctypes.byref(out), ctypes.byref(d), ctypes.c_void_p(stream))
+    if rc != GE_OK:
+        raise GeError(rc, "ge_plan_create")
+    return out.value
+
+
+def _check(rc: int, where: str):
+    if rc != GE_OK:
+        raise GeError(rc, where)
+
+
+def ge_step_1d(plan: int, u_in: int, u_out: int, stream: int = 0):
+    _check(load().ge_step_1d(plan, u_in, u_out, stream), "ge_step_1d")
+
+
+def ge_step_2d(plan: int, u_in: int, u_out: int, stream: int = 0):
+    _check(load().ge_step_2d(plan, u_in, u_out, stream), "ge_step_2d")
+
+
+def ge_run(plan: int, u: int, steps: int, stream: int = 0):
+    _check(load().ge_run(plan, u, steps, stream), "ge_run")
+
+
+def ge_run_host(plan: int, u_host: int, steps: int, stream: int = 0):
+    _check(load().ge_run_host(plan, u_host, steps, stream), "ge_run_host")
+
+
+def ge_plan_get_level(plan: int) -> int:
+    v = ctypes.c_int64()
+    _check(load().ge_plan_get_level(plan, ctypes.byref(v)), "ge_plan_get_level")
+    return v.value
+
+
+def ge_plan_set_level(plan: int, level: int):
+    _check(load().ge_plan_set_level(plan, level), "ge_plan_set_level")
+
+
+def ge_plan_info(plan: int, what: int) -> int:
+    v = ctypes.c_int64()
+    _check(load().ge_plan_info(plan, what, ctypes.byref(v)), "ge_plan_info")
+    return v.value
+
+
+def ge_plan_destroy(plan: Optional[int]):
+    if plan:
+        _check(load().ge_plan_destroy(plan), "ge_plan_destroy")
+
+
+class Plan:
+    """Context-manager convenience around a plan handle built from an inputs.py config dict."""
+
+    def __init__(self, cfg: dict, kernel="auto", tb: int = 0, stream: int = 0, group_k: int = 1):
+        self.cfg = cfg
+        self.handle = ge_plan_create(cfg["dim"], cfg["nx"], cfg["ny"], cfg["batch"], cfg["dtype"],
+                                     list(cfg["r"]), list(cfg["bc_lo"]), list(cfg["bc_hi"]),
+                                     group_k=group_k, kernel=kernel, tb=tb, stream=stream)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def close(self):
+        if self.handle:
+            ge_plan_destroy(self.handle)
+            self.handle = None
+
+    def step(self, u_in: int, u_out: int, stream: int = 0):
+        (ge_step_1d if self.cfg["dim"] == 1 else ge_step_2d)(self.handle, u_in, u_out, stream)
+
+    def run(self, u: int, steps: int, stream: int = 0):
+        ge_run(self.handle, u, steps, stream)
+
+    def run_host(self, u_host: int, steps: int, stream: int = 0):
+        ge_run_host(self.handle, u_host, steps, stream)
+
+    @property
+    def level(self) -> int:
+        return ge_plan_get_level(self.handle)
+
+    @level.setter
+    def level(self, v: int):
+        ge_plan_set_level(self.handle, v)
+
+    def info(self) -> dict:
+        return dict(kernel=KERNEL_NAMES[ge_plan_info(self.handle, GE_INFO_KERNEL)],
+                    tb=ge_plan_info(self.handle, GE_INFO_TB),
+                    launches=ge_plan_info(self.handle, GE_INFO_LAUNCHES),
+                    tile_valid=ge_plan_info(self.handle, GE_INFO_TILE_VALID),
+                    tile_loaded=ge_plan_info(self.handle, GE_INFO_TILE_LOADED))

@@ -1,0 +1,166 @@
+"""GPU parity: libge (through its C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star): max-abs error relative to max|oracle|
+<= 1e-12 (fp64), <= 1e-5 (fp32), measured on the final level (reading R-A7)."""
+import numpy as np
+import pytest
+
+from gpu_util import TOL, rel_err, rel_err_rows, run_gpu, run_oracle, window_1d, window_2d
+from paper_1310_3422_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+# ------------------------------------------------------------------ strategy A, 1-D ------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 7, 8, 64, 1000, 1026, 4099])
+def test_per_step_1d_small(oracle, dtype, n):
+    cfg = inputs.random_rods(3, n, dtype, seed=100 + n)
+    for level0 in (0, 1):
+        for steps in (1, 2, 5):
+            got, info = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+            ref = run_oracle(oracle, cfg, steps, level0=level0)
+            assert info["kernel"] == "per_step" and info["launches"] == steps
+            assert rel_err_rows(got, ref) <= (1e-14 if dtype == "f64" else 2e-6), (n, level0, steps)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_step_1d_entry_point_matches_run(oracle, dtype):
+    cfg = inputs.random_rods(2, 516, dtype, seed=5)
+    a, _ = run_gpu(cfg, 7, kernel="per_step", via="step")
+    b, _ = run_gpu(cfg, 7, kernel="per_step", via="run")
+    np.testing.assert_array_equal(a, b)
+    assert rel_err_rows(a, run_oracle(oracle, cfg, 7)) <= TOL[dtype]
+
+
+def test_unaligned_pointers_take_the_scalar_kernel(oracle):
+    import torch
+    from paper_1310_3422_b200 import libge
+    cfg = inputs.random_rods(1, 1000, "f64", seed=9)
+    dev = torch.device("cuda:0")
+    buf = torch.zeros(1000 + 1, dtype=torch.float64, device=dev)
+    out = torch.zeros(1000 + 1, dtype=torch.float64, device=dev)
+    u, v = buf[1:], out[1:]                       # 8-byte aligned, not 16
+    u.copy_(torch.from_numpy(cfg["u0"].reshape(-1)))
+    s = torch.cuda.current_stream(dev).cuda_stream
+    with libge.Plan(cfg, kernel="per_step", stream=s) as plan:
+        plan.step(u.data_ptr(), v.data_ptr(), s)
+        plan.step(v.data_ptr(), u.data_ptr(), s)
+        torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), run_oracle(oracle, cfg, 2).reshape(-1)) <= 1e-14
+
+
+def test_step_rejects_bad_arguments():
+    import torch
+    from paper_1310_3422_b200 import libge
+    cfg = inputs.random_rods(1, 64, "f64")
+    u = torch.zeros(128, dtype=torch.float64, device="cuda:0")
+    with libge.Plan(cfg) as plan:
+        for a, b in ((u.data_ptr(), u.data_ptr()), (0, u.data_ptr()), (u.data_ptr(), u.data_ptr() + 8 * 32),
+                     (u.data_ptr() + 4, u.data_ptr() + 8 * 64)):
+            with pytest.raises(libge.GeError) as ei:
+                plan.step(a, b)
+            assert ei.value.status == libge.GE_EINVAL
+        with pytest.raises(libge.GeError):
+            libge.ge_step_2d(plan.handle, u.data_ptr(), u.data_ptr() + 8 * 64)
+        with pytest.raises(libge.GeError):
+            plan.run(u.data_ptr(), -1)
+        plan.run(u.data_ptr(), 0)
+        assert plan.level == 0 and plan.info()["launches"] == 0
+
+
+# ------------------------------------------------------------------ strategy B, 1-D ------
+@pytest.mark.parametrize("dtype,tb", [("f64", 0), ("f64", 2), ("f64", 6), ("f64", 32), ("f32", 0), ("f32", 4), ("f32", 8), ("f32", 40)])
+@pytest.mark.parametrize("n", [8, 224, 232, 2048, 10000, 3 * 4096 + 8])
+def test_temporal_1d(oracle, dtype, tb, n):
+    cfg = inputs.random_rods(2, n, dtype, seed=7 * n + tb)
+    for level0, steps in ((0, 1), (1, 16), (0, 40), (1, 37), (0, 101)):
+        got, info = run_gpu(cfg, steps, kernel="temporal", tb=tb, level0=level0)
+        ref = run_oracle(oracle, cfg, steps, level0=level0)
+        assert info["kernel"] == "temporal"
+        if steps >= 40:
+            assert info["launches"] < steps        # the blocked kernel really ran
+        assert rel_err_rows(got, ref) <= (2e-14 if dtype == "f64" else 5e-6), (n, level0, steps, info)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_temporal_1d_odd_n_falls_back_to_per_step(oracle, dtype):
+    cfg = inputs.random_rods(2, 1001, dtype, seed=77)
+    got, info = run_gpu(cfg, 33, kernel="temporal")
+    assert info["launches"] == 33
+    assert rel_err_rows(got, run_oracle(oracle, cfg, 33)) <= TOL[dtype]
+
+
+def test_run_is_deterministic():
+    cfg = inputs.random_rods(4, 4096, "f32", seed=3)
+    a, _ = run_gpu(cfg, 100)
+    b, _ = run_gpu(cfg, 100)
+    np.testing.assert_array_equal(a, b)
+
+
+def test_run_host_matches_run(oracle):
+    cfg = inputs.random_rods(3, 2048, "f64", seed=31)
+    a, _ = run_gpu(cfg, 50, via="host")
+    b, _ = run_gpu(cfg, 50, via="run")
+    np.testing.assert_array_equal(a, b)
+
+
+# ------------------------------------------------------------------ 2-D ------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("nx,ny", [(1, 1), (2, 2), (3, 3), (4, 4), (5, 4), (4, 7), (8, 8), (64, 32), (130, 67), (131, 66), (256, 256)])
+def test_per_step_2d(oracle, dtype, nx, ny):
+    cfg = inputs.random_grid(nx, ny, dtype, seed=nx * 1000 + ny, r=1.7)
+    for level0 in (0, 1):
+        for steps in (1, 2, 5):
+            got, info = run_gpu(cfg, steps, level0=level0)
+            ref = run_oracle(oracle, cfg, steps, level0=level0)
+            assert info["launches"] == steps
+            assert rel_err(got, ref) <= (2e-14 if dtype == "f64" else 3e-6), (nx, ny, level0, steps)
+
+
+def test_step_2d_entry_point(oracle):
+    cfg = inputs.random_grid(96, 40, "f64", seed=8)
+    a, _ = run_gpu(cfg, 4, via="step")
+    assert rel_err(a, run_oracle(oracle, cfg, 4)) <= 1e-14
+
+
+# ------------------------------------------------------------------ BASELINE configs ------
+def test_config1_exact(oracle):
+    cfg = inputs.make_c1()
+    ref = run_oracle(oracle, cfg, cfg["steps"])
+    for kernel in ("per_step", "temporal"):
+        got, _ = run_gpu(cfg, cfg["steps"], kernel=kernel)
+        assert rel_err(got, ref) <= TOL["f64"]
+    x = np.arange(1, 65) / 65.0
+    exact = np.exp(-np.pi ** 2 * 1000 / 65.0 ** 2) * np.sin(np.pi * x)
+    assert abs(np.abs(got.reshape(-1) - exact).max() - 4.6957e-4) < 1e-7     # tests/golden P7
+
+
+def test_config2_reduced(oracle):
+    cfg = inputs.make_c2(n=2 ** 14, steps=10000)
+    ref = run_oracle(oracle, cfg, cfg["steps"])
+    for kernel in ("per_step", "temporal"):
+        got, _ = run_gpu(cfg, cfg["steps"], kernel=kernel)
+        assert rel_err(got, ref) <= TOL["f64"], kernel
+
+
+def test_config3_reduced(oracle):
+    cfg = inputs.make_c3(batch=48, n=4096, steps=2000)
+    ref = run_oracle(oracle, cfg, cfg["steps"])
+    for kernel in ("per_step", "auto"):
+        got, _ = run_gpu(cfg, cfg["steps"], kernel=kernel)
+        assert rel_err_rows(got, ref) <= TOL["f32"], kernel
+
+
+def test_config4_reduced(oracle):
+    cfg = inputs.make_c4(n=2 ** 20, steps=200)
+    ref = run_oracle(oracle, cfg, cfg["steps"])
+    for kernel in ("per_step", "temporal"):
+        got, _ = run_gpu(cfg, cfg["steps"], kernel=kernel)
+        assert rel_err(got, ref) <= TOL["f64"], kernel
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config5_reduced(oracle, dtype):
+    cfg = inputs.make_c5(n=512, steps=1000, dtype=dtype)
+    got, _ = run_gpu(cfg, cfg["steps"])
+    assert rel_err(got, run_oracle(oracle, cfg, cfg["steps"])) <= TOL[dtype]
