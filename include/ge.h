@@ -73,7 +73,8 @@ typedef struct {
     const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; copied  */
     const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; copied  */
     int32_t   kernel;     /* ge_kernel                                                                 */
-    int32_t   tb;         /* levels per launch for TEMPORAL (0 = auto); ignored otherwise              */
+    int32_t   tb;         /* levels per launch for TEMPORAL (0 = auto; any value >= 1, both starting
+                             phases are handled in-kernel); ignored otherwise                          */
 } ge_desc;
 
 /* Create a plan: validates desc, uploads per-rod coefficients (r, r/(1+2r), r/(1+r), ... computed in
@@ -112,6 +113,16 @@ enum {
     GE_INFO_TILE_LOADED = 4    /* elements loaded per tile of the temporal kernel (per axis)      */
 };
 int ge_plan_info(const ge_plan *p, int32_t what, int64_t *value);
+
+/* Tuning knobs of the temporally blocked kernel (benchmark sweeps; defaults are picked at create).
+ * GE_EINVAL for a value the kernels are not instantiated for; nothing is enqueued. */
+enum {
+    GE_TUNE_TEMPORAL_C = 0,    /* values per lane of the 1-D temporal kernel: 8 or 16 (f64), 16 or 32 (f32) */
+    GE_TUNE_TB = 1,            /* levels per launch (1-D: >= 1, clamped to the largest the tile allows;
+                                  2-D: one of the compiled-in block lengths 4, 8)                            */
+    GE_TUNE_SEG_PAIRS = 2      /* 2-D temporal kernel: output row pairs per warp segment (default 64)       */
+};
+int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
 
 /* Frees the plan's device buffers (stream-ordered on the stream last used) and the plan. */
 int ge_plan_destroy(ge_plan *p);

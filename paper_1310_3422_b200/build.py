@@ -20,6 +20,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
+    "-fmad=false",            # every fma in the kernels is written out; no implicit contraction
     "-Xcompiler", "-fPIC", "-shared",
     "-cudart", "static",
 ]

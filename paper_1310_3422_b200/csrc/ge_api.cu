@@ -14,6 +14,7 @@
 #include "ge_common.cuh"
 #include "ge_level.cuh"
 #include "ge_temporal.cuh"
+#include "ge_temporal2d.cuh"
 
 namespace {
 
@@ -35,6 +36,8 @@ inline size_t elem_size(int dtype) { return dtype == GE_F64 ? 8 : 4; }
 
 struct ge_plan {
     int32_t dim, dtype, group_k, kernel, tb;
+    int32_t tc;               // values per lane of the temporal kernel
+    int32_t hp;               // 2-D temporal kernel: output row pairs per segment
     int64_t nx, ny, batch;
     int64_t count;            // elements of the state
     int64_t level;
@@ -143,21 +146,56 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     return rc;
 }
 
-// ---- strategy B launch (1-D): tb levels, starting at an even level ---------
+// ---- strategy B launch (1-D): tb levels from the plan's current level (any phase) ----
 template <typename T>
 int launch_temporal_1d(ge_plan* p, const void* uin, void* uout, int tb, cudaStream_t s) {
-    int rc = ge::temporal1d_launch<T>((const T*)uin, (T*)uout, p->nx, p->batch,
-                                      (const ge::Coef1<T>*)p->coef, tb, s);
-    if (rc != 0) { g_last_cuda = (cudaError_t)rc; return GE_ECUDA; }
+    const int phase = (int)(p->level & 1);
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    auto* c = (const ge::Coef1<T>*)p->coef;
+    cudaError_t e;
+    constexpr int C0 = 16 / (int)sizeof(T) * 4;     // 8 (f64) / 16 (f32)
+    switch (p->tc) {
+        case C0:     e = ge::temporal1d_launch<T, C0>(in, out, p->nx, p->batch, c, tb, phase, s); break;
+        case 2 * C0: e = ge::temporal1d_launch<T, 2 * C0>(in, out, p->nx, p->batch, c, tb, phase, s); break;
+        default: return GE_EINVAL;
+    }
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     p->launches += 1;
     p->level += tb;
     return GE_OK;
 }
 
+// ---- strategy B launch (2-D): plan->tb levels (a compiled-in block length) from the current level ----
+template <typename T>
+int launch_temporal_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
+    const int phase = (int)(p->level & 1);
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    auto* c = (const ge::Coef2<T>*)p->coef;
+    cudaError_t e;
+    switch (p->tb) {
+        case 4: e = ge::temporal2d_launch<T, 4, 4>(in, out, p->nx, p->ny, c, phase, p->hp, s); break;
+        case 8: e = ge::temporal2d_launch<T, 4, 8>(in, out, p->nx, p->ny, c, phase, p->hp, s); break;
+        default: return GE_EINVAL;
+    }
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += p->tb;
+    return GE_OK;
+}
+bool temporal2d_tb_ok(int64_t tb) { return tb == 4 || tb == 8; }
+
 bool temporal_ok(const ge_plan* p, const void* u) {
-    if (p->dim != 1) return false;
+    if (p->dim == 2 && (p->nx >= (1 << 30) || p->ny >= (1 << 30))) return false;
     const int V = p->dtype == GE_F64 ? 2 : 4;
     return p->nx % V == 0 && ((uintptr_t)u % 16 == 0) && ((uintptr_t)p->scratch % 16 == 0);
+}
+
+int default_tc(int dtype) { return dtype == GE_F64 ? 16 : 32; }
+int clamp_tb(const ge_plan* p, int64_t tb) {
+    const int mx = ge::temporal1d_max_tb(p->tc);
+    return (int)(tb > mx ? mx : tb);
 }
 
 int step_common(ge_plan* p, int dim, const void* uin, void* uout, cudaStream_t s) {
@@ -231,13 +269,17 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
 
     // strategy selection
     int kernel = d->kernel;
-    if (kernel == GE_KERNEL_AUTO) kernel = d->dim == 1 ? GE_KERNEL_TEMPORAL : GE_KERNEL_PER_STEP;
-    if (kernel == GE_KERNEL_PERSISTENT) kernel = d->dim == 1 ? GE_KERNEL_TEMPORAL : GE_KERNEL_PER_STEP;
-    if (kernel == GE_KERNEL_TEMPORAL && d->dim != 1) kernel = GE_KERNEL_PER_STEP;
+    if (kernel == GE_KERNEL_AUTO) kernel = GE_KERNEL_TEMPORAL;
+    if (kernel == GE_KERNEL_PERSISTENT) kernel = GE_KERNEL_TEMPORAL;
     p->kernel = kernel;
     p->tb = 0;
-    if (kernel == GE_KERNEL_TEMPORAL) {
-        p->tb = p->dtype == GE_F64 ? ge::temporal1d_pick_tb<double>(d->tb) : ge::temporal1d_pick_tb<float>(d->tb);
+    p->tc = default_tc(p->dtype);
+    p->hp = 64;
+    if (kernel == GE_KERNEL_TEMPORAL && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : 16);
+    if (kernel == GE_KERNEL_TEMPORAL && d->dim == 2) {
+        p->tc = 4;
+        p->tb = d->tb > 0 ? d->tb : 8;
+        if (!temporal2d_tb_ok(p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
     }
     *out = p;
     return GE_OK;
@@ -263,14 +305,19 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     int rc = GE_OK;
     const bool temporal = p->kernel == GE_KERNEL_TEMPORAL && temporal_ok(p, u);
     while (left > 0 && rc == GE_OK) {
-        // a temporal block starts at an odd level (ge_temporal.cuh); its length is the plan's tb,
-        // or what is left rounded down to the vector width
-        int tbn = 0;
-        if (temporal && (p->level & 1) == 1) {
-            const int64_t want = left < p->tb ? left : p->tb;
-            tbn = p->dtype == GE_F64 ? ge::temporal1d_round_tb<double>(want) : ge::temporal1d_round_tb<float>(want);
-        }
-        if (tbn > 0) {
+        if (temporal && p->dim == 2) {
+            if (left >= p->tb) {
+                rc = p->dtype == GE_F64 ? launch_temporal_2d<double>(p, cur, oth, s)
+                                        : launch_temporal_2d<float>(p, cur, oth, s);
+                left -= p->tb;
+            } else {
+                rc = launch_level(p, cur, oth, s);
+                left -= 1;
+            }
+        } else if (temporal) {
+            // equal-sized blocks: ceil(left / tb) launches of (almost) the same number of levels
+            const int64_t nl = (left + p->tb - 1) / p->tb;
+            const int tbn = (int)((left + nl - 1) / nl);
             rc = p->dtype == GE_F64 ? launch_temporal_1d<double>(p, cur, oth, tbn, s)
                                     : launch_temporal_1d<float>(p, cur, oth, tbn, s);
             left -= tbn;
@@ -317,14 +364,40 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
         case GE_INFO_TB: *value = p->tb; return GE_OK;
         case GE_INFO_LAUNCHES: *value = p->launches; return GE_OK;
         case GE_INFO_TILE_VALID:
-            *value = p->kernel == GE_KERNEL_TEMPORAL
-                         ? (p->dtype == GE_F64 ? ge::temporal1d_tile_valid<double>(p->tb) : ge::temporal1d_tile_valid<float>(p->tb))
-                         : 0;
+            *value = p->kernel != GE_KERNEL_TEMPORAL ? 0
+                     : p->dim == 1 ? ge::temporal1d_geom(p->tc, p->dtype == GE_F64 ? 2 : 4, p->tb, 1).valid
+                                   : ge::temporal2d_geom(p->tc, p->dtype == GE_F64 ? 2 : 4, p->tb, 0, p->nx, p->ny, p->hp).valid;
             return GE_OK;
         case GE_INFO_TILE_LOADED:
-            *value = p->kernel == GE_KERNEL_TEMPORAL
-                         ? (p->dtype == GE_F64 ? ge::temporal1d_tile_loaded<double>() : ge::temporal1d_tile_loaded<float>())
-                         : 0;
+            *value = p->kernel == GE_KERNEL_TEMPORAL ? 32 * p->tc : 0;
+            return GE_OK;
+        default: return GE_EINVAL;
+    }
+}
+
+int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
+    if (!p) return GE_EINVAL;
+    switch (what) {
+        case GE_TUNE_SEG_PAIRS:
+            if (value < 1 || value > (1 << 20) || p->dim != 2) return GE_EINVAL;
+            p->hp = (int32_t)value;
+            return GE_OK;
+        case GE_TUNE_TEMPORAL_C: {
+            if (p->dim != 1) return GE_EINVAL;
+            const int c0 = p->dtype == GE_F64 ? 8 : 16;
+            if (value != c0 && value != 2 * c0) return GE_EINVAL;
+            p->tc = (int32_t)value;
+            if (p->kernel == GE_KERNEL_TEMPORAL) p->tb = clamp_tb(p, p->tb);
+            return GE_OK;
+        }
+        case GE_TUNE_TB:
+            if (value < 1 || p->kernel != GE_KERNEL_TEMPORAL) return GE_EINVAL;
+            if (p->dim == 2) {
+                if (!temporal2d_tb_ok(value)) return GE_EINVAL;
+                p->tb = (int32_t)value;
+                return GE_OK;
+            }
+            p->tb = clamp_tb(p, value);
             return GE_OK;
         default: return GE_EINVAL;
     }

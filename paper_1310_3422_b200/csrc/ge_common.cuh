@@ -90,4 +90,14 @@ __device__ __forceinline__ void pair_update_bc(T a, T b, T c, T d, const Coef1<T
     hi = fma(-g, t, q);
 }
 
+// Slide a lane's register window right by one element: slot j takes slot j+1, the last slot takes
+// the next lane's slot 0 (lane 31 keeps a stale value there; the tile geometry accounts for it).
+template <typename T, int C>
+__device__ __forceinline__ void shift_window(T (&v)[C]) {
+    const T t = __shfl_down_sync(0xffffffffu, v[0], 1);
+#pragma unroll
+    for (int j = 0; j + 1 < C; ++j) v[j] = v[j + 1];
+    v[C - 1] = t;
+}
+
 }  // namespace ge

@@ -105,11 +105,10 @@ __device__ __forceinline__ void group_update(const T (&w)[4][4], const Coef2<T>&
     if (xg == 0 && yg == 0) {
         const T E1 = Ra - Rd, E2 = Rb - Rc;
         const T Q = (Ra + Rd) - (Rb + Rc);
-        const T gq = k.g4 * Q;
-        na = fma(-k.g2, E1, Ra) - gq;
-        nd = fma(k.g2, E1, Rd) - gq;
-        nb = fma(-k.g2, E2, Rb) + gq;
-        nc = fma(k.g2, E2, Rc) + gq;
+        na = fma(-k.g4, Q, fma(-k.g2, E1, Ra));
+        nd = fma(-k.g4, Q, fma(k.g2, E1, Rd));
+        nb = fma(k.g4, Q, fma(-k.g2, E2, Rb));
+        nc = fma(k.g4, Q, fma(k.g2, E2, Rc));
         return;
     }
     na = a; nb = b; nc = c; nd = d;

@@ -4,64 +4,74 @@
 // Blackwell redesign of the paper's synchronisation question (PAPER.md:138-150:
 // two block barriers per level pair).  Here a WARP is an independent
 // halo-redundant tile: lane t holds C consecutive values; a two-point group
-// (i,i+1) reads u_{i-1}..u_{i+2}, so the dependency cone of a
-// pair widens by one node per side per level ("one group per sub-step").  The
-// warp loads 32*C values, advances tb levels exchanging only two values per
-// lane per level through warp shuffles, and stores the 32*C - 2*tb values whose
-// cone stayed inside the tile.  No __syncthreads, no shared memory, no
-// inter-block barrier: the alternating group shift happens in registers.
+// (i,i+1) reads u_{i-1}..u_{i+2} and the pattern shifts by
+// one node per level, so a tile edge placed ON a group boundary moves inward by
+// one node per level ("one group per sub-step").  The warp loads 32*C values,
+// advances tb levels exchanging ONE value per lane per level through a warp
+// shuffle, and stores the ~32*C - 2*tb values whose cone stayed inside the
+// tile.  No __syncthreads, no shared memory, no inter-block barrier: the
+// alternating group shift happens in registers.
 //
-// Sliding window.  Before a level whose pairs have their left members at odd
-// element indices (phase 1), lane t holds elements [a, a+C) with a even.  It
-// fetches elements a+C, a+C+1 (the first pair of lane t+1) and updates the pairs
-// (a+1,a+2) ... (a+C-1,a+C): its window becomes [a+1, a+C+1).  Now a+1 is odd and
-// the next level (phase 0) has its left members at even indices, i.e. again at
-// window start + 1: every level is the same code, the window slides right by
-// one element per level, and after an even tb it is 16-byte aligned again.
-// Hence a temporal block must START AT AN ODD LEVEL (ge_run peels one per-level
-// launch if needed) and tb is a multiple of the vector width.
+// Sliding window.  Before a level, lane t holds the window [w, w+C) (element
+// indices; element e is node e+1) with the level's left members at w+1, w+3, ...
+// It updates the pairs (w+1,w+2) ... (w+C-1,w+C); its window becomes
+// [w+1, w+C+1).  The next level's pattern is shifted by one node, i.e. its left
+// members again sit at (new window start)+1: every level is the same code and
+// the window slides right by one element per level.  A launch that starts at a
+// phase-0 level (left members at even elements) first shifts the 16-byte
+// aligned window right by one element (`pre`), and after the tb levels the
+// window is shifted by `post` < V more elements so that it is 16-byte aligned
+// again for the vector stores; each shift is one shuffle per lane.
+//
+// Arithmetic per level and lane (3 flops per node update; ge_common.cuh has
+// the derivation of the factored form).  With e_m = v[2m+1] - v[2m] the
+// difference ACROSS the group boundary left of pair m (shared by the two
+// adjacent pairs):
+//     p_m     = v[2m+1] - r e_m          right-hand side of Eq (2) at the left member
+//     z_m     = v[2m]   + r e_m          right-hand side of Eq (1) at the right member
+//                                        of the pair to the LEFT (= q_{m-1})
+//     q_{C/2-1} comes from lane t+1's z_0 (the one shuffle)
+//     w = g (q_m - p_m);  new left = p_m + w;  new right = q_m - w
 #pragma once
 #include "ge_common.cuh"
 
 namespace ge {
 
-template <typename T> struct Temporal1dCfg;
-template <> struct Temporal1dCfg<double> { static constexpr int C = 8;  static constexpr int TB = 16; };
-template <> struct Temporal1dCfg<float>  { static constexpr int C = 16; static constexpr int TB = 16; };
-
 constexpr int kTemporalWarps = 4;   // warps per CTA (independent tiles)
 
-template <typename T>
-inline int temporal1d_round_tb(int64_t tb) {
-    constexpr int V = VecOf<T>::V;
-    constexpr int C = Temporal1dCfg<T>::C;
-    const int64_t maxtb = 8 * C;                 // keeps at least half of the lanes valid
-    if (tb > maxtb) tb = maxtb;
-    return (int)(tb - tb % V);
+// Geometry of one launch: fixed by (C, V, tb, starting phase).
+struct Temporal1dGeom {
+    int tb;        // levels in this launch
+    int pre;       // 1 if the launch starts at a phase-0 level
+    int post;      // realignment shifts after the last level, < V
+    int shift;     // pre + tb + post: element offset between loaded and stored window
+    int valid;     // outputs per tile (multiple of V)
+};
+
+inline Temporal1dGeom temporal1d_geom(int C, int V, int tb, int phase) {
+    Temporal1dGeom g;
+    g.tb = tb;
+    g.pre = phase == 0 ? 1 : 0;
+    g.post = (V - (g.pre + tb) % V) % V;
+    g.shift = g.pre + tb + g.post;
+    // a stale slot spreads by 2 slots per level from an even slot, by 3 in the first level from the odd
+    // slot the pre-shift leaves behind, by 1 per realignment shift
+    const int v = 32 * C - 2 * tb - 2 * g.pre - g.post;
+    g.valid = v - v % V;
+    return g;
 }
-template <typename T>
-inline int temporal1d_pick_tb(int requested) {
-    int tb = requested > 0 ? requested : Temporal1dCfg<T>::TB;
-    tb = temporal1d_round_tb<T>(tb);
-    return tb < VecOf<T>::V ? VecOf<T>::V : tb;
-}
-template <typename T>
-inline int temporal1d_valid_lanes(int tb) {
-    constexpr int C = Temporal1dCfg<T>::C;
-    return 32 - (2 * tb + C - 1) / C;
-}
-template <typename T> inline int64_t temporal1d_tile_valid(int tb) { return (int64_t)temporal1d_valid_lanes<T>(tb) * Temporal1dCfg<T>::C; }
-template <typename T> inline int64_t temporal1d_tile_loaded() { return 32 * Temporal1dCfg<T>::C; }
+inline int temporal1d_max_tb(int C) { return 8 * C; }      // keeps at least half of every tile valid
 
 template <typename T, int C, bool EDGE>
 __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __restrict__ out, int64_t nx,
-                                                const Coef1<T>& k, int tb, int64_t w_valid,
+                                                const Coef1<T>& k, const Temporal1dGeom g,
                                                 int64_t tile, int lane) {
     constexpr int V = VecOf<T>::V;
     constexpr unsigned FULL = 0xffffffffu;
-    // element index of v[0] before the first level
-    const int64_t a0 = tile * w_valid - tb + (int64_t)lane * C;
-    T v[C + 2];
+    static_assert(C % 2 == 0 && C % V == 0, "C must hold whole pairs and whole vectors");
+    // element index of v[0] at load time
+    const int64_t a0 = tile * g.valid - g.shift + (int64_t)lane * C;
+    T v[C];
 #pragma unroll
     for (int c = 0; c < C / V; ++c) {
         const int64_t idx = a0 + c * V;
@@ -75,45 +85,64 @@ __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __r
 #pragma unroll
         for (int j = 0; j < V; ++j) v[c * V + j] = t[j];
     }
+    if (g.pre) shift_window<T, C>(v);
+    // EDGE tiles: position of the Dirichlet ghosts relative to the window start, as 32-bit ints
+    // (element -1 = node 0, element nx = node N+1); far-away ghosts are clamped out of reach.
+    int glo = 0, ghi = 0;
+    if constexpr (EDGE) {
+        const int64_t w0 = a0 + g.pre;
+        const int64_t dlo = -1 - w0, dhi = nx - w0;
+        glo = (int)(dlo < -(1 << 20) ? -(1 << 20) : (dlo > (1 << 20) ? (1 << 20) : dlo));
+        ghi = (int)(dhi < -(1 << 20) ? -(1 << 20) : (dhi > (1 << 20) ? (1 << 20) : dhi));
+    }
+    const T r = k.r, gg = k.g;
 #pragma unroll 2
-    for (int l = 0; l < tb; ++l) {
-        v[C] = __shfl_down_sync(FULL, v[0], 1);
-        v[C + 1] = __shfl_down_sync(FULL, v[1], 1);
+    for (int l = 0; l < g.tb; ++l) {
+        T p[C / 2], q[C / 2];
+        T z0;
+#pragma unroll
+        for (int m = 0; m < C / 2; ++m) {
+            const T e = v[2 * m + 1] - v[2 * m];
+            p[m] = fma(-r, e, v[2 * m + 1]);
+            const T z = fma(r, e, v[2 * m]);
+            if (m == 0) z0 = z; else q[m - 1] = z;
+        }
+        q[C / 2 - 1] = __shfl_down_sync(FULL, z0, 1);
         T nv[C];
 #pragma unroll
         for (int m = 0; m < C / 2; ++m) {
+            T pm = p[m], qm = q[m], gm = gg;
             if constexpr (EDGE) {
-                const int64_t bidx = a0 + l + 2 * m + 1;    // element index of the pair's left member
-                pair_update_bc(v[2 * m], v[2 * m + 1], v[2 * m + 2], v[2 * m + 3], k,
-                               bidx == -1, bidx + 1 == nx, nv[2 * m], nv[2 * m + 1]);
-            } else {
-                pair_update(v[2 * m], v[2 * m + 1], v[2 * m + 2], v[2 * m + 3], k.r, k.g, nv[2 * m], nv[2 * m + 1]);
+                // window slot of the pair's left member is 2m+1; slots are relative to w0 + l
+                if (2 * m + 1 == glo - l) { pm = k.lo; gm = k.e; }     // left member is node 0
+                if (2 * m + 2 == ghi - l) { qm = k.hi; gm = k.e; }     // right member is node N+1
             }
+            const T t = qm - pm;
+            nv[2 * m] = fma(gm, t, pm);
+            nv[2 * m + 1] = fma(-gm, t, qm);
         }
         if constexpr (EDGE) {
-            // keep the Dirichlet ghosts (node 0 = element -1, node N+1 = element nx) constant
+            // keep the ghosts constant: new slot j is old slot j+1
 #pragma unroll
             for (int j = 0; j < C; ++j) {
-                const int64_t idx = a0 + l + 1 + j;
-                if (idx == -1) nv[j] = k.lo;
-                if (idx == nx) nv[j] = k.hi;
+                if (j + 1 == glo - l) nv[j] = k.lo;
+                if (j + 1 == ghi - l) nv[j] = k.hi;
             }
         }
 #pragma unroll
         for (int j = 0; j < C; ++j) v[j] = nv[j];
     }
-    // window is now [a0 + tb, a0 + tb + C); store the lanes whose cone stayed inside the tile
-    const int64_t o0 = tile * w_valid + (int64_t)lane * C;
-    if ((int64_t)lane * C < w_valid) {
+    for (int s = 0; s < g.post; ++s) shift_window<T, C>(v);
+    // window start is now a0 + shift = tile*valid + lane*C: store what stayed inside the cone
+    const int64_t o0 = tile * g.valid + (int64_t)lane * C;
 #pragma unroll
-        for (int c = 0; c < C / V; ++c) {
-            const int64_t idx = o0 + c * V;
-            if (idx + V <= nx) {
-                T t[V];
+    for (int c = 0; c < C / V; ++c) {
+        const int64_t idx = o0 + c * V;
+        if (lane * C + c * V < g.valid && idx + V <= nx) {
+            T t[V];
 #pragma unroll
-                for (int j = 0; j < V; ++j) t[j] = v[c * V + j];
-                st_vec(out + idx, t);
-            }
+            for (int j = 0; j < V; ++j) t[j] = v[c * V + j];
+            st_vec(out + idx, t);
         }
     }
 }
@@ -121,33 +150,32 @@ __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __r
 template <typename T, int C>
 __global__ void __launch_bounds__(kTemporalWarps * 32)
 ge1d_temporal_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
-                     const Coef1<T>* __restrict__ coef, int tb, int64_t w_valid, int64_t tiles_per_rod) {
+                     const Coef1<T>* __restrict__ coef, const Temporal1dGeom g, int64_t tiles_per_rod) {
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int64_t tile = (int64_t)blockIdx.x * kTemporalWarps + warp;
     if (tile >= tiles_per_rod) return;
+    const int64_t lo_idx = tile * g.valid - g.shift;          // first element loaded
+    const bool edge = lo_idx < 0 || lo_idx + 32 * C > nx;
     for (int64_t rod = blockIdx.y; rod < batch; rod += gridDim.y) {
         const Coef1<T> k = coef[rod];
         const T* __restrict__ in = uin + rod * nx;
         T* __restrict__ out = uout + rod * nx;
-        const int64_t lo_idx = tile * w_valid - tb;              // first element touched
-        const int64_t hi_idx = lo_idx + 32 * C + tb;             // one past the last element touched
-        if (lo_idx < 0 || hi_idx > nx) temporal1d_tile<T, C, true>(in, out, nx, k, tb, w_valid, tile, lane);
-        else                           temporal1d_tile<T, C, false>(in, out, nx, k, tb, w_valid, tile, lane);
+        if (edge) temporal1d_tile<T, C, true>(in, out, nx, k, g, tile, lane);
+        else      temporal1d_tile<T, C, false>(in, out, nx, k, g, tile, lane);
     }
 }
 
-// Host launcher.  Requires: nx % V == 0, 16-byte aligned rows, tb % V == 0, tb >= V,
-// and the first of the tb levels is an odd (phase 1) level.  Returns a cudaError_t as int.
-template <typename T>
-inline int temporal1d_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
-                             int tb, cudaStream_t s) {
-    constexpr int C = Temporal1dCfg<T>::C;
-    const int64_t w_valid = temporal1d_tile_valid<T>(tb);
-    const int64_t tiles = (nx + w_valid - 1) / w_valid;
+// Host launcher: tb levels starting at a level of the given phase.
+// Requires nx % V == 0, 16-byte aligned rows, 1 <= tb <= temporal1d_max_tb(C).
+template <typename T, int C>
+inline cudaError_t temporal1d_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
+                                     int tb, int phase, cudaStream_t s) {
+    const Temporal1dGeom g = temporal1d_geom(C, VecOf<T>::V, tb, phase);
+    const int64_t tiles = (nx + g.valid - 1) / g.valid;
     dim3 grid((unsigned)((tiles + kTemporalWarps - 1) / kTemporalWarps), (unsigned)(batch < 65535 ? batch : 65535));
-    ge1d_temporal_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, tb, w_valid, tiles);
-    return (int)cudaGetLastError();
+    ge1d_temporal_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, g, tiles);
+    return cudaGetLastError();
 }
 
 }  // namespace ge

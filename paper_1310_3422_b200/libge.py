@@ -21,6 +21,7 @@ GE_F32, GE_F64 = 0, 1
 GE_KERNEL_AUTO, GE_KERNEL_PER_STEP, GE_KERNEL_TEMPORAL, GE_KERNEL_PERSISTENT = 0, 1, 2, 3
 GE_OK, GE_EINVAL, GE_ENOMEM, GE_ECUDA, GE_EUNSUPPORTED = 0, -1, -2, -3, -4
 GE_INFO_KERNEL, GE_INFO_TB, GE_INFO_LAUNCHES, GE_INFO_TILE_VALID, GE_INFO_TILE_LOADED = 0, 1, 2, 3, 4
+GE_TUNE_TEMPORAL_C, GE_TUNE_TB, GE_TUNE_SEG_PAIRS = 0, 1, 2
 
 KERNEL_NAMES = {0: "auto", 1: "per_step", 2: "temporal", 3: "persistent"}
 _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
@@ -28,7 +29,7 @@ _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 
 # every symbol include/ge.h declares
 EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_2d", "ge_run", "ge_run_host",
-           "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_destroy",
+           "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
            "ge_strerror", "ge_version")
 
 
@@ -75,6 +76,7 @@ def load() -> ctypes.CDLL:
     lib.ge_plan_get_level.argtypes = [vp, ctypes.POINTER(i64)]
     lib.ge_plan_set_level.argtypes = [vp, i64]
     lib.ge_plan_info.argtypes = [vp, i32, ctypes.POINTER(i64)]
+    lib.ge_plan_tune.argtypes = [vp, i32, i64]
     lib.ge_plan_destroy.argtypes = [vp]
     lib.ge_strerror.argtypes = [ctypes.c_int]
     lib.ge_strerror.restype = ctypes.c_char_p
@@ -157,6 +159,10 @@ def ge_plan_info(plan: int, what: int) -> int:
     return v.value
 
 
+def ge_plan_tune(plan: int, what: int, value: int):
+    _check(load().ge_plan_tune(plan, what, value), "ge_plan_tune")
+
+
 def ge_plan_destroy(plan: Optional[int]):
     if plan:
         _check(load().ge_plan_destroy(plan), "ge_plan_destroy")
@@ -198,6 +204,9 @@ class Plan:
     @level.setter
     def level(self, v: int):
         ge_plan_set_level(self.handle, v)
+
+    def tune(self, what: int, value: int):
+        ge_plan_tune(self.handle, what, value)
 
     def info(self) -> dict:
         return dict(kernel=KERNEL_NAMES[ge_plan_info(self.handle, GE_INFO_KERNEL)],

@@ -4,7 +4,7 @@ import numpy as np
 _TORCH_DT = {"f32": "float32", "f64": "float64"}
 
 
-def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run"):
+def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0):
     """Run `steps` levels on cuda:0 and return the final state as a numpy array."""
     import torch
     from paper_1310_3422_b200 import libge
@@ -13,6 +13,10 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run"):
     stream = torch.cuda.current_stream(dev).cuda_stream
     with libge.Plan(cfg, kernel=kernel, tb=tb, stream=stream) as plan:
         plan.level = level0
+        if tc:
+            plan.tune(libge.GE_TUNE_TEMPORAL_C, tc)
+        if hp:
+            plan.tune(libge.GE_TUNE_SEG_PAIRS, hp)
         if via == "run":
             plan.run(u.data_ptr(), steps, stream)
         elif via == "step":
@@ -53,11 +57,16 @@ def rel_err(got, ref):
     return float(np.abs(got - ref).max() / max(np.abs(ref).max(), 1e-300))
 
 
-def rel_err_rows(got, ref):
+def rel_err_rows(got, ref, cfg=None):
+    """Per-rod max-abs error over the scale of the rod's data: max|oracle| over the interior and, when
+    cfg is given, the rod's two Dirichlet values (they are part of the solution, nodes 0 and N+1;
+    without them a 1-node rod between O(1) boundary values has no meaningful scale)."""
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
     d = np.abs(got - ref).max(axis=1)
     s = np.maximum(np.abs(ref).max(axis=1), 1e-300)
+    if cfg is not None:
+        s = np.maximum(s, np.maximum(np.abs(cfg["bc_lo"]), np.abs(cfg["bc_hi"])))
     return float((d / s).max())
 
 
