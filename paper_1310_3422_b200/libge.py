@@ -15,7 +15,8 @@ import os
 from typing import Optional, Sequence
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "lib", "libge.so")
+# LIBGE_PATH overrides the in-tree location (e.g. to compare two builds); it must still be a libge.so
+LIB_PATH = os.environ.get("LIBGE_PATH") or os.path.join(_HERE, "lib", "libge.so")
 
 GE_F32, GE_F64 = 0, 1
 GE_KERNEL_AUTO, GE_KERNEL_PER_STEP, GE_KERNEL_TEMPORAL, GE_KERNEL_PERSISTENT = 0, 1, 2, 3
