@@ -51,7 +51,10 @@ typedef enum {
     GE_KERNEL_AUTO = 0,       /* library picks per shape                  */
     GE_KERNEL_PER_STEP = 1,   /* A: one launch per level, one HBM round trip per level              */
     GE_KERNEL_TEMPORAL = 2,   /* B: tb levels per launch in registers/SMEM, halo-redundant tiles    */
-    GE_KERNEL_PERSISTENT = 3  /* C: state stays on chip for the whole run (rod-per-warp, batched 1-D) */
+    GE_KERNEL_PERSISTENT = 3  /* C: state stays in registers for the whole run, one launch (1-D): a rod
+                                 per CTA (batched rods), or one rod spread over the whole chip by a
+                                 cooperative launch whose tiles meet every tb levels; shapes that do not
+                                 fit on the chip fall back to B (GE_INFO_KERNEL tells)                  */
 } ge_kernel;
 
 typedef enum {
@@ -74,7 +77,8 @@ typedef struct {
     const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; copied  */
     int32_t   kernel;     /* ge_kernel                                                                 */
     int32_t   tb;         /* levels per launch for TEMPORAL (0 = auto; any value >= 1, both starting
-                             phases are handled in-kernel); ignored otherwise                          */
+                             phases are handled in-kernel); levels between two meetings of the tiles for
+                             PERSISTENT on one long rod (0 = the largest the halo allows)              */
 } ge_desc;
 
 /* Create a plan: validates desc, uploads per-rod coefficients (r, r/(1+2r), r/(1+r), ... computed in
@@ -110,7 +114,15 @@ enum {
     GE_INFO_TB = 1,            /* levels per launch of the temporal kernel (0 if not used)        */
     GE_INFO_LAUNCHES = 2,      /* kernels launched through this plan so far                       */
     GE_INFO_TILE_VALID = 3,    /* valid outputs per tile of the temporal kernel (per axis)        */
-    GE_INFO_TILE_LOADED = 4    /* elements loaded per tile of the temporal kernel (per axis)      */
+    GE_INFO_TILE_LOADED = 4,   /* elements loaded per tile of the temporal kernel (per axis)      */
+    GE_INFO_RESIDENT_PATH = 5, /* strategy C: 0 not in use, 1 rod per CTA, 2 one rod on the whole chip */
+    GE_INFO_RESIDENT_C = 6,    /* strategy C: values per lane                                     */
+    GE_INFO_RESIDENT_WARPS = 7,/* path 1: warps per rod; path 2: tiles (warps) in the launch      */
+    GE_INFO_RESIDENT_CAPACITY = 8, /* path 2: co-resident tiles the device offers                 */
+    GE_INFO_RESIDENT_TB = 9,   /* path 2: levels between two meetings                             */
+    GE_INFO_MEETINGS = 10,     /* path 2: meetings (halo exchanges) performed so far              */
+    GE_INFO_SYNC_FAULT = 11    /* path 2: 1 if a tile ever gave up waiting for a neighbour (the result
+                                  is then invalid); SYNCHRONISES the last stream used              */
 };
 int ge_plan_info(const ge_plan *p, int32_t what, int64_t *value);
 
@@ -118,9 +130,14 @@ int ge_plan_info(const ge_plan *p, int32_t what, int64_t *value);
  * GE_EINVAL for a value the kernels are not instantiated for; nothing is enqueued. */
 enum {
     GE_TUNE_TEMPORAL_C = 0,    /* values per lane of the 1-D temporal kernel: 8 or 16 (f64), 16 or 32 (f32) */
-    GE_TUNE_TB = 1,            /* levels per launch (1-D: >= 1, clamped to the largest the tile allows;
+    GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
                                   2-D: one of the compiled-in block lengths 4, 8)                            */
-    GE_TUNE_SEG_PAIRS = 2      /* 2-D temporal kernel: output row pairs per warp segment (default 64)       */
+    GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 64)       */
+    GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
+                                  long rod: 16, 32 (f64) / 32, 64 (f32)); may synchronise and reallocate      */
+    GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8 (tb <= lanes * C); may synchronise      */
+    GE_TUNE_SYNC_MODE = 5      /* path 2: 0 = neighbour flags (release/acquire per tile), 1 = grid-wide
+                                  barrier (cooperative groups) at every meeting                             */
 };
 int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
 

@@ -15,6 +15,7 @@
 #include "ge_level.cuh"
 #include "ge_temporal.cuh"
 #include "ge_temporal2d.cuh"
+#include "ge_resident.cuh"
 
 namespace {
 
@@ -48,6 +49,18 @@ struct ge_plan {
     void* hostpath;           // device: state buffer for ge_run_host (lazy)
     cudaStream_t last_stream;
     int sm_count;
+    // strategy C (ge_resident.cuh)
+    int32_t res_path;         // 0 none, 1 rod per CTA, 2 one rod on the whole chip
+    int32_t res_c, res_w;     // values per lane, warps per rod (path 1)
+    int32_t res_hl;           // halo lanes per side (path 2)
+    int32_t res_tb;           // levels between two meetings (path 2)
+    int32_t res_sync;         // kSyncFlags / kSyncGrid (path 2)
+    int64_t res_tiles;        // tiles (warps) of path 2
+    int64_t res_capacity;     // co-resident tiles the device offers for path 2
+    void* res_xbuf;           // device: exchange buffer of path 2
+    unsigned* res_flags;      // device: one flag per tile, + the fault word at [res_tiles]
+    unsigned res_epoch;       // value every flag holds between launches
+    int64_t meetings;         // meetings of the persistent kernel so far (info)
 };
 
 namespace {
@@ -198,6 +211,162 @@ int clamp_tb(const ge_plan* p, int64_t tb) {
     return (int)(tb > mx ? mx : tb);
 }
 
+// ---- strategy C (ge_resident.cuh) ------------------------------------------
+// Values per lane the resident kernels are instantiated for (ascending).
+template <typename T> struct ResidentC;
+template <> struct ResidentC<float>  { static constexpr int n = 4; static constexpr int c[4] = {16, 32, 64, 128}; };
+template <> struct ResidentC<double> { static constexpr int n = 4; static constexpr int c[4] = {8, 16, 32, 64}; };
+constexpr int kRodMaxWarps = 8;
+
+inline const int* resident_c_list(int dtype) { return dtype == GE_F64 ? ResidentC<double>::c : ResidentC<float>::c; }
+
+// Path 1 geometry: a rod of nx nodes in one CTA.  Prefers one warp (no barrier) with as many lanes
+// in use as possible, then the largest C with the fewest warps.  `want_c` != 0 pins C.
+bool rod_resident_pick(int dtype, int64_t nx, int want_c, int* c_out, int* w_out) {
+    const int* cs = resident_c_list(dtype);
+    if (nx % 2) return false;
+    if (want_c) {
+        bool known = false;
+        for (int i = 0; i < 4; ++i) known |= cs[i] == want_c;
+        if (!known || nx % want_c) return false;
+        const int64_t lanes = nx / want_c;
+        int w = 1;
+        while (32 * w < lanes) w *= 2;
+        if (w > kRodMaxWarps) return false;
+        *c_out = want_c; *w_out = w;
+        return true;
+    }
+    for (int i = 0; i < 4; ++i)
+        if (nx % cs[i] == 0 && nx / cs[i] <= 32) { *c_out = cs[i]; *w_out = 1; return true; }
+    for (int i = 3; i >= 0; --i) {
+        if (nx % cs[i]) continue;
+        const int64_t lanes = nx / cs[i];
+        int w = 1;
+        while (32 * w < lanes) w *= 2;
+        if (w <= kRodMaxWarps) { *c_out = cs[i]; *w_out = w; return true; }
+    }
+    return false;
+}
+
+template <typename T, int C>
+cudaError_t rod_resident_dispatch_w(ge_plan* p, T* u, int phase0, int64_t steps, cudaStream_t s) {
+    auto* c = (const ge::Coef1<T>*)p->coef;
+    switch (p->res_w) {
+        case 1: return ge::rod_resident_launch<T, C, 1>(u, p->nx, p->batch, c, phase0, steps, s);
+        case 2: return ge::rod_resident_launch<T, C, 2>(u, p->nx, p->batch, c, phase0, steps, s);
+        case 4: return ge::rod_resident_launch<T, C, 4>(u, p->nx, p->batch, c, phase0, steps, s);
+        case 8: return ge::rod_resident_launch<T, C, 8>(u, p->nx, p->batch, c, phase0, steps, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename T>
+int launch_rod_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
+    const int phase0 = (int)(p->level & 1);
+    constexpr const int* cs = ResidentC<T>::c;
+    cudaError_t e = cudaErrorInvalidValue;
+    if (p->res_c == cs[0]) e = rod_resident_dispatch_w<T, cs[0]>(p, (T*)u, phase0, steps, s);
+    else if (p->res_c == cs[1]) e = rod_resident_dispatch_w<T, cs[1]>(p, (T*)u, phase0, steps, s);
+    else if (p->res_c == cs[2]) e = rod_resident_dispatch_w<T, cs[2]>(p, (T*)u, phase0, steps, s);
+    else if (p->res_c == cs[3]) e = rod_resident_dispatch_w<T, cs[3]>(p, (T*)u, phase0, steps, s);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += steps;
+    return GE_OK;
+}
+
+// Path 2: the grid-resident kernel is instantiated for the two largest C of the dtype.
+template <typename T, int C>
+const void* grid_resident_fn() { return (const void*)&ge::ge1d_grid_resident_kernel<T, C>; }
+
+const void* grid_resident_fn_for(int dtype, int c) {
+    if (dtype == GE_F64) {
+        if (c == 16) return grid_resident_fn<double, 16>();
+        if (c == 32) return grid_resident_fn<double, 32>();
+    } else {
+        if (c == 32) return grid_resident_fn<float, 32>();
+        if (c == 64) return grid_resident_fn<float, 64>();
+    }
+    return nullptr;
+}
+
+// (Re)derive path-2 geometry from res_c / res_hl / res_tb and (re)allocate its buffers.
+// Returns GE_OK with res_path = 2 when the rod fits on the chip, GE_OK with res_path = 0 when not.
+int grid_resident_configure(ge_plan* p) {
+    p->res_path = 0;
+    if (p->dim != 1 || p->batch != 1) return GE_OK;
+    const void* fn = grid_resident_fn_for(p->dtype, p->res_c);
+    if (!fn || p->nx % p->res_c) return GE_OK;
+    if (p->res_hl < 1 || p->res_hl > 8) return GE_OK;
+    const int64_t valid = (int64_t)(32 - 2 * p->res_hl) * p->res_c;
+    const int64_t tiles = (p->nx + valid - 1) / valid;
+    int coop = 0, per_sm = 0;
+    GE_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
+    if (!coop) return GE_OK;
+    GE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * ge::kGridWarps, 0));
+    p->res_capacity = (int64_t)per_sm * p->sm_count * ge::kGridWarps;
+    if (tiles > p->res_capacity) return GE_OK;
+    int tb = p->res_tb > 0 ? p->res_tb : p->res_hl * p->res_c;
+    if (tb > p->res_hl * p->res_c) tb = p->res_hl * p->res_c;
+    tb -= tb % 2;
+    if (tb < 2) return GE_OK;
+    // buffers: exchange (2 parities x tiles x 2 sides x hl*C) and flags (+ fault word)
+    GE_CUDA(cudaStreamSynchronize(p->last_stream));      // an earlier launch may still use the old ones
+    cudaFree(p->res_xbuf); cudaFree(p->res_flags);
+    p->res_xbuf = nullptr; p->res_flags = nullptr;
+    const size_t xb = (size_t)2 * tiles * 2 * p->res_hl * p->res_c * elem_size(p->dtype);
+    GE_CUDA(cudaMalloc(&p->res_xbuf, xb));
+    GE_CUDA(cudaMalloc((void**)&p->res_flags, (size_t)(tiles + 1) * sizeof(unsigned)));
+    GE_CUDA(cudaMemset(p->res_flags, 0, (size_t)(tiles + 1) * sizeof(unsigned)));
+    p->res_epoch = 0;
+    p->res_tiles = tiles;
+    p->res_tb = tb;
+    p->res_path = 2;
+    return GE_OK;
+}
+
+int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
+    ge::GridResidentArgs a;
+    a.nx = p->nx; a.ntiles = p->res_tiles; a.steps = steps; a.phase0 = (int)(p->level & 1);
+    a.hl = p->res_hl; a.tb = p->res_tb; a.sync_mode = p->res_sync; a.epoch0 = p->res_epoch;
+    void* xbuf = p->res_xbuf;
+    void* coef = p->coef;
+    unsigned* flags = p->res_flags;
+    unsigned* fault = p->res_flags + p->res_tiles;
+    void* args[] = {&u, &xbuf, &coef, &flags, &fault, &a};
+    const void* fn = grid_resident_fn_for(p->dtype, p->res_c);
+    const unsigned ctas = (unsigned)((p->res_tiles + ge::kGridWarps - 1) / ge::kGridWarps);
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(ctas), dim3(32 * ge::kGridWarps), args, 0, s);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    const int64_t meet = ge::grid_resident_meetings(steps, a.phase0, a.tb);
+    if (p->res_sync == ge::kSyncFlags) p->res_epoch += (unsigned)(1 + meet);
+    p->meetings += meet;
+    p->launches += 1;
+    p->level += steps;
+    return GE_OK;
+}
+
+// Decide the strategy-C path at plan creation / after a tuning call.
+int resident_configure(ge_plan* p, int want_c) {
+    p->res_path = 0;
+    if (p->dim != 1) return GE_OK;
+    const int* cs = resident_c_list(p->dtype);
+    int c = 0, w = 0;
+    const bool rod = rod_resident_pick(p->dtype, p->nx, want_c, &c, &w);
+    // one rod that needs more than one warp: spread it over the chip when it fits there
+    if (p->batch == 1 && (!rod || w > 1)) {
+        p->res_c = want_c ? want_c : cs[2];
+        const int rc = grid_resident_configure(p);
+        if (rc != GE_OK || p->res_path == 2) return rc;
+    }
+    if (rod) { p->res_path = 1; p->res_c = c; p->res_w = w; }
+    return GE_OK;
+}
+
+bool resident_ok(const ge_plan* p, const void* u) {
+    return p->res_path != 0 && ((uintptr_t)u % 16 == 0);
+}
+
 int step_common(ge_plan* p, int dim, const void* uin, void* uout, cudaStream_t s) {
     if (!p || !uin || !uout || uin == uout || p->dim != dim) return GE_EINVAL;
     const size_t es = elem_size(p->dtype);
@@ -267,16 +436,24 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     }
     if (rc != GE_OK) { cudaFree(p->coef); cudaFree(p->scratch); cudaGetLastError(); delete p; return rc; }
 
-    // strategy selection
-    int kernel = d->kernel;
-    if (kernel == GE_KERNEL_AUTO) kernel = GE_KERNEL_TEMPORAL;
-    if (kernel == GE_KERNEL_PERSISTENT) kernel = GE_KERNEL_TEMPORAL;
-    p->kernel = kernel;
+    // strategy selection: AUTO takes the resident kernels when the state fits on
+    // the chip (1-D only), else the temporally blocked ones
     p->tb = 0;
     p->tc = default_tc(p->dtype);
     p->hp = 64;
-    if (kernel == GE_KERNEL_TEMPORAL && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : 16);
-    if (kernel == GE_KERNEL_TEMPORAL && d->dim == 2) {
+    p->res_hl = 1;
+    p->res_sync = ge::kSyncFlags;
+    int kernel = d->kernel;
+    if (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT) {
+        p->res_tb = d->tb;
+        rc = resident_configure(p, 0);
+        if (rc != GE_OK) { cudaFree(p->coef); cudaFree(p->scratch); cudaFree(p->res_xbuf); cudaFree(p->res_flags); cudaGetLastError(); delete p; return rc; }
+        kernel = p->res_path ? GE_KERNEL_PERSISTENT : GE_KERNEL_TEMPORAL;
+    }
+    p->kernel = kernel;
+    const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
+    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : 16);
+    if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : 8;
         if (!temporal2d_tb_ok(p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
@@ -303,7 +480,15 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     void* oth = p->scratch;
     int64_t left = steps;
     int rc = GE_OK;
-    const bool temporal = p->kernel == GE_KERNEL_TEMPORAL && temporal_ok(p, u);
+    if (p->kernel == GE_KERNEL_PERSISTENT && resident_ok(p, u)) {
+        // strategy C: the whole run is one launch, in place
+        if (steps == 0) return GE_OK;
+        if (p->res_path == 1)
+            return p->dtype == GE_F64 ? launch_rod_resident<double>(p, u, steps, s)
+                                      : launch_rod_resident<float>(p, u, steps, s);
+        return launch_grid_resident(p, u, steps, s);
+    }
+    const bool temporal = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && temporal_ok(p, u);
     while (left > 0 && rc == GE_OK) {
         if (temporal && p->dim == 2) {
             if (left >= p->tb) {
@@ -371,6 +556,24 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
         case GE_INFO_TILE_LOADED:
             *value = p->kernel == GE_KERNEL_TEMPORAL ? 32 * p->tc : 0;
             return GE_OK;
+        case GE_INFO_RESIDENT_PATH: *value = p->kernel == GE_KERNEL_PERSISTENT ? p->res_path : 0; return GE_OK;
+        case GE_INFO_RESIDENT_C: *value = p->res_path ? p->res_c : 0; return GE_OK;
+        case GE_INFO_RESIDENT_WARPS:
+            *value = p->res_path == 1 ? p->res_w : (p->res_path == 2 ? p->res_tiles : 0);
+            return GE_OK;
+        case GE_INFO_RESIDENT_CAPACITY: *value = p->res_path == 2 ? p->res_capacity : 0; return GE_OK;
+        case GE_INFO_RESIDENT_TB: *value = p->res_path == 2 ? p->res_tb : 0; return GE_OK;
+        case GE_INFO_MEETINGS: *value = p->meetings; return GE_OK;
+        case GE_INFO_SYNC_FAULT: {
+            *value = 0;
+            if (p->res_path == 2 && p->res_flags) {
+                unsigned f = 0;
+                GE_CUDA(cudaStreamSynchronize(p->last_stream));
+                GE_CUDA(cudaMemcpy(&f, p->res_flags + p->res_tiles, sizeof(f), cudaMemcpyDeviceToHost));
+                *value = f;
+            }
+            return GE_OK;
+        }
         default: return GE_EINVAL;
     }
 }
@@ -390,8 +593,47 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             if (p->kernel == GE_KERNEL_TEMPORAL) p->tb = clamp_tb(p, p->tb);
             return GE_OK;
         }
+        case GE_TUNE_RESIDENT_C: {
+            // path 1: values per lane (warps follow); path 2: values per lane of a tile
+            if (p->kernel != GE_KERNEL_PERSISTENT || value < 2 || value > 128) return GE_EINVAL;
+            const int32_t path0 = p->res_path, c0 = p->res_c, w0 = p->res_w;
+            int rc = resident_configure(p, (int)value);
+            if (rc != GE_OK) return rc;
+            if (p->res_path == 0) {                            // not instantiated / does not fit: restore
+                p->res_c = c0; p->res_w = w0;
+                if (path0 == 2) { rc = grid_resident_configure(p); if (rc != GE_OK) return rc; }
+                else p->res_path = path0;
+                return GE_EINVAL;
+            }
+            return GE_OK;
+        }
+        case GE_TUNE_HALO_LANES: {
+            if (p->kernel != GE_KERNEL_PERSISTENT || p->res_path != 2 || value < 1 || value > 8) return GE_EINVAL;
+            const int32_t hl0 = p->res_hl, tb0 = p->res_tb;
+            p->res_hl = (int32_t)value; p->res_tb = 0;
+            int rc = grid_resident_configure(p);
+            if (rc == GE_OK && p->res_path != 2) {
+                p->res_hl = hl0; p->res_tb = tb0;
+                rc = grid_resident_configure(p);
+                return rc == GE_OK ? GE_EINVAL : rc;
+            }
+            return rc;
+        }
+        case GE_TUNE_SYNC_MODE:
+            if (p->kernel != GE_KERNEL_PERSISTENT || p->res_path != 2) return GE_EINVAL;
+            if (value != ge::kSyncFlags && value != ge::kSyncGrid) return GE_EINVAL;
+            p->res_sync = (int32_t)value;
+            return GE_OK;
         case GE_TUNE_TB:
-            if (value < 1 || p->kernel != GE_KERNEL_TEMPORAL) return GE_EINVAL;
+            if (value < 1) return GE_EINVAL;
+            if (p->kernel == GE_KERNEL_PERSISTENT && p->res_path == 2) {
+                int64_t tb = value > (int64_t)p->res_hl * p->res_c ? (int64_t)p->res_hl * p->res_c : value;
+                tb -= tb % 2;
+                if (tb < 2) return GE_EINVAL;
+                p->res_tb = (int32_t)tb;
+                return GE_OK;
+            }
+            if (p->kernel != GE_KERNEL_TEMPORAL) return GE_EINVAL;
             if (p->dim == 2) {
                 if (!temporal2d_tb_ok(value)) return GE_EINVAL;
                 p->tb = (int32_t)value;
@@ -410,6 +652,8 @@ int ge_plan_destroy(ge_plan* p) {
     cudaFree(p->coef);
     cudaFree(p->scratch);
     cudaFree(p->hostpath);
+    cudaFree(p->res_xbuf);
+    cudaFree(p->res_flags);
     delete p;
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     return GE_OK;

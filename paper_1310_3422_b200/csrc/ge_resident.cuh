@@ -1,0 +1,444 @@
+// ge_resident.cuh -- strategy C (1-D): the state stays in REGISTERS for the
+// whole run; HBM is touched once at the start and once at the end.
+//
+// This is the Blackwell answer to the paper's synchronisation question
+// (one thread per sub-domain couple, two block barriers per
+// level pair, and no correct barrier ACROSS blocks -- PAPER.md:160, :216).
+// Two kernels share one level code:
+//
+//   (i)  ge1d_rod_resident_kernel   a rod (nx <= 32*C*W nodes) lives in one CTA
+//        of W warps, C values per lane.  W = 1: no barrier at all, one warp
+//        shuffle per lane and level.  W > 1: the two warp-edge values cross
+//        through shared memory, one __syncthreads per level.  Batched rods
+//        (SURVEY.md 8(a) a6): one rod per CTA, loaded once, marched `steps`
+//        levels, stored once.
+//   (ii) ge1d_grid_resident_kernel  ONE long rod spread over the whole chip by a
+//        cooperative launch: a warp owns a tile of (32-2*hl)*C nodes plus hl
+//        halo lanes on either side.  The halo goes stale by one node per level
+//        (below), so tiles only meet every tb <= hl*C levels: each warp
+//        publishes its outermost valid lanes to a small L2-resident exchange
+//        buffer and refreshes its halo lanes from its two neighbours'.  The
+//        meeting is either NEIGHBOUR-ONLY (a release/acquire flag per tile --
+//        the paper's observation that only wall nodes are shared,
+//        PAPER.md:138) or a GRID-WIDE barrier (cooperative groups), selectable
+//        for the comparison north_star asks for.
+//
+// Level code (drift-free sliding window).  In the "even state" lane t holds
+// the window [w, w+C), w even.  Levels come in pairs:
+//   R  (phase 1: left members at odd elements)  the lane updates the pairs
+//      (w+1,w+2) ... (w+C-1,w+C); the last pair's right-hand side q comes from
+//      the next lane (one shuffle); the window becomes [w+1, w+C+1).
+//   L  (phase 0: left members at even elements, i.e. again at odd SLOTS of the
+//      shifted window)  the lane updates (w,w+1) ... (w+C-2,w+C-1); the first
+//      pair's left right-hand side p comes from the previous lane (one
+//      shuffle); the window is [w, w+C) again.
+// So a pair of levels costs two shuffles and no register moves, and the
+// arithmetic is the 3-flop-per-node factored form of ge_temporal.cuh (the
+// difference e across a group boundary is shared by the two adjacent pairs) --
+// the same expression tree as every other libge kernel, so results are
+// bit-identical to the per-level kernel.
+// A run that starts at a phase-0 level first takes one in-lane level I (pairs
+// (w,w+1) ..., two shuffles); a run with one level left over takes R followed
+// by a one-slot shift back.
+//
+// Validity.  A window edge that lies ON a group boundary loses one node per
+// level: the pair that straddles it in the next (shifted) pattern cannot be
+// formed.  After n levels a lane group that started fully valid has n stale
+// nodes on either side (I and the shift back are counted as 2).
+//
+// Boundaries.  nx % C == 0 is required, so element 0 is
+// slot 0 of some lane (`is_lo`) and element nx-1 is slot C-1 of some lane
+// (`is_hi`); the Dirichlet values never occupy a slot of a valid lane:
+//   R: node 1 is single: new = z0 - e (z0 - beta_lo) (Eq (1));
+//      it leaves the shifted window and is kept in the extra register x0.
+//      The last pair of lane is_hi is (N, N+1): q := beta_hi, g := e (Eq (2)).
+//   L: the first pair of lane is_lo is (1,2): its p is formed from x0 and
+//      beta_lo instead of the shuffled value.
+// Lanes outside the rod hold finite filler and never feed a valid lane.
+#pragma once
+#include <cooperative_groups.h>
+
+#include "ge_common.cuh"
+
+namespace ge {
+
+namespace cg = cooperative_groups;
+
+template <typename T>
+__device__ __forceinline__ void ld_vec_plain(const T* p, T (&x)[VecOf<T>::V]) {
+    using VT = typename VecOf<T>::type;
+    const VT v = *reinterpret_cast<const VT*>(p);
+    if constexpr (VecOf<T>::V == 4) { x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
+    else { x[0] = v.x; x[1] = v.y; }
+}
+template <typename T>
+__device__ __forceinline__ void ld_vec_cg(const T* p, T (&x)[VecOf<T>::V]) {
+    using VT = typename VecOf<T>::type;
+    const VT v = __ldcg(reinterpret_cast<const VT*>(p));
+    if constexpr (VecOf<T>::V == 4) { x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
+    else { x[0] = v.x; x[1] = v.y; }
+}
+template <typename T>
+__device__ __forceinline__ void st_vec_cg(T* p, const T (&x)[VecOf<T>::V]) {
+    using VT = typename VecOf<T>::type;
+    VT v;
+    if constexpr (VecOf<T>::V == 4) { v.x = x[0]; v.y = x[1]; v.z = x[2]; v.w = x[3]; }
+    else { v.x = x[0]; v.y = x[1]; }
+    __stcg(reinterpret_cast<VT*>(p), v);
+}
+
+// Per-lane constants of the resident level code.  XW: the W > 1 warps of the CTA hold one rod and
+// exchange their edge values through shared memory (sx: [2 buffers][2 sides][nwarps]).
+template <typename T, bool XW>
+struct ResidentCtx {
+    T r, g, e, lo, hi;
+    bool is_lo, is_hi;
+    int lane, warp, nwarps;
+    T* sx;
+};
+
+// value `mine` of lane+1 (next warp's lane 0 through shared memory when XW)
+template <typename T, bool XW>
+__device__ __forceinline__ T from_right(const ResidentCtx<T, XW>& c, T mine, int buf) {
+    T got = __shfl_down_sync(0xffffffffu, mine, 1);
+    if constexpr (XW) {
+        T* slot = c.sx + (buf * 2 + 0) * c.nwarps;
+        if (c.lane == 0) slot[c.warp] = mine;
+        __syncthreads();
+        if (c.lane == 31 && c.warp + 1 < c.nwarps) got = slot[c.warp + 1];
+    }
+    return got;
+}
+// value `mine` of lane-1 (previous warp's lane 31 through shared memory when XW)
+template <typename T, bool XW>
+__device__ __forceinline__ T from_left(const ResidentCtx<T, XW>& c, T mine, int buf) {
+    T got = __shfl_up_sync(0xffffffffu, mine, 1);
+    if constexpr (XW) {
+        T* slot = c.sx + (buf * 2 + 1) * c.nwarps;
+        if (c.lane == 31) slot[c.warp] = mine;
+        __syncthreads();
+        if (c.lane == 0 && c.warp > 0) got = slot[c.warp - 1];
+    }
+    return got;
+}
+
+// R: even state -> shifted state, left members at odd slots (a phase-1 level).  In place.
+template <typename T, int C, bool XW>
+__device__ __forceinline__ void level_R(T (&v)[C], T& x0, const ResidentCtx<T, XW>& c, int buf) {
+    const T r = c.r, g = c.g;
+    T e = v[1] - v[0];
+    T pprev = fma(-r, e, v[1]);               // rhs of Eq (2) at the left member in slot 1
+    const T z0 = fma(r, e, v[0]);             // rhs of Eq (1) at the right member in slot 0
+    const T zin = from_right<T, XW>(c, z0, buf);
+    // node 1 when it is single (partner is node 0): only lane is_lo reads x0 later
+    x0 = fma(-c.e, z0 - c.lo, z0);
+#pragma unroll
+    for (int m = 1; m < C / 2; ++m) {
+        e = v[2 * m + 1] - v[2 * m];
+        const T pm = fma(-r, e, v[2 * m + 1]);
+        const T zm = fma(r, e, v[2 * m]);
+        const T t = zm - pprev;               // pair (slots 2m-1, 2m): q = z_m, p = p_{m-1}
+        v[2 * m - 2] = fma(g, t, pprev);
+        v[2 * m - 1] = fma(-g, t, zm);
+        pprev = pm;
+    }
+    const T ql = c.is_hi ? c.hi : zin;        // (N, N+1): the boundary value is the new-level neighbour
+    const T gl = c.is_hi ? c.e : g;
+    const T t = ql - pprev;
+    v[C - 2] = fma(gl, t, pprev);
+    const T last = fma(-gl, t, ql);
+    v[C - 1] = c.is_hi ? c.hi : last;         // the ghost stays pinned
+}
+
+// L: shifted state -> even state, left members at odd slots of the shifted window (a phase-0 level).
+template <typename T, int C, bool XW>
+__device__ __forceinline__ void level_L(T (&v)[C], const T x0, const ResidentCtx<T, XW>& c, int buf) {
+    const T r = c.r, g = c.g;
+    T e = v[C - 1] - v[C - 2];
+    const T plast = fma(-r, e, v[C - 1]);     // p of the pair this lane hands to the next one
+    T znext = fma(r, e, v[C - 2]);
+    const T pin = from_left<T, XW>(c, plast, buf);
+#pragma unroll
+    for (int m = C / 2 - 2; m >= 0; --m) {
+        e = v[2 * m + 1] - v[2 * m];
+        const T pm = fma(-r, e, v[2 * m + 1]);
+        const T zm = fma(r, e, v[2 * m]);
+        const T t = znext - pm;               // pair (slots 2m+1, 2m+2) lands in slots 2m+2, 2m+3
+        v[2 * m + 2] = fma(g, t, pm);
+        v[2 * m + 3] = fma(-g, t, znext);
+        znext = zm;
+    }
+    const T pl = fma(-r, x0 - c.lo, x0);      // pair (1,2): left member is x0, its left neighbour node 0
+    const T P = c.is_lo ? pl : pin;
+    const T t = znext - P;
+    v[0] = fma(g, t, P);
+    v[1] = fma(-g, t, znext);
+}
+
+// I: even state -> even state, pairs (slots 2m, 2m+1) inside the lane (a phase-0 level).
+template <typename T, int C, bool XW>
+__device__ __forceinline__ void level_I(T (&v)[C], const ResidentCtx<T, XW>& c, int buf) {
+    const T r = c.r, g = c.g;
+    T a = from_left<T, XW>(c, v[C - 1], buf);
+    T d = from_right<T, XW>(c, v[0], buf);
+    if (c.is_lo) a = c.lo;
+    if (c.is_hi) d = c.hi;
+#pragma unroll
+    for (int m = 0; m < C / 2; ++m) {
+        const T b = v[2 * m], cc = v[2 * m + 1];
+        const T dd = (m == C / 2 - 1) ? d : v[2 * m + 2];
+        const T p = fma(r, a - b, b);
+        const T q = fma(r, dd - cc, cc);
+        const T t = q - p;
+        a = cc;
+        v[2 * m] = fma(g, t, p);
+        v[2 * m + 1] = fma(-g, t, q);
+    }
+}
+
+// shifted state -> even state without a level (after a lone R at the end of a run)
+template <typename T, int C, bool XW>
+__device__ __forceinline__ void unshift(T (&v)[C], const T x0, const ResidentCtx<T, XW>& c, int buf) {
+    T left = from_left<T, XW>(c, v[C - 1], buf);
+    if (c.is_lo) left = x0;
+#pragma unroll
+    for (int j = C - 1; j >= 1; --j) v[j] = v[j - 1];
+    v[0] = left;
+}
+
+// ------------------------------------------------------------------ (i) rod per CTA ------
+template <typename T, int C, int W>
+__global__ void __launch_bounds__(32 * W)
+ge1d_rod_resident_kernel(T* u, int64_t nx, int64_t batch, const Coef1<T>* __restrict__ coef,
+                         int phase0, int64_t steps) {
+    constexpr int V = VecOf<T>::V;
+    constexpr bool XW = W > 1;
+    static_assert(C % 2 == 0 && C % V == 0, "C must hold whole pairs and whole vectors");
+    __shared__ T sx[4 * W];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gl = warp * 32 + lane;                 // lane index within the rod
+    const int used = (int)(nx / C);                  // lanes that hold nodes
+    for (int64_t rod = blockIdx.x; rod < batch; rod += gridDim.x) {
+        const Coef1<T> k = coef[rod];
+        ResidentCtx<T, XW> c;
+        c.r = k.r; c.g = k.g; c.e = k.e; c.lo = k.lo; c.hi = k.hi;
+        c.is_lo = gl == 0; c.is_hi = gl == used - 1;
+        c.lane = lane; c.warp = warp; c.nwarps = W; c.sx = sx;
+        T* row = u + rod * nx + (int64_t)gl * C;
+        T v[C];
+        T x0 = T(0);
+        if (gl < used) {
+#pragma unroll
+            for (int j = 0; j < C / V; ++j) {
+                T t[V];
+                ld_vec_plain(row + j * V, t);
+#pragma unroll
+                for (int i = 0; i < V; ++i) v[j * V + i] = t[i];
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < C; ++j) v[j] = k.hi;
+        }
+        int64_t left = steps;
+        int buf = 0;
+        if (phase0 == 0 && left > 0) { level_I<T, C, XW>(v, c, buf); buf ^= 1; --left; }
+#pragma unroll 1
+        for (; left >= 2; left -= 2) {
+            level_R<T, C, XW>(v, x0, c, buf);
+            level_L<T, C, XW>(v, x0, c, buf ^ 1);
+        }
+        if (left) {
+            level_R<T, C, XW>(v, x0, c, buf);
+            unshift<T, C, XW>(v, x0, c, buf ^ 1);
+        }
+        if (gl < used) {
+#pragma unroll
+            for (int j = 0; j < C / V; ++j) {
+                T t[V];
+#pragma unroll
+                for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
+                st_vec(row + j * V, t);
+            }
+        }
+        if constexpr (XW) __syncthreads();           // the exchange slots are reused by the next rod
+    }
+}
+
+template <typename T, int C, int W>
+inline cudaError_t rod_resident_launch(T* u, int64_t nx, int64_t batch, const Coef1<T>* coef, int phase0,
+                                       int64_t steps, cudaStream_t s) {
+    const unsigned grid = (unsigned)(batch < (1 << 30) ? batch : (1 << 30));
+    ge1d_rod_resident_kernel<T, C, W><<<grid, 32 * W, 0, s>>>(u, nx, batch, coef, phase0, steps);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ (ii) one rod on the whole chip ------
+constexpr int kGridWarps = 4;              // warps (tiles) per CTA
+constexpr int kSyncFlags = 0, kSyncGrid = 1;
+
+struct GridResidentArgs {
+    int64_t nx;
+    int64_t ntiles;
+    int64_t steps;
+    int phase0;
+    int hl;            // halo lanes per side
+    int tb;            // levels between two meetings, <= hl*C
+    int sync_mode;     // kSyncFlags / kSyncGrid
+    unsigned epoch0;   // flag value all tiles had when the launch started
+};
+
+// number of meetings of a run (the same loop as in the kernel); host and device
+__host__ __device__ inline int64_t grid_resident_meetings(int64_t steps, int phase0, int tb) {
+    int64_t left = steps, n = 0;
+    int usedl = 0;
+    if (phase0 == 0 && left > 0) { usedl = 2; --left; }
+    while (left >= 2) {
+        if (usedl + 2 > tb) { ++n; usedl = 0; }
+        usedl += 2; left -= 2;
+    }
+    if (left) { if (usedl + 2 > tb) { ++n; usedl = 0; } }
+    return n;
+}
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Spin until *p has reached `target` (wrap-safe).  Bounded: a tile that never arrives (which a
+// cooperative launch rules out) ends the wait after ~1 s and is reported through `fault`.
+__device__ __forceinline__ void wait_flag(const unsigned* p, unsigned target, unsigned* fault) {
+    for (unsigned it = 0; it < (1u << 24); ++it) {
+        if ((int)(ld_acquire_u32(p) - target) >= 0) return;
+        if (it > 64) __nanosleep(40);
+    }
+    atomicExch(fault, 1u);
+}
+
+template <typename T, int C>
+__global__ void __launch_bounds__(32 * kGridWarps)
+ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsigned* flags, unsigned* fault,
+                          const GridResidentArgs a) {
+    constexpr int V = VecOf<T>::V;
+    static_assert(C % 2 == 0 && C % V == 0, "C must hold whole pairs and whole vectors");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kGridWarps + warp;
+    const bool active = tile < a.ntiles;
+    const int hl = a.hl;
+    const int64_t valid = (int64_t)(32 - 2 * hl) * C;
+    const int64_t e0 = tile * valid + (int64_t)(lane - hl) * C;      // element in slot 0 (even state)
+    const bool inside = active && e0 >= 0 && e0 < a.nx;
+    const Coef1<T> k = coef[0];
+    ResidentCtx<T, false> c;
+    c.r = k.r; c.g = k.g; c.e = k.e; c.lo = k.lo; c.hi = k.hi;
+    c.is_lo = active && e0 == 0; c.is_hi = active && e0 + C == a.nx;
+    c.lane = lane; c.warp = warp; c.nwarps = kGridWarps; c.sx = nullptr;
+    cg::grid_group grid = cg::this_grid();
+
+    T v[C];
+    T x0 = T(0);
+    if (inside) {
+#pragma unroll
+        for (int j = 0; j < C / V; ++j) {
+            T t[V];
+            ld_vec_plain(u + e0 + j * V, t);
+#pragma unroll
+            for (int i = 0; i < V; ++i) v[j * V + i] = t[i];
+        }
+    } else {
+        const T f = e0 < 0 ? k.lo : k.hi;
+#pragma unroll
+        for (int j = 0; j < C; ++j) v[j] = f;
+    }
+    // stage 0: every tile has read its window; nobody may overwrite u before its neighbours did
+    unsigned stage = a.epoch0 + 1;
+    const bool own_l = lane >= hl && lane < 2 * hl;                   // outermost valid lanes
+    const bool own_r = lane >= 32 - 2 * hl && lane < 32 - hl;
+    const bool halo_l = lane < hl, halo_r = lane >= 32 - hl;
+    const bool has_l = active && tile > 0, has_r = active && tile + 1 < a.ntiles;
+    const size_t side = (size_t)hl * C;                               // elements per published side
+    auto signal = [&]() {
+        if (a.sync_mode == kSyncGrid) { grid.sync(); return; }
+        if (!active) return;
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) st_release_u32(flags + tile, stage);
+    };
+    auto await = [&]() {
+        if (a.sync_mode == kSyncGrid || !active) return;
+        if (halo_l && has_l) wait_flag(flags + tile - 1, stage, fault);
+        if (halo_r && has_r) wait_flag(flags + tile + 1, stage, fault);
+        __syncwarp();
+    };
+    signal();
+
+    int parity = 0;
+    auto meet = [&]() {
+        // publish the outermost valid lanes, meet the neighbours, refresh the halo lanes
+        ++stage;
+        if (active) {
+            T* mine = xbuf + ((size_t)parity * a.ntiles + tile) * 2 * side;
+            if (own_l || own_r) {
+                T* dst = mine + (own_l ? (size_t)(lane - hl) * C : side + (size_t)(lane - (32 - 2 * hl)) * C);
+#pragma unroll
+                for (int j = 0; j < C / V; ++j) {
+                    T t[V];
+#pragma unroll
+                    for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
+                    st_vec_cg(dst + j * V, t);
+                }
+            }
+        }
+        signal();
+        await();
+        if (active) {
+            const T* src = nullptr;
+            if (halo_l && has_l)      // the left neighbour's right side
+                src = xbuf + ((size_t)parity * a.ntiles + tile - 1) * 2 * side + side + (size_t)lane * C;
+            else if (halo_r && has_r) // the right neighbour's left side
+                src = xbuf + ((size_t)parity * a.ntiles + tile + 1) * 2 * side + (size_t)(lane - (32 - hl)) * C;
+            if (src) {
+#pragma unroll
+                for (int j = 0; j < C / V; ++j) {
+                    T t[V];
+                    ld_vec_cg(src + j * V, t);
+#pragma unroll
+                    for (int i = 0; i < V; ++i) v[j * V + i] = t[i];
+                }
+            }
+        }
+        parity ^= 1;
+    };
+
+    int64_t left = a.steps;
+    int usedl = 0;
+    if (a.phase0 == 0 && left > 0) { level_I<T, C, false>(v, c, 0); usedl = 2; --left; }
+#pragma unroll 1
+    while (left >= 2) {
+        if (usedl + 2 > a.tb) { meet(); usedl = 0; }
+        level_R<T, C, false>(v, x0, c, 0);
+        level_L<T, C, false>(v, x0, c, 0);
+        usedl += 2; left -= 2;
+    }
+    if (left) {
+        if (usedl + 2 > a.tb) { meet(); usedl = 0; }
+        level_R<T, C, false>(v, x0, c, 0);
+        unshift<T, C, false>(v, x0, c, 0);
+    }
+    // with no meeting at all the neighbours may still be reading u: wait for their stage 0
+    if (stage == a.epoch0 + 1) await();
+    if (inside && lane >= hl && lane < 32 - hl) {
+#pragma unroll
+        for (int j = 0; j < C / V; ++j) {
+            T t[V];
+#pragma unroll
+            for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
+            st_vec(u + e0 + j * V, t);
+        }
+    }
+}
+
+}  // namespace ge

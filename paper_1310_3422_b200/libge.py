@@ -22,7 +22,11 @@ GE_F32, GE_F64 = 0, 1
 GE_KERNEL_AUTO, GE_KERNEL_PER_STEP, GE_KERNEL_TEMPORAL, GE_KERNEL_PERSISTENT = 0, 1, 2, 3
 GE_OK, GE_EINVAL, GE_ENOMEM, GE_ECUDA, GE_EUNSUPPORTED = 0, -1, -2, -3, -4
 GE_INFO_KERNEL, GE_INFO_TB, GE_INFO_LAUNCHES, GE_INFO_TILE_VALID, GE_INFO_TILE_LOADED = 0, 1, 2, 3, 4
+(GE_INFO_RESIDENT_PATH, GE_INFO_RESIDENT_C, GE_INFO_RESIDENT_WARPS, GE_INFO_RESIDENT_CAPACITY,
+ GE_INFO_RESIDENT_TB, GE_INFO_MEETINGS, GE_INFO_SYNC_FAULT) = 5, 6, 7, 8, 9, 10, 11
 GE_TUNE_TEMPORAL_C, GE_TUNE_TB, GE_TUNE_SEG_PAIRS = 0, 1, 2
+GE_TUNE_RESIDENT_C, GE_TUNE_HALO_LANES, GE_TUNE_SYNC_MODE = 3, 4, 5
+GE_SYNC_FLAGS, GE_SYNC_GRID = 0, 1
 
 KERNEL_NAMES = {0: "auto", 1: "per_step", 2: "temporal", 3: "persistent"}
 _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
@@ -214,4 +218,14 @@ class Plan:
                     tb=ge_plan_info(self.handle, GE_INFO_TB),
                     launches=ge_plan_info(self.handle, GE_INFO_LAUNCHES),
                     tile_valid=ge_plan_info(self.handle, GE_INFO_TILE_VALID),
-                    tile_loaded=ge_plan_info(self.handle, GE_INFO_TILE_LOADED))
+                    tile_loaded=ge_plan_info(self.handle, GE_INFO_TILE_LOADED),
+                    resident_path=ge_plan_info(self.handle, GE_INFO_RESIDENT_PATH),
+                    resident_c=ge_plan_info(self.handle, GE_INFO_RESIDENT_C),
+                    resident_warps=ge_plan_info(self.handle, GE_INFO_RESIDENT_WARPS),
+                    resident_capacity=ge_plan_info(self.handle, GE_INFO_RESIDENT_CAPACITY),
+                    resident_tb=ge_plan_info(self.handle, GE_INFO_RESIDENT_TB),
+                    meetings=ge_plan_info(self.handle, GE_INFO_MEETINGS))
+
+    def sync_fault(self) -> int:
+        """1 if a tile of the whole-chip persistent kernel gave up waiting (synchronises)."""
+        return ge_plan_info(self.handle, GE_INFO_SYNC_FAULT)

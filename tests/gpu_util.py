@@ -4,7 +4,8 @@ import numpy as np
 _TORCH_DT = {"f32": "float32", "f64": "float64"}
 
 
-def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0):
+def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc=0, hl=0, sync=None, rtb=0,
+            chunks=None):
     """Run `steps` levels on cuda:0 and return the final state as a numpy array."""
     import torch
     from paper_1310_3422_b200 import libge
@@ -17,7 +18,19 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0):
             plan.tune(libge.GE_TUNE_TEMPORAL_C, tc)
         if hp:
             plan.tune(libge.GE_TUNE_SEG_PAIRS, hp)
-        if via == "run":
+        if rc:
+            plan.tune(libge.GE_TUNE_RESIDENT_C, rc)
+        if hl:
+            plan.tune(libge.GE_TUNE_HALO_LANES, hl)
+        if sync is not None:
+            plan.tune(libge.GE_TUNE_SYNC_MODE, sync)
+        if rtb:
+            plan.tune(libge.GE_TUNE_TB, rtb)
+        if via == "run" and chunks:
+            for c in chunks:                      # the same run cut into several ge_run calls
+                plan.run(u.data_ptr(), c, stream)
+            assert sum(chunks) == steps
+        elif via == "run":
             plan.run(u.data_ptr(), steps, stream)
         elif via == "step":
             v = torch.empty_like(u)
@@ -34,6 +47,8 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0):
         torch.cuda.synchronize(dev)
         assert plan.level == level0 + steps
         info = plan.info()
+        if info["resident_path"] == 2:
+            assert plan.sync_fault() == 0
     return u.cpu().numpy(), info
 
 

@@ -120,6 +120,80 @@ def test_run_host_matches_run(oracle):
     np.testing.assert_array_equal(a, b)
 
 
+# ------------------------------------------------------------------ strategy C, 1-D ------
+@pytest.mark.parametrize("dtype,n,rc", [("f32", 64, 0), ("f32", 512, 16), ("f32", 4096, 0), ("f32", 4096, 64),
+                                        ("f32", 4096, 32), ("f32", 2048 + 128, 0), ("f32", 96, 0), ("f32", 16384, 0),
+                                        ("f64", 8, 0), ("f64", 64, 0), ("f64", 2048, 0), ("f64", 2048, 32),
+                                        ("f64", 2048, 16), ("f64", 1000, 8), ("f64", 16384, 64)])
+def test_persistent_rods(oracle, dtype, n, rc):
+    """Strategy C, path 1 (a rod per CTA, state in registers for the whole run): one launch whatever
+    the number of levels; one warp (shuffles only) and several warps (shared-memory edge exchange);
+    lanes and warps that hold no nodes; both starting phases, odd and even level counts; per-rod r
+    and unequal boundary values.  Must equal the per-level kernel bit for bit."""
+    cfg = inputs.random_rods(5, n, dtype, seed=3 * n + rc)
+    for level0, steps in ((0, 1), (1, 1), (0, 2), (1, 2), (0, 37), (1, 64), (0, 301)):
+        got, info = run_gpu(cfg, steps, kernel="persistent", level0=level0, rc=rc)
+        assert info["kernel"] == "persistent" and info["resident_path"] == 1 and info["launches"] == 1, info
+        if rc:
+            assert info["resident_c"] == rc
+        ref = run_oracle(oracle, cfg, steps, level0=level0)
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (n, level0, steps, info)
+        same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+        np.testing.assert_array_equal(got, same, err_msg=str((dtype, n, level0, steps, info)))
+
+
+@pytest.mark.parametrize("dtype,n,rc,hl,rtb,sync", [
+    ("f64", 4096, 0, 0, 0, None), ("f64", 4096, 16, 0, 0, None), ("f64", 30720, 0, 0, 6, None),
+    ("f64", 100000, 0, 2, 0, None), ("f64", 100000, 16, 3, 10, 1), ("f64", 2 ** 20, 0, 0, 0, None),
+    ("f64", 2 ** 20, 0, 0, 0, 1), ("f32", 16384 * 4, 0, 0, 0, None), ("f32", 200000 - 200000 % 64, 32, 2, 20, None),
+    ("f32", 2 ** 20, 0, 0, 0, 1)])
+def test_persistent_whole_chip(oracle, dtype, n, rc, hl, rtb, sync):
+    """Strategy C, path 2 (one rod spread over the chip by a cooperative launch, tiles meet every tb
+    levels): neighbour flags and grid-wide barrier, one and several halo lanes, many meetings, no
+    meeting, ragged last tile, both starting phases, odd level counts, and several ge_run calls on
+    one plan (the flag epoch carries over).  Must equal the per-level kernel bit for bit."""
+    cfg = inputs.random_rods(1, n, dtype, seed=n % 1000 + rc + hl)
+    for level0, steps, chunks in ((0, 1, None), (1, 2, None), (0, 40, None), (1, 77, None), (0, 203, (100, 3, 100))):
+        got, info = run_gpu(cfg, steps, kernel="persistent", level0=level0, rc=rc, hl=hl, rtb=rtb, sync=sync,
+                            chunks=chunks)
+        assert info["kernel"] == "persistent" and info["resident_path"] == 2, info
+        assert info["launches"] == (len(chunks) if chunks else 1)
+        assert info["resident_warps"] <= info["resident_capacity"]
+        if steps > 2 * info["resident_tb"]:
+            assert info["meetings"] >= steps // info["resident_tb"] - 3
+        same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+        np.testing.assert_array_equal(got, same, err_msg=str((dtype, n, level0, steps, info)))
+    ref = run_oracle(oracle, cfg, 77, level0=1)
+    got, _ = run_gpu(cfg, 77, kernel="persistent", level0=1, rc=rc, hl=hl, rtb=rtb, sync=sync)
+    assert rel_err_rows(got, ref, cfg) <= TOL[dtype]
+
+
+def test_persistent_falls_back_when_the_shape_does_not_fit(oracle):
+    # odd N: no resident kernel, no vector kernel either -> per-level launches
+    cfg = inputs.random_rods(2, 1001, "f64", seed=5)
+    got, info = run_gpu(cfg, 20, kernel="persistent")
+    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 20
+    assert rel_err_rows(got, run_oracle(oracle, cfg, 20), cfg) <= TOL["f64"]
+    # 2-D: strategy C is 1-D only
+    cfg = inputs.random_grid(64, 64, "f32", seed=6)
+    got, info = run_gpu(cfg, 16, kernel="persistent")
+    assert info["kernel"] == "temporal" and info["resident_path"] == 0
+    assert rel_err(got, run_oracle(oracle, cfg, 16)) <= TOL["f32"]
+    # batched rods too long for a CTA
+    cfg = inputs.random_rods(2, 128 * 32 * 8 * 2, "f32", seed=7)
+    got, info = run_gpu(cfg, 33, kernel="persistent")
+    assert info["kernel"] == "temporal" and info["launches"] < 33
+    assert rel_err_rows(got, run_oracle(oracle, cfg, 33), cfg) <= TOL["f32"]
+
+
+def test_auto_picks_the_resident_kernels_when_the_state_fits_on_chip():
+    for cfg, path in ((inputs.make_c1(), 1), (inputs.make_c3(batch=4, n=4096, steps=10), 1),
+                      (inputs.make_c2(n=2 ** 20, steps=10), 2), (inputs.make_c4(n=2 ** 24, steps=10), 0)):
+        _, info = run_gpu(cfg, 10)
+        assert info["resident_path"] == path, (cfg["name"], info)
+        assert info["kernel"] == ("persistent" if path else "temporal")
+
+
 # ------------------------------------------------------------------ 2-D ------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("nx,ny", [(1, 1), (2, 2), (3, 3), (4, 4), (5, 4), (4, 7), (8, 8), (64, 32), (130, 67), (131, 66), (256, 256)])
