@@ -227,6 +227,14 @@ def run_ours(args):
     host0 = torch.from_numpy(cfg["u0"].reshape(-1))
     u = host0.to(dev)
     plan = libge.Plan(cfg, kernel=args.kernel, tb=args.tb, stream=stream)
+    if args.rc:
+        plan.tune(libge.GE_TUNE_RESIDENT_C, args.rc)
+    if args.hl:
+        plan.tune(libge.GE_TUNE_HALO_LANES, args.hl)
+    if args.sync:
+        plan.tune(libge.GE_TUNE_SYNC_MODE, {"flags": libge.GE_SYNC_FLAGS, "grid": libge.GE_SYNC_GRID, "lines": libge.GE_SYNC_LINES}[args.sync])
+    if args.rtb:
+        plan.tune(libge.GE_TUNE_TB, args.rtb)
     info0 = plan.info()
 
     # ---- device-resident timing: W warm-up steps, then exactly K timed steps ----
@@ -234,7 +242,7 @@ def run_ours(args):
         plan.run(u.data_ptr(), levels, stream)
     barrier()
     clocks = ClockSampler(local) if rank == 0 else None
-    l0 = plan.info()["launches"]
+    l0, m0 = plan.info()["launches"], plan.info()["meetings"]
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
     if clocks:
@@ -249,6 +257,7 @@ def run_ours(args):
     total_ms = ev[0].elapsed_time(ev[-1])
     per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     launches = plan.info()["launches"] - l0
+    meetings = plan.info()["meetings"] - m0
     tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -256,8 +265,9 @@ def run_ours(args):
     value = units(cfg) * args.steps * world / (total_ms_max * 1e-3) / 1e9
     finite = bool(torch.isfinite(u).all().item())
 
-    # ---- dominant kernel alone: m back-to-back launches between two events on the launching stream ----
-    roof = dominant_kernel_roofline(plan, u, cfg, info0, stream_obj, stream, dev, args)
+    # ---- roofline of the dominant kernel: its average launch duration over the timed region ----
+    roof = roofline(cfg, info0, total_ms, launches, args.steps)
+    fault = plan.sync_fault() if info0["resident_path"] == 2 else 0
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -314,13 +324,18 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
         "config": {"workload": workload_desc(cfg), "levels_per_step": levels, "kernel": info["kernel"],
-                   "tb": info["tb"], "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "tb": info["resident_tb"] if info["resident_path"] == 2 else (0 if info["resident_path"] else info["tb"]),
+                   "resident": {"path": info["resident_path"], "c": info["resident_c"],
+                                "warps": info["resident_warps"], "capacity": info["resident_capacity"],
+                                "meetings_per_step": meetings // max(1, args.steps),
+                                "sync": args.sync or "grid"} if info["resident_path"] else None,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "state %.0f MiB %s L2 (126 MB)" % (nelem * es / 2 ** 20,
                                                               "larger than" if nelem * es > 126e6 else "fits in"),
                    "r": float(cfg["r"][0]) if cfg["batch"] == 1 else "per rod U[0.5,8]"},
         "effective_gbs": value * 2 * es,            # what one-round-trip-per-level would have had to move
         "ms_per_step_each": per_step,
-        "finite": finite,
+        "finite": finite and not fault,
         "gpu_launches": launches,
         "roofline": roof,
         "e2e": e2e,
@@ -340,38 +355,60 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
-def dominant_kernel_roofline(plan, u, cfg, info0, stream_obj, stream, dev, args):
-    """Average launch duration of the kernel that dominates the step, CUDA events on the launching
-    stream, and the roofline fraction it reaches."""
-    import torch
+# fp32 / fp64 lanes per SM and the SM count the ALU peak is derived from
+LANES = {"f32": 128, "f64": 64}
+SMS = 148
+# floating-point instructions and flops (FMA = 2) per node update of the factored forms
+INSTR = {1: 3.0, 2: 6.75}
+FLOPS = {1: 5.0, 2: 9.75}
+
+
+def traffic_of(kernel_key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full
+    captures (profiles/traffic.json), or None when this kernel/workload has not been captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(kernel_key, {}).get("dram_bytes_per_launch")
+
+
+def roofline(cfg, info, total_ms, launches, steps):
+    """The step is `launches/steps` launches of ONE kernel; its average duration is the CUDA-event
+    time of the timed region divided by the launches in it.  Per-level kernel: HBM-bound, achieved =
+    algorithmic bytes (2*sizeof(T) per update) per second against the measured copy
+    rate.  Temporally blocked and resident kernels: bound by the plain fp32/fp64 pipes, achieved =
+    flops of the factored form per second against 2 x lanes x SMs x max clock."""
     es = ESIZE[cfg["dtype"]]
     nelem = cfg["nx"] * cfg["ny"] * cfg["batch"]
     peaks, src = measured_peaks()
-    kernel, tb = info0["kernel"], info0["tb"]
-    lv_per_launch = tb if kernel == "temporal" and tb > 0 else 1
-    m = max(4, min(64, (cfg["steps"] // lv_per_launch)))
-    plan.level = 1                       # a run of m*tb levels from an odd level is m identical launches
-    for _ in range(2):
-        plan.run(u.data_ptr(), lv_per_launch * 2, stream)
-    torch.cuda.synchronize(dev)
-    plan.level = 1
-    l0 = plan.info()["launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream_obj)
-    plan.run(u.data_ptr(), lv_per_launch * m, stream)
-    e1.record(stream_obj)
-    torch.cuda.synchronize(dev)
-    n_l = plan.info()["launches"] - l0
-    ms = e0.elapsed_time(e1) / n_l
-    alg_bytes = 2.0 * es * nelem * lv_per_launch           # SURVEY.md 8(d): 2*sizeof(T) per update
-    achieved = alg_bytes / (ms * 1e-3) / 1e9
-    out = {"kernel": "ge%dd_%s_kernel<%s>" % (cfg["dim"], "temporal" if lv_per_launch > 1 else "level", cfg["dtype"]),
-           "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-           "frac": achieved / peaks["hbm_gbs"], "peak_source": src, "traffic": None,
-           "levels_per_launch": lv_per_launch, "launches_timed": n_l, "ms_per_launch": ms,
-           "algorithmic_bytes_per_launch": alg_bytes,
-           "compulsory_bytes_per_launch": 2.0 * es * nelem,
-           "compulsory_gbs": 2.0 * es * nelem / (ms * 1e-3) / 1e9}
+    kernel = info["kernel"]
+    ms = total_ms / max(launches, 1)
+    lv = cfg["steps"] * steps / max(launches, 1)            # levels per launch (average)
+    upd = nelem * lv                                        # updates per launch
+    names = {"per_step": "ge%dd_level_kernel", "temporal": "ge%dd_temporal_kernel"}
+    if kernel == "persistent":
+        name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
+    else:
+        name = names[kernel] % cfg["dim"]
+    name = "%s<%s>" % (name, cfg["dtype"])
+    key = "%s/%s" % (cfg["name"], name)
+    eff = 2.0 * es * upd / (ms * 1e-3) / 1e9
+    out = {"kernel": name, "levels_per_launch": lv, "launches_timed": launches, "ms_per_launch": ms,
+           "traffic": traffic_of(key), "peak_source": src,
+           "algorithmic_bytes_per_launch": 2.0 * es * upd, "effective_gbs": eff,
+           "effective_frac_of_hbm": eff / peaks["hbm_gbs"]}
+    if kernel == "per_step" or lv <= 1.0:
+        out.update({"bound": "hbm", "achieved": eff, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": eff / peaks["hbm_gbs"]})
+    else:
+        clk = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        peak = 2.0 * LANES[cfg["dtype"]] * SMS * clk / 1e12
+        ach = FLOPS[cfg["dim"]] * upd / (ms * 1e-3) / 1e12
+        out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                    "issue_frac": INSTR[cfg["dim"]] * upd / (ms * 1e-3) / (LANES[cfg["dtype"]] * SMS * clk),
+                    "peak_derivation": "2 flop x %d %s lanes/SM x %d SMs x %.0f MHz" % (
+                        LANES[cfg["dtype"]], cfg["dtype"], SMS, clk / 1e6)})
     return out
 
 
@@ -384,6 +421,10 @@ def main():
     ap.add_argument("--config", default="c4")
     ap.add_argument("--kernel", default="auto")
     ap.add_argument("--tb", type=int, default=0)
+    ap.add_argument("--rc", type=int, default=0, help="persistent kernels: values per lane")
+    ap.add_argument("--hl", type=int, default=0, help="whole-chip persistent kernel: halo lanes per side")
+    ap.add_argument("--rtb", type=int, default=0, help="whole-chip persistent kernel: levels between meetings")
+    ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines"], help="whole-chip persistent kernel: meeting kind")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

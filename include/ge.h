@@ -134,10 +134,11 @@ enum {
                                   2-D: one of the compiled-in block lengths 4, 8)                            */
     GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 64)       */
     GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
-                                  long rod: 16, 32 (f64) / 32, 64 (f32)); may synchronise and reallocate      */
-    GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8 (tb <= lanes * C); may synchronise      */
-    GE_TUNE_SYNC_MODE = 5      /* path 2: 0 = neighbour flags (release/acquire per tile), 1 = grid-wide
-                                  barrier (cooperative groups) at every meeting                             */
+                                  long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
+    GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */
+    GE_TUNE_SYNC_MODE = 5      /* path 2, how the tiles meet: 0 = neighbour flags (data, release fence, flag per
+                                  tile, acquire), 1 = grid-wide barrier (cooperative groups), 2 = neighbour
+                                  flag-in-data lines (no fence, no separate flag); default 1, the fastest measured               */
 };
 int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
 

@@ -275,7 +275,7 @@ int launch_rod_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     return GE_OK;
 }
 
-// Path 2: the grid-resident kernel is instantiated for the two largest C of the dtype.
+// Path 2: the grid-resident kernel is instantiated for the three largest C of the dtype.
 template <typename T, int C>
 const void* grid_resident_fn() { return (const void*)&ge::ge1d_grid_resident_kernel<T, C>; }
 
@@ -283,9 +283,11 @@ const void* grid_resident_fn_for(int dtype, int c) {
     if (dtype == GE_F64) {
         if (c == 16) return grid_resident_fn<double, 16>();
         if (c == 32) return grid_resident_fn<double, 32>();
+        if (c == 64) return grid_resident_fn<double, 64>();
     } else {
         if (c == 32) return grid_resident_fn<float, 32>();
         if (c == 64) return grid_resident_fn<float, 64>();
+        if (c == 128) return grid_resident_fn<float, 128>();
     }
     return nullptr;
 }
@@ -314,8 +316,10 @@ int grid_resident_configure(ge_plan* p) {
     GE_CUDA(cudaStreamSynchronize(p->last_stream));      // an earlier launch may still use the old ones
     cudaFree(p->res_xbuf); cudaFree(p->res_flags);
     p->res_xbuf = nullptr; p->res_flags = nullptr;
-    const size_t xb = (size_t)2 * tiles * 2 * p->res_hl * p->res_c * elem_size(p->dtype);
+    // sized for the flag-in-data lines: 16 bytes per fp64 value (8 per fp32 value)
+    const size_t xb = (size_t)2 * tiles * 2 * p->res_hl * p->res_c * 2 * elem_size(p->dtype);
     GE_CUDA(cudaMalloc(&p->res_xbuf, xb));
+    GE_CUDA(cudaMemset(p->res_xbuf, 0, xb));
     GE_CUDA(cudaMalloc((void**)&p->res_flags, (size_t)(tiles + 1) * sizeof(unsigned)));
     GE_CUDA(cudaMemset(p->res_flags, 0, (size_t)(tiles + 1) * sizeof(unsigned)));
     p->res_epoch = 0;
@@ -339,7 +343,9 @@ int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(ctas), dim3(32 * ge::kGridWarps), args, 0, s);
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     const int64_t meet = ge::grid_resident_meetings(steps, a.phase0, a.tb);
-    if (p->res_sync == ge::kSyncFlags) p->res_epoch += (unsigned)(1 + meet);
+    // every launch moves the epoch past all flag values / line tags it used (one extra meeting is held
+    // by the flag-in-data mode when the run has none)
+    p->res_epoch += (unsigned)(2 + meet);
     p->meetings += meet;
     p->launches += 1;
     p->level += steps;
@@ -441,8 +447,8 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->tb = 0;
     p->tc = default_tc(p->dtype);
     p->hp = 64;
-    p->res_hl = 1;
-    p->res_sync = ge::kSyncFlags;
+    p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
+    p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
     if (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT) {
         p->res_tb = d->tb;
@@ -597,6 +603,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             // path 1: values per lane (warps follow); path 2: values per lane of a tile
             if (p->kernel != GE_KERNEL_PERSISTENT || value < 2 || value > 128) return GE_EINVAL;
             const int32_t path0 = p->res_path, c0 = p->res_c, w0 = p->res_w;
+            p->res_tb = 0;                                     // back to the largest the new halo allows
             int rc = resident_configure(p, (int)value);
             if (rc != GE_OK) return rc;
             if (p->res_path == 0) {                            // not instantiated / does not fit: restore
@@ -621,7 +628,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         }
         case GE_TUNE_SYNC_MODE:
             if (p->kernel != GE_KERNEL_PERSISTENT || p->res_path != 2) return GE_EINVAL;
-            if (value != ge::kSyncFlags && value != ge::kSyncGrid) return GE_EINVAL;
+            if (value != ge::kSyncFlags && value != ge::kSyncGrid && value != ge::kSyncLL) return GE_EINVAL;
             p->res_sync = (int32_t)value;
             return GE_OK;
         case GE_TUNE_TB:

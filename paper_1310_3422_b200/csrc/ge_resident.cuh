@@ -123,7 +123,9 @@ __device__ __forceinline__ T from_left(const ResidentCtx<T, XW>& c, T mine, int 
 }
 
 // R: even state -> shifted state, left members at odd slots (a phase-1 level).  In place.
-template <typename T, int C, bool XW>
+// BC = false: the lane group holds no boundary (interior tiles of ge_temporal.cuh): the boundary
+// selects and the x0 bookkeeping drop out at compile time.
+template <typename T, int C, bool XW, bool BC = true>
 __device__ __forceinline__ void level_R(T (&v)[C], T& x0, const ResidentCtx<T, XW>& c, int buf) {
     const T r = c.r, g = c.g;
     T e = v[1] - v[0];
@@ -131,7 +133,7 @@ __device__ __forceinline__ void level_R(T (&v)[C], T& x0, const ResidentCtx<T, X
     const T z0 = fma(r, e, v[0]);             // rhs of Eq (1) at the right member in slot 0
     const T zin = from_right<T, XW>(c, z0, buf);
     // node 1 when it is single (partner is node 0): only lane is_lo reads x0 later
-    x0 = fma(-c.e, z0 - c.lo, z0);
+    if constexpr (BC) x0 = fma(-c.e, z0 - c.lo, z0);
 #pragma unroll
     for (int m = 1; m < C / 2; ++m) {
         e = v[2 * m + 1] - v[2 * m];
@@ -142,16 +144,17 @@ __device__ __forceinline__ void level_R(T (&v)[C], T& x0, const ResidentCtx<T, X
         v[2 * m - 1] = fma(-g, t, zm);
         pprev = pm;
     }
-    const T ql = c.is_hi ? c.hi : zin;        // (N, N+1): the boundary value is the new-level neighbour
-    const T gl = c.is_hi ? c.e : g;
+    const bool hi = BC && c.is_hi;
+    const T ql = hi ? c.hi : zin;             // (N, N+1): the boundary value is the new-level neighbour
+    const T gl = hi ? c.e : g;
     const T t = ql - pprev;
     v[C - 2] = fma(gl, t, pprev);
     const T last = fma(-gl, t, ql);
-    v[C - 1] = c.is_hi ? c.hi : last;         // the ghost stays pinned
+    v[C - 1] = hi ? c.hi : last;              // the ghost stays pinned
 }
 
 // L: shifted state -> even state, left members at odd slots of the shifted window (a phase-0 level).
-template <typename T, int C, bool XW>
+template <typename T, int C, bool XW, bool BC = true>
 __device__ __forceinline__ void level_L(T (&v)[C], const T x0, const ResidentCtx<T, XW>& c, int buf) {
     const T r = c.r, g = c.g;
     T e = v[C - 1] - v[C - 2];
@@ -168,21 +171,24 @@ __device__ __forceinline__ void level_L(T (&v)[C], const T x0, const ResidentCtx
         v[2 * m + 3] = fma(-g, t, znext);
         znext = zm;
     }
-    const T pl = fma(-r, x0 - c.lo, x0);      // pair (1,2): left member is x0, its left neighbour node 0
-    const T P = c.is_lo ? pl : pin;
+    T P = pin;
+    if constexpr (BC) {
+        const T pl = fma(-r, x0 - c.lo, x0);  // pair (1,2): left member is x0, its left neighbour node 0
+        P = c.is_lo ? pl : pin;
+    }
     const T t = znext - P;
     v[0] = fma(g, t, P);
     v[1] = fma(-g, t, znext);
 }
 
 // I: even state -> even state, pairs (slots 2m, 2m+1) inside the lane (a phase-0 level).
-template <typename T, int C, bool XW>
+template <typename T, int C, bool XW, bool BC = true>
 __device__ __forceinline__ void level_I(T (&v)[C], const ResidentCtx<T, XW>& c, int buf) {
     const T r = c.r, g = c.g;
     T a = from_left<T, XW>(c, v[C - 1], buf);
     T d = from_right<T, XW>(c, v[0], buf);
-    if (c.is_lo) a = c.lo;
-    if (c.is_hi) d = c.hi;
+    if (BC && c.is_lo) a = c.lo;
+    if (BC && c.is_hi) d = c.hi;
 #pragma unroll
     for (int m = 0; m < C / 2; ++m) {
         const T b = v[2 * m], cc = v[2 * m + 1];
@@ -197,10 +203,10 @@ __device__ __forceinline__ void level_I(T (&v)[C], const ResidentCtx<T, XW>& c, 
 }
 
 // shifted state -> even state without a level (after a lone R at the end of a run)
-template <typename T, int C, bool XW>
+template <typename T, int C, bool XW, bool BC = true>
 __device__ __forceinline__ void unshift(T (&v)[C], const T x0, const ResidentCtx<T, XW>& c, int buf) {
     T left = from_left<T, XW>(c, v[C - 1], buf);
-    if (c.is_lo) left = x0;
+    if (BC && c.is_lo) left = x0;
 #pragma unroll
     for (int j = C - 1; j >= 1; --j) v[j] = v[j - 1];
     v[0] = left;
@@ -274,7 +280,9 @@ inline cudaError_t rod_resident_launch(T* u, int64_t nx, int64_t batch, const Co
 
 // ------------------------------------------------------------------ (ii) one rod on the whole chip ------
 constexpr int kGridWarps = 4;              // warps (tiles) per CTA
-constexpr int kSyncFlags = 0, kSyncGrid = 1;
+// how the tiles meet: 0 = per-tile flag with a release fence (neighbours only), 1 = grid-wide barrier,
+// 2 = flag-in-data lines, no fence and no separate flag (neighbours only; the default)
+constexpr int kSyncFlags = 0, kSyncGrid = 1, kSyncLL = 2;
 
 struct GridResidentArgs {
     int64_t nx;
@@ -283,7 +291,7 @@ struct GridResidentArgs {
     int phase0;
     int hl;            // halo lanes per side
     int tb;            // levels between two meetings, <= hl*C
-    int sync_mode;     // kSyncFlags / kSyncGrid
+    int sync_mode;     // kSyncFlags / kSyncGrid / kSyncLL
     unsigned epoch0;   // flag value all tiles had when the launch started
 };
 
@@ -301,22 +309,60 @@ __host__ __device__ inline int64_t grid_resident_meetings(int64_t steps, int pha
 }
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
-    unsigned v;
+    unsigned v;      // LDG.STRONG.GPU + CCTL.IVALL: no MEMBAR on the reader's side
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void st_relaxed_u32(unsigned* p, unsigned v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-// Spin until *p has reached `target` (wrap-safe).  Bounded: a tile that never arrives (which a
-// cooperative launch rules out) ends the wait after ~1 s and is reported through `fault`.
-__device__ __forceinline__ void wait_flag(const unsigned* p, unsigned target, unsigned* fault) {
+// One lane spins until BOTH neighbours' flags have reached `target` (wrap-safe); the two loads of a
+// round are in flight together.  Bounded: a tile that never arrives (which a cooperative launch rules
+// out) ends the wait after ~1 s and is reported through `fault`.
+__device__ __forceinline__ void wait_flags(const unsigned* pl, const unsigned* pr, unsigned target,
+                                           unsigned* fault) {
     for (unsigned it = 0; it < (1u << 24); ++it) {
-        if ((int)(ld_acquire_u32(p) - target) >= 0) return;
-        if (it > 64) __nanosleep(40);
+        const unsigned a = pl ? ld_acquire_u32(pl) : target;
+        const unsigned b = pr ? ld_acquire_u32(pr) : target;
+        if ((int)(a - target) >= 0 && (int)(b - target) >= 0) return;
+        if (it > 4096) __nanosleep(64);
     }
     atomicExch(fault, 1u);
 }
+
+// Flag-in-data exchange lines (the scheme of low-latency collectives): every 8-byte unit carries 32
+// bits of payload and the 32-bit meeting number, so a reader that sees the expected number in both
+// units of a 16-byte line has the payload -- no fence, no separate flag, one L2 round trip.
+// An fp64 value fills one line (lo, tag, hi, tag); two fp32 values share one.
+__device__ __forceinline__ void st_line(uint4* p, unsigned a, unsigned b, unsigned tag) {
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(tag), "r"(b), "r"(tag)
+                 : "memory");
+}
+__device__ __forceinline__ uint4 ld_line(const uint4* p) {
+    uint4 q;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(q.x), "=r"(q.y), "=r"(q.z), "=r"(q.w) : "l"(p) : "memory");
+    return q;
+}
+template <typename T> struct Line;
+template <> struct Line<double> {
+    static constexpr int per = 1;     // values per line
+    static __device__ __forceinline__ void put(uint4* p, const double* x, unsigned tag) {
+        st_line(p, (unsigned)__double2loint(x[0]), (unsigned)__double2hiint(x[0]), tag);
+    }
+    static __device__ __forceinline__ void get(const uint4 q, double* x) {
+        x[0] = __hiloint2double((int)q.z, (int)q.x);
+    }
+};
+template <> struct Line<float> {
+    static constexpr int per = 2;
+    static __device__ __forceinline__ void put(uint4* p, const float* x, unsigned tag) {
+        st_line(p, __float_as_uint(x[0]), __float_as_uint(x[1]), tag);
+    }
+    static __device__ __forceinline__ void get(const uint4 q, float* x) {
+        x[0] = __uint_as_float(q.x); x[1] = __uint_as_float(q.z);
+    }
+};
 
 template <typename T, int C>
 __global__ void __launch_bounds__(32 * kGridWarps)
@@ -362,21 +408,67 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
     const size_t side = (size_t)hl * C;                               // elements per published side
     auto signal = [&]() {
         if (a.sync_mode == kSyncGrid) { grid.sync(); return; }
-        if (!active) return;
-        __threadfence();
+        if (a.sync_mode == kSyncLL || !active) return;
+        // release: the warp's stores are ordered before lane 0's fence by __syncwarp, the fence is cumulative
         __syncwarp();
-        if (lane == 0) st_release_u32(flags + tile, stage);
+        if (lane == 0) { __threadfence(); st_relaxed_u32(flags + tile, stage); }
     };
     auto await = [&]() {
-        if (a.sync_mode == kSyncGrid || !active) return;
-        if (halo_l && has_l) wait_flag(flags + tile - 1, stage, fault);
-        if (halo_r && has_r) wait_flag(flags + tile + 1, stage, fault);
+        if (a.sync_mode != kSyncFlags || !active) return;
+        // lane 0 acquires for the warp; __syncwarp orders the other lanes' reads after it
+        if (lane == 0 && (has_l || has_r))
+            wait_flags(has_l ? flags + tile - 1 : nullptr, has_r ? flags + tile + 1 : nullptr, stage, fault);
         __syncwarp();
     };
     signal();
 
     int parity = 0;
+    constexpr int NQ = C / Line<T>::per;                              // lines per lane
+    auto meet_lines = [&]() {
+        // flag-in-data: publish tagged lines, then poll the neighbours' lines until every tag matches
+        ++stage;
+        if (active) {
+            uint4* xl = reinterpret_cast<uint4*>(xbuf);
+            const size_t lside = (size_t)hl * NQ;
+            if (own_l || own_r) {
+                uint4* dst = xl + ((size_t)parity * a.ntiles + tile) * 2 * lside +
+                             (own_l ? (size_t)(lane - hl) * NQ : lside + (size_t)(lane - (32 - 2 * hl)) * NQ);
+#pragma unroll
+                for (int j = 0; j < NQ; ++j) Line<T>::put(dst + j, &v[j * Line<T>::per], stage);
+            }
+            const uint4* src = nullptr;
+            if (halo_l && has_l)
+                src = xl + ((size_t)parity * a.ntiles + tile - 1) * 2 * lside + lside + (size_t)lane * NQ;
+            else if (halo_r && has_r)
+                src = xl + ((size_t)parity * a.ntiles + tile + 1) * 2 * lside + (size_t)(lane - (32 - hl)) * NQ;
+            if (src) {
+                uint4 q[NQ];
+                bool ok = false;
+                // watch the line written last with a back-off (a spinning lane would take issue slots from
+                // the warp that shares this scheduler and is still computing), then fetch all of them
+                for (unsigned it = 0; it < (1u << 22); ++it) {
+                    const uint4 w = ld_line(src + NQ - 1);
+                    if (w.y == stage && w.w == stage) break;
+                    __nanosleep(it < 64 ? 20 : 200);
+                }
+                for (unsigned it = 0; it < (1u << 20) && !ok; ++it) {
+#pragma unroll
+                    for (int j = 0; j < NQ; ++j) q[j] = ld_line(src + j);
+                    ok = true;
+#pragma unroll
+                    for (int j = 0; j < NQ; ++j) ok = ok && q[j].y == stage && q[j].w == stage;
+                    if (!ok) __nanosleep(100);
+                }
+                if (!ok) atomicExch(fault, 1u);
+#pragma unroll
+                for (int j = 0; j < NQ; ++j) Line<T>::get(q[j], &v[j * Line<T>::per]);
+            }
+            __syncwarp();
+        }
+        parity ^= 1;
+    };
     auto meet = [&]() {
+        if (a.sync_mode == kSyncLL) { meet_lines(); return; }
         // publish the outermost valid lanes, meet the neighbours, refresh the halo lanes
         ++stage;
         if (active) {
@@ -428,8 +520,9 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
         level_R<T, C, false>(v, x0, c, 0);
         unshift<T, C, false>(v, x0, c, 0);
     }
-    // with no meeting at all the neighbours may still be reading u: wait for their stage 0
-    if (stage == a.epoch0 + 1) await();
+    // with no meeting at all the neighbours may still be reading u: wait for their stage 0 (flags), or
+    // hold one meeting whose lines can only arrive from a neighbour that has loaded (flag-in-data)
+    if (stage == a.epoch0 + 1) { if (a.sync_mode == kSyncLL) meet_lines(); else await(); }
     if (inside && lane >= hl && lane < 32 - hl) {
 #pragma unroll
         for (int j = 0; j < C / V; ++j) {
