@@ -227,6 +227,8 @@ def run_ours(args):
     host0 = torch.from_numpy(cfg["u0"].reshape(-1))
     u = host0.to(dev)
     plan = libge.Plan(cfg, kernel=args.kernel, tb=args.tb, stream=stream)
+    if args.tc:
+        plan.tune(libge.GE_TUNE_TEMPORAL_C, args.tc)
     if args.rc:
         plan.tune(libge.GE_TUNE_RESIDENT_C, args.rc)
     if args.hl:
@@ -421,6 +423,7 @@ def main():
     ap.add_argument("--config", default="c4")
     ap.add_argument("--kernel", default="auto")
     ap.add_argument("--tb", type=int, default=0)
+    ap.add_argument("--tc", type=int, default=0, help="1-D temporal kernel: values per lane")
     ap.add_argument("--rc", type=int, default=0, help="persistent kernels: values per lane")
     ap.add_argument("--hl", type=int, default=0, help="whole-chip persistent kernel: halo lanes per side")
     ap.add_argument("--rtb", type=int, default=0, help="whole-chip persistent kernel: levels between meetings")

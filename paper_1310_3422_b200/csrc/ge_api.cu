@@ -16,6 +16,7 @@
 #include "ge_temporal.cuh"
 #include "ge_temporal2d.cuh"
 #include "ge_resident.cuh"
+#include "ge_stream.cuh"
 
 namespace {
 
@@ -37,7 +38,8 @@ inline size_t elem_size(int dtype) { return dtype == GE_F64 ? 8 : 4; }
 
 struct ge_plan {
     int32_t dim, dtype, group_k, kernel, tb;
-    int32_t tc;               // values per lane of the temporal kernel
+    int32_t tc;               // values per lane of the temporal kernel (18 f64 / 36 f32: the TMA-staged one)
+    int32_t stream_ctas;      // persistent grid of the TMA-staged kernel (0: not queried yet)
     int32_t hp;               // 2-D temporal kernel: output row pairs per segment
     int64_t nx, ny, batch;
     int64_t count;            // elements of the state
@@ -168,9 +170,36 @@ int launch_temporal_1d(ge_plan* p, const void* uin, void* uout, int tb, cudaStre
     auto* c = (const ge::Coef1<T>*)p->coef;
     cudaError_t e;
     constexpr int C0 = 16 / (int)sizeof(T) * 4;     // 8 (f64) / 16 (f32)
+    // rods of at least one tile take the drift-free kernels, shorter ones the generic (drifting) one
+    const bool df = p->nx >= 32 * (int64_t)p->tc;
+    constexpr int CS = 144 / (int)sizeof(T);         // 18 (f64) / 36 (f32): the TMA-staged kernel
     switch (p->tc) {
-        case C0:     e = ge::temporal1d_launch<T, C0>(in, out, p->nx, p->batch, c, tb, phase, s); break;
-        case 2 * C0: e = ge::temporal1d_launch<T, 2 * C0>(in, out, p->nx, p->batch, c, tb, phase, s); break;
+        case CS: {
+            if (!df) return GE_EINVAL;
+            if (p->stream_ctas == 0) {
+                int per_sm = 0;
+                auto* fn = &ge::ge1d_stream_kernel<T, CS>;
+                GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+                GE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ge::kStreamWarps * 32,
+                                                                      ge::stream_smem_bytes<T, CS>()));
+                p->stream_ctas = per_sm * p->sm_count;
+                if (p->stream_ctas < 1) return GE_ECUDA;
+            }
+            e = ge::stream1d_launch<T, CS>(in, out, p->nx, p->batch, c, tb, phase, p->stream_ctas, s);
+            break;
+        }
+        case C0:
+            e = df ? ge::temporal1d_launch<T, C0>(in, out, p->nx, p->batch, c, tb, phase, s)
+                   : ge::temporal1d_generic_launch<T, C0>(in, out, p->nx, p->batch, c, tb, phase, s);
+            break;
+        case 2 * C0:
+            e = df ? ge::temporal1d_launch<T, 2 * C0>(in, out, p->nx, p->batch, c, tb, phase, s)
+                   : ge::temporal1d_generic_launch<T, 2 * C0>(in, out, p->nx, p->batch, c, tb, phase, s);
+            break;
+        case 4 * C0:
+            e = df ? ge::temporal1d_launch<T, 4 * C0>(in, out, p->nx, p->batch, c, tb, phase, s)
+                   : ge::temporal1d_generic_launch<T, 4 * C0>(in, out, p->nx, p->batch, c, tb, phase, s);
+            break;
         default: return GE_EINVAL;
     }
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
@@ -205,7 +234,11 @@ bool temporal_ok(const ge_plan* p, const void* u) {
     return p->nx % V == 0 && ((uintptr_t)u % 16 == 0) && ((uintptr_t)p->scratch % 16 == 0);
 }
 
-int default_tc(int dtype) { return dtype == GE_F64 ? 16 : 32; }
+int stream_tc(int dtype) { return dtype == GE_F64 ? 18 : 36; }
+// the TMA-staged kernel when the rod holds at least a few tiles, else the warp-per-tile one
+int default_tc(int dtype, int64_t nx) {
+    return nx >= 4 * 32 * (int64_t)stream_tc(dtype) ? stream_tc(dtype) : (dtype == GE_F64 ? 16 : 32);
+}
 int clamp_tb(const ge_plan* p, int64_t tb) {
     const int mx = ge::temporal1d_max_tb(p->tc);
     return (int)(tb > mx ? mx : tb);
@@ -445,7 +478,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     // strategy selection: AUTO takes the resident kernels when the state fits on
     // the chip (1-D only), else the temporally blocked ones
     p->tb = 0;
-    p->tc = default_tc(p->dtype);
+    p->tc = default_tc(p->dtype, p->nx);
     p->hp = 64;
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
@@ -458,7 +491,8 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     }
     p->kernel = kernel;
     const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
-    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : 16);
+    // measured on C4: the TMA-staged kernel is fp64-bound from tb ~ 12 on, best near 20
+    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (p->tc == stream_tc(p->dtype) ? 20 : 16));
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : 8;
@@ -594,7 +628,8 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_TEMPORAL_C: {
             if (p->dim != 1) return GE_EINVAL;
             const int c0 = p->dtype == GE_F64 ? 8 : 16;
-            if (value != c0 && value != 2 * c0) return GE_EINVAL;
+            if (value == stream_tc(p->dtype)) { if (p->nx < 32 * value) return GE_EINVAL; }
+            else if (value != c0 && value != 2 * c0 && value != 4 * c0) return GE_EINVAL;
             p->tc = (int32_t)value;
             if (p->kernel == GE_KERNEL_TEMPORAL) p->tb = clamp_tb(p, p->tb);
             return GE_OK;

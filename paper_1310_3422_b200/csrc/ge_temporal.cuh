@@ -32,8 +32,15 @@
 //                                        of the pair to the LEFT (= q_{m-1})
 //     q_{C/2-1} comes from lane t+1's z_0 (the one shuffle)
 //     w = g (q_m - p_m);  new left = p_m + w;  new right = q_m - w
+//
+// Interior tiles (no Dirichlet node inside the loaded window -- all but the first and last few)
+// take the DRIFT-FREE level code of ge_resident.cuh instead: levels in pairs R/L that slide the
+// window right then left, so the state returns to the same registers after two levels (no
+// register moves), the halo is symmetric (tb stale nodes on either side) and the tile's output
+// range is the same [tile*valid, (tile+1)*valid).  Same expression tree, bit-identical results.
 #pragma once
 #include "ge_common.cuh"
+#include "ge_resident.cuh"
 
 namespace ge {
 
@@ -46,6 +53,7 @@ struct Temporal1dGeom {
     int post;      // realignment shifts after the last level, < V
     int shift;     // pre + tb + post: element offset between loaded and stored window
     int valid;     // outputs per tile (multiple of V)
+    int halo;      // interior tiles: nodes loaded left of the output range (multiple of V, even)
 };
 
 inline Temporal1dGeom temporal1d_geom(int C, int V, int tb, int phase) {
@@ -58,6 +66,12 @@ inline Temporal1dGeom temporal1d_geom(int C, int V, int tb, int phase) {
     // slot the pre-shift leaves behind, by 1 per realignment shift
     const int v = 32 * C - 2 * tb - 2 * g.pre - g.post;
     g.valid = v - v % V;
+    // drift-free interior tiles: one stale node per side and level; the in-lane level I that opens a
+    // launch at phase 0 and the shift back after an odd number of R/L levels each cost one more
+    const int rest = tb - g.pre;
+    const int stale = tb + g.pre + (rest & 1);
+    g.halo = (stale + V - 1) / V * V;
+    if (g.valid > 32 * C - 2 * g.halo) g.valid = 32 * C - 2 * g.halo;
     return g;
 }
 inline int temporal1d_max_tb(int C) { return 8 * C; }      // keeps at least half of every tile valid
@@ -147,9 +161,104 @@ __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __r
     }
 }
 
+// Drift-free tiles (rods with nx >= 32*C, valid + 2*halo <= 32*C):
+//   tile 0            left-aligned: loads [0, 32*C), element 0 in slot 0 of lane 0, writes [0, valid)
+//   tile t, 1..nreg-1 loads [t*valid - halo, +32*C) (fits inside the rod), writes [t*valid, (t+1)*valid)
+//   tile nreg (last)  right-aligned: loads [nx - 32*C, nx), element nx-1 in slot C-1 of lane 31,
+//                     writes [nreg*valid, nx)
+// so a Dirichlet node never sits inside a lane and the boundary logic of ge_resident.cuh applies
+// (BC = true for the first and last tile only).  nreg*valid <= nx - halo, so the last tile always
+// exists, and since tile nreg would not fit, nreg*valid > nx - 32*C + halo: its outputs are valid.
+struct Temporal1dTiles {
+    int64_t nreg;      // left-aligned + regular tiles
+    int64_t ntiles;    // nreg + 1
+};
+inline Temporal1dTiles temporal1d_tiles(int C, const Temporal1dGeom& g, int64_t nx) {
+    Temporal1dTiles t;
+    t.nreg = 1 + (nx + g.halo - 32 * (int64_t)C) / g.valid;
+    t.ntiles = t.nreg + 1;
+    return t;
+}
+
+template <typename T, int C, bool BC>
+__device__ __forceinline__ void temporal1d_tile_df(const T* __restrict__ in, T* __restrict__ out,
+                                                   const Coef1<T>& k, const Temporal1dGeom g, int64_t a0,
+                                                   int64_t out_lo, int64_t out_hi, bool first, bool last,
+                                                   int lane) {
+    constexpr int V = VecOf<T>::V;
+    const int64_t e0 = a0 + (int64_t)lane * C;     // element in slot 0 (even: a0, C are)
+    T v[C];
+#pragma unroll
+    for (int c = 0; c < C / V; ++c) {
+        T t[V];
+        ld_vec(in + e0 + c * V, t);
+#pragma unroll
+        for (int j = 0; j < V; ++j) v[c * V + j] = t[j];
+    }
+    ResidentCtx<T, false> cx;
+    cx.r = k.r; cx.g = k.g; cx.e = k.e; cx.lo = k.lo; cx.hi = k.hi;
+    cx.is_lo = BC && first && lane == 0; cx.is_hi = BC && last && lane == 31;
+    cx.lane = lane; cx.warp = 0; cx.nwarps = 1; cx.sx = nullptr;
+    T x0 = T(0);
+    int left = g.tb;
+    if (g.pre) { level_I<T, C, false, BC>(v, cx, 0); --left; }
+#pragma unroll 1
+    for (; left >= 2; left -= 2) {
+        level_R<T, C, false, BC>(v, x0, cx, 0);
+        level_L<T, C, false, BC>(v, x0, cx, 0);
+    }
+    if (left) {
+        level_R<T, C, false, BC>(v, x0, cx, 0);
+        unshift<T, C, false, BC>(v, x0, cx, 0);
+    }
+#pragma unroll
+    for (int c = 0; c < C / V; ++c) {
+        const int64_t e = e0 + c * V;
+        if (e >= out_lo && e < out_hi) {
+            T t[V];
+#pragma unroll
+            for (int j = 0; j < V; ++j) t[j] = v[c * V + j];
+            st_vec(out + e, t);
+        }
+    }
+}
+
 template <typename T, int C>
 __global__ void __launch_bounds__(kTemporalWarps * 32)
 ge1d_temporal_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
+                     const Coef1<T>* __restrict__ coef, const Temporal1dGeom g, const Temporal1dTiles tl) {
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kTemporalWarps + warp;
+    if (tile >= tl.ntiles) return;
+    const bool first = tile == 0, last = tile == tl.nreg;
+    const int64_t a0 = first ? 0 : (last ? nx - 32 * (int64_t)C : tile * g.valid - g.halo);
+    const int64_t out_lo = tile * g.valid;
+    const int64_t out_hi = last ? nx : out_lo + g.valid;
+    for (int64_t rod = blockIdx.y; rod < batch; rod += gridDim.y) {
+        const Coef1<T> k = coef[rod];
+        const T* __restrict__ in = uin + rod * nx;
+        T* __restrict__ out = uout + rod * nx;
+        if (first || last) temporal1d_tile_df<T, C, true>(in, out, k, g, a0, out_lo, out_hi, first, last, lane);
+        else               temporal1d_tile_df<T, C, false>(in, out, k, g, a0, out_lo, out_hi, false, false, lane);
+    }
+}
+
+// Host launcher: tb levels starting at a level of the given phase.
+// Requires nx % V == 0, nx >= 32*C, 16-byte aligned rows, 1 <= tb <= temporal1d_max_tb(C).
+template <typename T, int C>
+inline cudaError_t temporal1d_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
+                                     int tb, int phase, cudaStream_t s) {
+    const Temporal1dGeom g = temporal1d_geom(C, VecOf<T>::V, tb, phase);
+    const Temporal1dTiles tl = temporal1d_tiles(C, g, nx);
+    dim3 grid((unsigned)((tl.ntiles + kTemporalWarps - 1) / kTemporalWarps), (unsigned)(batch < 65535 ? batch : 65535));
+    ge1d_temporal_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, g, tl);
+    return cudaGetLastError();
+}
+
+template <typename T, int C>
+__global__ void __launch_bounds__(kTemporalWarps * 32)
+ge1d_temporal_generic_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
                      const Coef1<T>* __restrict__ coef, const Temporal1dGeom g, int64_t tiles_per_rod) {
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -169,12 +278,12 @@ ge1d_temporal_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx
 // Host launcher: tb levels starting at a level of the given phase.
 // Requires nx % V == 0, 16-byte aligned rows, 1 <= tb <= temporal1d_max_tb(C).
 template <typename T, int C>
-inline cudaError_t temporal1d_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
+inline cudaError_t temporal1d_generic_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
                                      int tb, int phase, cudaStream_t s) {
     const Temporal1dGeom g = temporal1d_geom(C, VecOf<T>::V, tb, phase);
     const int64_t tiles = (nx + g.valid - 1) / g.valid;
     dim3 grid((unsigned)((tiles + kTemporalWarps - 1) / kTemporalWarps), (unsigned)(batch < 65535 ? batch : 65535));
-    ge1d_temporal_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, g, tiles);
+    ge1d_temporal_generic_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, g, tiles);
     return cudaGetLastError();
 }
 
