@@ -143,7 +143,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._pump, daemon=True)
             self.th.start()
         except OSError:
@@ -188,6 +188,24 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
                 "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ multi-rank plumbing ------
+def max_over_ranks(ms, world, device):
+    """Device time of the slowest rank (the job is as slow as its slowest replica)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(units_per_rank_step, steps, world, ms):
+    """Whole-job GLUPS: "replicas only" -- every rank marches its own copy of the workload (weak scaling),
+    no data-path collective; value = updates of all ranks / max-over-ranks time."""
+    return units_per_rank_step * steps * world / (ms * 1e-3) / 1e9
 
 
 # ------------------------------------------------------------------ our arm (CUDA) ------
@@ -260,11 +278,8 @@ def run_ours(args):
     per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     launches = plan.info()["launches"] - l0
     meetings = plan.info()["meetings"] - m0
-    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tmax.item())
-    value = units(cfg) * args.steps * world / (total_ms_max * 1e-3) / 1e9
+    total_ms_max = max_over_ranks(total_ms, world, dev)
+    value = job_value(units(cfg), args.steps, world, total_ms_max)
     finite = bool(torch.isfinite(u).all().item())
 
     # ---- roofline of the dominant kernel: its average launch duration over the timed region ----
@@ -289,12 +304,10 @@ def run_ours(args):
         barrier()
         ms = e0.elapsed_time(e1)
         wall = (time.perf_counter() - t0) * 1e3
-        tt = torch.tensor([max(ms, wall)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e = {"value": units(cfg) * ksteps * world / (float(tt.item()) * 1e-3) / 1e9, "unit": UNIT,
+        tt = max_over_ranks(max(ms, wall), world, dev)
+        e2e = {"value": job_value(units(cfg), ksteps, world, tt), "unit": UNIT,
                "h2d_bytes_per_step": nelem * es, "d2h_bytes_per_step": nelem * es,
-               "steps": ksteps, "ms_per_step": float(tt.item()) / ksteps}
+               "steps": ksteps, "ms_per_step": tt / ksteps}
         del hbuf
 
     info = plan.info()
@@ -391,6 +404,8 @@ def roofline(cfg, info, total_ms, launches, steps):
     names = {"per_step": "ge%dd_level_kernel", "temporal": "ge%dd_temporal_kernel"}
     if kernel == "persistent":
         name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
+    elif kernel == "temporal" and info.get("temporal_c") in (18, 36):
+        name = "ge1d_stream_kernel"                      # the TMA-staged form of strategy B
     else:
         name = names[kernel] % cfg["dim"]
     name = "%s<%s>" % (name, cfg["dtype"])
@@ -417,7 +432,7 @@ def roofline(cfg, info, total_ms, launches, steps):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c4")

@@ -121,6 +121,7 @@ enum {
     GE_INFO_RESIDENT_CAPACITY = 8, /* path 2: co-resident tiles the device offers                 */
     GE_INFO_RESIDENT_TB = 9,   /* path 2: levels between two meetings                             */
     GE_INFO_MEETINGS = 10,     /* path 2: meetings (halo exchanges) performed so far              */
+    GE_INFO_TEMPORAL_C = 12,   /* values per lane of the 1-D temporal kernel in use (18 / 36: TMA-staged)   */
     GE_INFO_SYNC_FAULT = 11    /* path 2: 1 if a tile ever gave up waiting for a neighbour (the result
                                   is then invalid); SYNCHRONISES the last stream used              */
 };

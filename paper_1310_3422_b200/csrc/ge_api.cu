@@ -596,6 +596,7 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
         case GE_INFO_TILE_LOADED:
             *value = p->kernel == GE_KERNEL_TEMPORAL ? 32 * p->tc : 0;
             return GE_OK;
+        case GE_INFO_TEMPORAL_C: *value = p->kernel == GE_KERNEL_TEMPORAL && p->dim == 1 ? p->tc : 0; return GE_OK;
         case GE_INFO_RESIDENT_PATH: *value = p->kernel == GE_KERNEL_PERSISTENT ? p->res_path : 0; return GE_OK;
         case GE_INFO_RESIDENT_C: *value = p->res_path ? p->res_c : 0; return GE_OK;
         case GE_INFO_RESIDENT_WARPS:

@@ -23,7 +23,7 @@ GE_KERNEL_AUTO, GE_KERNEL_PER_STEP, GE_KERNEL_TEMPORAL, GE_KERNEL_PERSISTENT = 0
 GE_OK, GE_EINVAL, GE_ENOMEM, GE_ECUDA, GE_EUNSUPPORTED = 0, -1, -2, -3, -4
 GE_INFO_KERNEL, GE_INFO_TB, GE_INFO_LAUNCHES, GE_INFO_TILE_VALID, GE_INFO_TILE_LOADED = 0, 1, 2, 3, 4
 (GE_INFO_RESIDENT_PATH, GE_INFO_RESIDENT_C, GE_INFO_RESIDENT_WARPS, GE_INFO_RESIDENT_CAPACITY,
- GE_INFO_RESIDENT_TB, GE_INFO_MEETINGS, GE_INFO_SYNC_FAULT) = 5, 6, 7, 8, 9, 10, 11
+ GE_INFO_RESIDENT_TB, GE_INFO_MEETINGS, GE_INFO_SYNC_FAULT, GE_INFO_TEMPORAL_C) = 5, 6, 7, 8, 9, 10, 11, 12
 GE_TUNE_TEMPORAL_C, GE_TUNE_TB, GE_TUNE_SEG_PAIRS = 0, 1, 2
 GE_TUNE_RESIDENT_C, GE_TUNE_HALO_LANES, GE_TUNE_SYNC_MODE = 3, 4, 5
 GE_SYNC_FLAGS, GE_SYNC_GRID, GE_SYNC_LINES = 0, 1, 2
@@ -224,7 +224,8 @@ class Plan:
                     resident_warps=ge_plan_info(self.handle, GE_INFO_RESIDENT_WARPS),
                     resident_capacity=ge_plan_info(self.handle, GE_INFO_RESIDENT_CAPACITY),
                     resident_tb=ge_plan_info(self.handle, GE_INFO_RESIDENT_TB),
-                    meetings=ge_plan_info(self.handle, GE_INFO_MEETINGS))
+                    meetings=ge_plan_info(self.handle, GE_INFO_MEETINGS),
+                    temporal_c=ge_plan_info(self.handle, GE_INFO_TEMPORAL_C))
 
     def sync_fault(self) -> int:
         """1 if a tile of the whole-chip persistent kernel gave up waiting (synchronises)."""
