@@ -17,6 +17,7 @@
 #include "ge_temporal2d.cuh"
 #include "ge_resident.cuh"
 #include "ge_stream.cuh"
+#include "ge_strip2d.cuh"
 
 namespace {
 
@@ -226,7 +227,29 @@ int launch_temporal_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) 
     p->level += p->tb;
     return GE_OK;
 }
-bool temporal2d_tb_ok(int64_t tb) { return tb == 4 || tb == 8; }
+// ---- strategy B launch (2-D, drift-free strips): plan->tb levels from the current PHASE-1 level ----
+constexpr int kStripC = 4;
+bool strip2d_ok(const ge_plan* p) { return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * kStripC; }
+
+template <typename T>
+int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    auto* c = (const ge::Coef2<T>*)p->coef;
+    cudaError_t e;
+    switch (p->tb) {
+        case 4: e = ge::strip2d_launch<T, kStripC, 4>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 6: e = ge::strip2d_launch<T, kStripC, 6>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 8: e = ge::strip2d_launch<T, kStripC, 8>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        default: return GE_EINVAL;
+    }
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += p->tb;
+    return GE_OK;
+}
+// block lengths: 4, 8 everywhere; 6 only where the strip kernel runs
+bool temporal2d_tb_ok(const ge_plan* p, int64_t tb) { return tb == 4 || tb == 8 || (tb == 6 && strip2d_ok(p)); }
 
 bool temporal_ok(const ge_plan* p, const void* u) {
     if (p->dim == 2 && (p->nx >= (1 << 30) || p->ny >= (1 << 30))) return false;
@@ -496,7 +519,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : 8;
-        if (!temporal2d_tb_ok(p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
+        if (!temporal2d_tb_ok(p, p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
     }
     *out = p;
     return GE_OK;
@@ -531,7 +554,16 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     const bool temporal = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && temporal_ok(p, u);
     while (left > 0 && rc == GE_OK) {
         if (temporal && p->dim == 2) {
-            if (left >= p->tb) {
+            const bool strips = strip2d_ok(p);
+            if (strips && left > p->tb && (p->level & 1) == 0) {
+                // the strip kernel starts at a phase-1 level: one per-level launch first
+                rc = launch_level(p, cur, oth, s);
+                left -= 1;
+            } else if (strips && left >= p->tb && (p->level & 1) == 1) {
+                rc = p->dtype == GE_F64 ? launch_strip_2d<double>(p, cur, oth, s)
+                                        : launch_strip_2d<float>(p, cur, oth, s);
+                left -= p->tb;
+            } else if (!strips && left >= p->tb) {
                 rc = p->dtype == GE_F64 ? launch_temporal_2d<double>(p, cur, oth, s)
                                         : launch_temporal_2d<float>(p, cur, oth, s);
                 left -= p->tb;
@@ -678,7 +710,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             }
             if (p->kernel != GE_KERNEL_TEMPORAL) return GE_EINVAL;
             if (p->dim == 2) {
-                if (!temporal2d_tb_ok(value)) return GE_EINVAL;
+                if (!temporal2d_tb_ok(p, value)) return GE_EINVAL;
                 p->tb = (int32_t)value;
                 return GE_OK;
             }
