@@ -518,7 +518,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (p->tc == stream_tc(p->dtype) ? 20 : 16));
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
-        p->tb = d->tb > 0 ? d->tb : 8;
+        p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
         if (!temporal2d_tb_ok(p, p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
     }
     *out = p;

@@ -1,5 +1,5 @@
 // ge_strip2d.cuh -- strategy B (2-D), drift-free: TB levels per HBM round trip,
-// state in registers, no shared memory, no barrier.
+// state in registers and lane-private shared memory, no barrier.
 //
 // Scheme: DESIGN.md reading R-2D (2x2 four-point groups, anchors shifted by
 // (1,1) between levels; PAPER.md:134, :228 only claim the extension).
@@ -22,9 +22,11 @@
 //     are a few selects on lane 0 / lane 31 of the first / last strip (BC),
 //     compiled out for interior strips.  In the shifted state column 0 of the
 //     first strip lives in one extra register per row.
-//   * the row loop is unrolled by two, so the rotating row registers
-//     (prev[l] <- cur) rotate by renaming, and row pairs are prefetched two
-//     iterations ahead.
+//   * the previous row pair of every stage lives in lane-private SHARED memory
+//     slots (conflict-free 16-byte accesses, no synchronisation), so registers
+//     hold only the pair that flows through the stages: 20+ warps per SM, no
+//     rotating register moves.  Row pairs arrive through a cp.async ring in
+//     shared memory, requested three iterations ahead.
 //   * groups cut by a y edge (and rows outside the grid) take a generic
 //     out-of-line path built on ge_level.cuh group_update.
 // Arithmetic: 6.75 flop-instructions per node update, the expression tree of
@@ -197,67 +199,144 @@ __device__ __noinline__ void strip_stage_edge(const T* __restrict__ ext, T* __re
     }
 }
 
-// Builds the extended rows (two neighbour columns per side) and runs the generic stage.
-template <typename T, int C, bool SHIFTED, bool BC>
-__device__ __forceinline__ void strip_stage_slow(const T (&P0)[C], const T (&P1)[C], const T (&Q0)[C],
-                                                 const T (&Q1)[C], const T (&pP)[2], const T (&pQ)[2],
-                                                 T (&N0)[C], T (&N1)[C], T (&nx0)[2], const Strip2dCtx<T>& k,
-                                                 const Coef2<T>* __restrict__ coef, int yg, bool outside) {
+// Out-of-line wrapper: io holds the four input rows P0, P1, Q0, Q1 (4*C values) followed by their
+// column-0 values (4: lane is_lo, shifted rows); builds the extended rows (two neighbour columns
+// per side, by shuffles), runs the generic stage and leaves N0, N1 (2*C values) and the new
+// column 0 of the two rows (2) at the start of io.  Called from a warp-uniform branch.
+template <typename T, int C, bool SHIFTED>
+__device__ __noinline__ void strip_stage_slow(T* __restrict__ io, const Coef2<T>* __restrict__ coef, int yg,
+                                              bool outside, bool is_lo, bool is_hi) {
     constexpr unsigned FULL = 0xffffffffu;
     constexpr int E = C + 4;
+    const T xlo = coef->xlo, xhi = coef->xhi;
     T ext[4 * E];
-    const T* rows[4] = {P0, P1, Q0, Q1};
-    const T col0[4] = {pP[0], pP[1], pQ[0], pQ[1]};
 #pragma unroll
     for (int rr = 0; rr < 4; ++rr) {
-        const T* v = rows[rr];
+        const T* v = io + rr * C;
 #pragma unroll
         for (int s = 0; s < C; ++s) ext[rr * E + s + 2] = v[s];
         T l2 = __shfl_up_sync(FULL, v[C - 2], 1), l1 = __shfl_up_sync(FULL, v[C - 1], 1);
         T r0 = __shfl_down_sync(FULL, v[0], 1), r1 = __shfl_down_sync(FULL, v[1], 1);
-        if (BC && k.is_lo) {
-            if (SHIFTED) { l1 = col0[rr]; l2 = k.xlo; } else { l1 = k.xlo; l2 = T(0); }
+        if (is_lo) {
+            if (SHIFTED) { l1 = io[4 * C + rr]; l2 = xlo; } else { l1 = xlo; l2 = T(0); }
         }
-        if (BC && k.is_hi) {
-            if (SHIFTED) { r0 = T(0); r1 = T(0); } else { r0 = k.xhi; r1 = T(0); }
+        if (is_hi) {
+            if (SHIFTED) { r0 = T(0); r1 = T(0); } else { r0 = xhi; r1 = T(0); }
         }
         ext[rr * E + 0] = l2; ext[rr * E + 1] = l1;
         ext[rr * E + C + 2] = r0; ext[rr * E + C + 3] = r1;
     }
     T o[2 * C + 2];
-    strip_stage_edge<T, C, SHIFTED>(ext, o, coef, yg, outside, BC && k.is_lo, BC && k.is_hi);
+    o[2 * C] = T(0); o[2 * C + 1] = T(0);
+    strip_stage_edge<T, C, SHIFTED>(ext, o, coef, yg, outside, is_lo, is_hi);
 #pragma unroll
-    for (int s = 0; s < C; ++s) { N0[s] = o[s]; N1[s] = o[C + s]; }
-    if (!SHIFTED) { nx0[0] = o[2 * C]; nx0[1] = o[2 * C + 1]; }
+    for (int s = 0; s < 2 * C + 2; ++s) io[s] = o[s];
 }
 
-// Row y of the lane's columns [e0, e0+C); rows outside the grid return the boundary value (y = -1,
-// y = ny) or a finite filler.  The strip lies inside the grid in x, so every load is a full vector.
+// One stage of the pipeline: P = previous row pair of level l (with its column 0: xP), Q = current
+// one; writes the level-(l+1) pair into N (xN).  Odd stages are L, even stages R.
+// (`odd` is a constant after the stage loop is unrolled.)
+template <typename T, int C, bool BC>
+__device__ __forceinline__ void strip_stage(const bool odd, const T (&P)[2][C], const T (&xP)[2],
+                                            const T (&Q)[2][C], const T (&xQ)[2], T (&N)[2][C], T (&xN)[2],
+                                            const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int j,
+                                            int ny) {
+    if ((unsigned)j < (unsigned)(ny - 1)) {          // group rows j, j+1 both interior: the fast stage
+        if (odd) strip_stage_L<T, C, BC>(P[0], P[1], Q[0], Q[1], xP, xQ, N[0], N[1], k);
+        else     strip_stage_R<T, C, BC>(P[0], P[1], Q[0], Q[1], N[0], N[1], xN, k);
+    } else {
+        T io[4 * C + 4];
+#pragma unroll
+        for (int s = 0; s < C; ++s) {
+            io[s] = P[0][s]; io[C + s] = P[1][s]; io[2 * C + s] = Q[0][s]; io[3 * C + s] = Q[1][s];
+        }
+        io[4 * C] = xP[0]; io[4 * C + 1] = xP[1]; io[4 * C + 2] = xQ[0]; io[4 * C + 3] = xQ[1];
+        const int yg = j == -1 ? 1 : (j + 1 == ny ? 2 : 0);
+        if (odd) strip_stage_slow<T, C, true>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
+        else     strip_stage_slow<T, C, false>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
+#pragma unroll
+        for (int s = 0; s < C; ++s) { N[0][s] = io[s]; N[1][s] = io[C + s]; }
+        if (!odd) { xN[0] = io[2 * C]; xN[1] = io[2 * C + 1]; }
+    }
+}
+
+// The pipeline state -- the previous row pair of every level 0 .. TB-1 -- lives in SHARED memory, in
+// lane-private slots (vector c of lane t at [(c*32 + t)*V], conflict-free, no synchronisation): stage l
+// loads its previous pair, computes, and stores the current pair in its place.  Registers hold only
+// the pair that flows through the stages and the row pairs in flight from HBM, so 20+ warps fit on
+// an SM and nothing rotates through register moves.
 template <typename T, int C>
-__device__ __forceinline__ void strip_load_row(const T* __restrict__ uin, int nx, int ny, T ylo, T yhi, int y,
-                                               int e0, T (&v)[C]) {
+__device__ __forceinline__ void strip_lds(const T* __restrict__ sp, int lane, T (&v)[2][C]) {
     constexpr int V = VecOf<T>::V;
-    if ((unsigned)y < (unsigned)ny) {
-        const T* __restrict__ row = uin + (int64_t)y * nx + e0;
+    using VT = typename VecOf<T>::type;
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr)
 #pragma unroll
         for (int c = 0; c < C / V; ++c) {
-            T t[V];
-            ld_vec(row + c * V, t);
-#pragma unroll
-            for (int j = 0; j < V; ++j) v[c * V + j] = t[j];
+            const VT q = *reinterpret_cast<const VT*>(sp + ((rr * (C / V) + c) * 32 + lane) * V);
+            if constexpr (V == 4) { v[rr][c * V] = q.x; v[rr][c * V + 1] = q.y; v[rr][c * V + 2] = q.z; v[rr][c * V + 3] = q.w; }
+            else { v[rr][c * V] = q.x; v[rr][c * V + 1] = q.y; }
         }
-    } else {
-        const T f = y == -1 ? ylo : (y == ny ? yhi : T(0));
+}
+template <typename T, int C>
+__device__ __forceinline__ void strip_sts(T* __restrict__ sp, int lane, const T (&v)[2][C]) {
+    constexpr int V = VecOf<T>::V;
+    using VT = typename VecOf<T>::type;
 #pragma unroll
-        for (int j = 0; j < C; ++j) v[j] = f;
+    for (int rr = 0; rr < 2; ++rr)
+#pragma unroll
+        for (int c = 0; c < C / V; ++c) {
+            VT q;
+            if constexpr (V == 4) { q.x = v[rr][c * V]; q.y = v[rr][c * V + 1]; q.z = v[rr][c * V + 2]; q.w = v[rr][c * V + 3]; }
+            else { q.x = v[rr][c * V]; q.y = v[rr][c * V + 1]; }
+            *reinterpret_cast<VT*>(sp + ((rr * (C / V) + c) * 32 + lane) * V) = q;
+        }
+}
+
+// Row pairs travel HBM -> shared memory with cp.async (16 bytes per lane, lane-private slots, so the
+// issuing lane is the only reader and cp.async.wait_group is all the synchronisation needed) through a
+// ring of kStripRing pairs: a pair is requested kStripRing-1 iterations before it is used, no register
+// holds data in flight, and nothing has to be moved while a load is pending.
+constexpr int kStripRing = 4;
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)),
+                 "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// request rows y, y+1 of the lane's columns into the pair slot `dst` (layout of strip_sts)
+template <typename T, int C>
+__device__ __forceinline__ void strip_request_pair(const T* __restrict__ uin, int nx, int ny, T ylo, T yhi, int y,
+                                                   int e0, T* __restrict__ dst, int lane) {
+    constexpr int V = VecOf<T>::V;
+    using VT = typename VecOf<T>::type;
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+        const int yy = y + rr;
+        if ((unsigned)yy < (unsigned)ny) {
+            const T* __restrict__ row = uin + (int64_t)yy * nx + e0;
+#pragma unroll
+            for (int c = 0; c < C / V; ++c) cp_async16(dst + ((rr * (C / V) + c) * 32 + lane) * V, row + c * V);
+        } else {
+            const T f = yy == -1 ? ylo : (yy == ny ? yhi : T(0));
+            VT q;
+            if constexpr (V == 4) { q.x = f; q.y = f; q.z = f; q.w = f; } else { q.x = f; q.y = f; }
+#pragma unroll
+            for (int c = 0; c < C / V; ++c) *reinterpret_cast<VT*>(dst + ((rr * (C / V) + c) * 32 + lane) * V) = q;
+        }
     }
 }
 
 template <typename T, int C, int TB, bool BC>
 __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny,
-                                          const Coef2<T>* __restrict__ coef, int a0, int out_lo, int out_hi,
-                                          bool first, bool last, int ys, int ye, int lane) {
+                                          const Coef2<T>* __restrict__ coef, T* __restrict__ sp, int a0,
+                                          int out_lo, int out_hi, bool first, bool last, int ys, int ye,
+                                          int lane) {
     constexpr int V = VecOf<T>::V;
+    constexpr int kPair = 2 * 32 * C;             // elements of one row pair of the strip
     static_assert(TB % 2 == 0 && C % 2 == 0 && C % V == 0, "TB even; C holds whole groups and vectors");
     const Coef2<T> kk = *coef;
     Strip2dCtx<T> k;
@@ -267,49 +346,42 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
     const int Y0 = ys - TB;                       // first row pair that enters the pipeline
     const int iters = (ye - ys + 1) / 2 + TB;
 
-    T prev[TB][2][C];
-    T px[TB][2];                                  // column 0 of prev[l] (odd l: shifted rows; lane is_lo)
+    {
+        T z[2][C];
 #pragma unroll
-    for (int l = 0; l < TB; ++l) {
+        for (int j = 0; j < C; ++j) { z[0][j] = T(0); z[1][j] = T(0); }
 #pragma unroll
-        for (int j = 0; j < C; ++j) { prev[l][0][j] = T(0); prev[l][1][j] = T(0); }
-        px[l][0] = T(0); px[l][1] = T(0);
+        for (int l = 0; l < TB; ++l) strip_sts<T, C>(sp + l * kPair, lane, z);
     }
-    T L0[2][C], L1[2][C];                         // row pairs in flight, two iterations ahead
-    strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, Y0, e0, L0[0]);
-    strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, Y0 + 1, e0, L0[1]);
-    strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, Y0 + 2, e0, L1[0]);
-    strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, Y0 + 3, e0, L1[1]);
-
-    auto body = [&](int it, T (&LL)[2][C]) {
-        const int y0 = Y0 + 2 * it;
-        T cur[2][C], cx[2] = {T(0), T(0)};
+    T px[TB][2];                                  // column 0 of the previous pairs (lane is_lo, odd levels)
 #pragma unroll
-        for (int s = 0; s < C; ++s) { cur[0][s] = LL[0][s]; cur[1][s] = LL[1][s]; }
-        strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, y0 + 4, e0, LL[0]);
-        strip_load_row<T, C>(uin, nx, ny, kk.ylo, kk.yhi, y0 + 5, e0, LL[1]);
+    for (int l = 0; l < TB; ++l) { px[l][0] = T(0); px[l][1] = T(0); }
+    T* ring = sp + TB * kPair;                    // kStripRing pair slots after the TB state slots
+#pragma unroll
+    for (int q = 0; q < kStripRing - 1; ++q) {
+        strip_request_pair<T, C>(uin, nx, ny, kk.ylo, kk.yhi, Y0 + 2 * q, e0, ring + q * kPair, lane);
+        cp_async_commit();
+    }
+
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+        const int y0 = Y0 + 2 * it;
+        // request the pair of iteration it + kStripRing - 1 (its slot was read in iteration it - 1)
+        strip_request_pair<T, C>(uin, nx, ny, kk.ylo, kk.yhi, y0 + 2 * (kStripRing - 1), e0,
+                                 ring + ((it + kStripRing - 1) % kStripRing) * kPair, lane);
+        cp_async_commit();
+        cp_async_wait<kStripRing - 1>();          // the pair of this iteration has landed
+        T cur[2][C], cx[2] = {T(0), T(0)};
+        strip_lds<T, C>(ring + (it % kStripRing) * kPair, lane, cur);
 #pragma unroll
         for (int l = 0; l < TB; ++l) {
-            const int j = y0 - 1 - l;             // lower row of this stage's groups
-            T nw[2][C], nwx[2] = {T(0), T(0)};
-            if ((unsigned)j < (unsigned)(ny - 1)) {
-                if (l % 2 == 0) strip_stage_R<T, C, BC>(prev[l][0], prev[l][1], cur[0], cur[1], nw[0], nw[1], nwx, k);
-                else            strip_stage_L<T, C, BC>(prev[l][0], prev[l][1], cur[0], cur[1], px[l], cx, nw[0], nw[1], k);
-            } else {
-                const int yg = j == -1 ? 1 : (j + 1 == ny ? 2 : 0);
-                if (l % 2 == 0)
-                    strip_stage_slow<T, C, false, BC>(prev[l][0], prev[l][1], cur[0], cur[1], px[l], cx, nw[0],
-                                                      nw[1], nwx, k, coef, yg, yg == 0);
-                else
-                    strip_stage_slow<T, C, true, BC>(prev[l][0], prev[l][1], cur[0], cur[1], px[l], cx, nw[0],
-                                                     nw[1], nwx, k, coef, yg, yg == 0);
-            }
+            T P[2][C], N[2][C], nx0[2] = {T(0), T(0)};
+            strip_lds<T, C>(sp + l * kPair, lane, P);
+            strip_stage<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, y0 - 1 - l, ny);
+            strip_sts<T, C>(sp + l * kPair, lane, cur);
 #pragma unroll
-            for (int s = 0; s < C; ++s) {
-                prev[l][0][s] = cur[0][s]; prev[l][1][s] = cur[1][s];
-                cur[0][s] = nw[0][s]; cur[1][s] = nw[1][s];
-            }
-            if constexpr (BC) { px[l][0] = cx[0]; px[l][1] = cx[1]; cx[0] = nwx[0]; cx[1] = nwx[1]; }
+            for (int s = 0; s < C; ++s) { cur[0][s] = N[0][s]; cur[1][s] = N[1][s]; }
+            if constexpr (BC) { px[l][0] = cx[0]; px[l][1] = cx[1]; cx[0] = nx0[0]; cx[1] = nx0[1]; }
         }
         // cur holds level-TB rows (y0 - TB, y0 - TB + 1), unshifted (TB is even)
         if (it >= TB) {
@@ -331,16 +403,21 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
                 }
             }
         }
-    };
-#pragma unroll 1
-    for (int it = 0; it < iters; it += 2) {
-        body(it, L0);
-        if (it + 1 < iters) body(it + 1, L1);
     }
 }
 
+// resident CTAs per SM the register allocation is held to (measured r01: tighter caps spill and lose
+// 3x; -DGE_STRIP_MINB_F32/F64 through GE_NVCC_EXTRA for sweeps)
+#ifndef GE_STRIP_MINB_F32
+#define GE_STRIP_MINB_F32 3
+#endif
+#ifndef GE_STRIP_MINB_F64
+#define GE_STRIP_MINB_F64 2
+#endif
+template <typename T> struct StripMinBlocks { static constexpr int n = sizeof(T) == 8 ? GE_STRIP_MINB_F64 : GE_STRIP_MINB_F32; };
+
 template <typename T, int C, int TB>
-__global__ void __launch_bounds__(kStripWarps * 32)
+__global__ void __launch_bounds__(kStripWarps * 32, StripMinBlocks<T>::n)
 ge2d_strip_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny,
                   const Coef2<T>* __restrict__ coef, const Strip2dGeom g) {
     const int lane = threadIdx.x & 31;
@@ -353,8 +430,10 @@ ge2d_strip_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
     const int out_hi = last ? nx : out_lo + g.valid;
     const int ys = 2 * g.hp * (int)blockIdx.y;
     const int ye = ys + 2 * g.hp < ny ? ys + 2 * g.hp : ny;
-    if (first || last) strip_run<T, C, TB, true>(uin, uout, nx, ny, coef, a0, out_lo, out_hi, first, last, ys, ye, lane);
-    else               strip_run<T, C, TB, false>(uin, uout, nx, ny, coef, a0, out_lo, out_hi, false, false, ys, ye, lane);
+    extern __shared__ __align__(16) unsigned char strip_smem[];
+    T* sp = reinterpret_cast<T*>(strip_smem) + (size_t)warp * (TB + kStripRing) * 2 * 32 * C;   // state + ring of this warp
+    if (first || last) strip_run<T, C, TB, true>(uin, uout, nx, ny, coef, sp, a0, out_lo, out_hi, first, last, ys, ye, lane);
+    else               strip_run<T, C, TB, false>(uin, uout, nx, ny, coef, sp, a0, out_lo, out_hi, false, false, ys, ye, lane);
 }
 
 // Host launcher: TB levels starting at a PHASE-1 level.  Requires nx % V == 0, nx even, nx >= 32*C,
@@ -364,7 +443,15 @@ inline cudaError_t strip2d_launch(const T* uin, T* uout, int64_t nx, int64_t ny,
                                   cudaStream_t s) {
     const Strip2dGeom g = strip2d_geom(C, VecOf<T>::V, TB, nx, ny, hp);
     dim3 grid((unsigned)((g.nstrips + kStripWarps - 1) / kStripWarps), (unsigned)g.segs);
-    ge2d_strip_kernel<T, C, TB><<<grid, kStripWarps * 32, 0, s>>>(uin, uout, (int)nx, (int)ny, coef, g);
+    constexpr size_t smem = (size_t)kStripWarps * (TB + kStripRing) * 2 * 32 * C * sizeof(T);
+    static bool configured = false;               // per instantiation: allow > 48 KB and the full carve-out
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(ge2d_strip_kernel<T, C, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(ge2d_strip_kernel<T, C, TB>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    ge2d_strip_kernel<T, C, TB><<<grid, kStripWarps * 32, smem, s>>>(uin, uout, (int)nx, (int)ny, coef, g);
     return cudaGetLastError();
 }
 
