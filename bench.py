@@ -258,10 +258,10 @@ def run_ours(args):
     info0 = plan.info()
 
     # ---- device-resident timing: W warm-up steps, then exactly K timed steps ----
+    clocks = ClockSampler(local) if rank == 0 else None       # started early: nvidia-smi needs ~0.2 s to come up
     for _ in range(args.warmup):
         plan.run(u.data_ptr(), levels, stream)
     barrier()
-    clocks = ClockSampler(local) if rank == 0 else None
     l0, m0 = plan.info()["launches"], plan.info()["meetings"]
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
@@ -406,6 +406,8 @@ def roofline(cfg, info, total_ms, launches, steps):
         name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
     elif kernel == "temporal" and info.get("temporal_c") in (18, 36):
         name = "ge1d_stream_kernel"                      # the TMA-staged form of strategy B
+    elif kernel == "temporal" and cfg["dim"] == 2 and cfg["nx"] % 4 == 0 and cfg["nx"] >= 128:
+        name = "ge2d_strip_kernel"                       # the drift-free form of strategy B in 2-D
     else:
         name = names[kernel] % cfg["dim"]
     name = "%s<%s>" % (name, cfg["dtype"])

@@ -26,7 +26,7 @@
 //     slots (conflict-free 16-byte accesses, no synchronisation), so registers
 //     hold only the pair that flows through the stages: 20+ warps per SM, no
 //     rotating register moves.  Row pairs arrive through a cp.async ring in
-//     shared memory, requested three iterations ahead.
+//     shared memory, requested two iterations ahead.
 //   * groups cut by a y edge (and rows outside the grid) take a generic
 //     out-of-line path built on ge_level.cuh group_update.
 // Arithmetic: 6.75 flop-instructions per node update, the expression tree of
@@ -37,7 +37,13 @@
 
 namespace ge {
 
-constexpr int kStripWarps = 4;        // warps per CTA = adjacent strips (their halos share L2 lines)
+#ifndef GE_STRIP_WARPS
+#define GE_STRIP_WARPS 4
+#endif
+#ifndef GE_STRIP_RING
+#define GE_STRIP_RING 3
+#endif
+constexpr int kStripWarps = GE_STRIP_WARPS;   // warps per CTA = adjacent strips (their halos share L2 lines)
 
 struct Strip2dGeom {
     int halo;        // stale columns per side of an interior strip (multiple of V)
@@ -297,7 +303,7 @@ __device__ __forceinline__ void strip_sts(T* __restrict__ sp, int lane, const T 
 // issuing lane is the only reader and cp.async.wait_group is all the synchronisation needed) through a
 // ring of kStripRing pairs: a pair is requested kStripRing-1 iterations before it is used, no register
 // holds data in flight, and nothing has to be moved while a load is pending.
-constexpr int kStripRing = 4;
+constexpr int kStripRing = GE_STRIP_RING;
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)),
