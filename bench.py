@@ -244,7 +244,7 @@ def run_ours(args):
 
     host0 = torch.from_numpy(cfg["u0"].reshape(-1))
     u = host0.to(dev)
-    plan = libge.Plan(cfg, kernel=args.kernel, tb=args.tb, stream=stream)
+    plan = libge.Plan(cfg, kernel=args.kernel, tb=args.tb, stream=stream, group_k=args.k)
     if args.tc:
         plan.tune(libge.GE_TUNE_TEMPORAL_C, args.tc)
     if args.rc:
@@ -283,6 +283,7 @@ def run_ours(args):
     finite = bool(torch.isfinite(u).all().item())
 
     # ---- roofline of the dominant kernel: its average launch duration over the timed region ----
+    info0["group_k"] = args.k
     roof = roofline(cfg, info0, total_ms, launches, args.steps)
     fault = plan.sync_fault() if info0["resident_path"] == 2 else 0
 
@@ -339,7 +340,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
         "config": {"workload": workload_desc(cfg), "levels_per_step": levels, "kernel": info["kernel"],
-                   "tb": info["resident_tb"] if info["resident_path"] == 2 else (0 if info["resident_path"] else info["tb"]),
+                   "group_k": args.k, "tb": info["resident_tb"] if info["resident_path"] == 2 else (0 if info["resident_path"] else info["tb"]),
                    "resident": {"path": info["resident_path"], "c": info["resident_c"],
                                 "warps": info["resident_warps"], "capacity": info["resident_capacity"],
                                 "meetings_per_step": meetings // max(1, args.steps),
@@ -402,6 +403,8 @@ def roofline(cfg, info, total_ms, launches, steps):
     lv = cfg["steps"] * steps / max(launches, 1)            # levels per launch (average)
     upd = nelem * lv                                        # updates per launch
     names = {"per_step": "ge%dd_level_kernel", "temporal": "ge%dd_temporal_kernel"}
+    if info.get("group_k", 1) >= 2:
+        names["per_step"] = "ge%dd_level_k_kernel"
     if kernel == "persistent":
         name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
     elif kernel == "temporal" and info.get("temporal_c") in (18, 36):
@@ -440,6 +443,7 @@ def main():
     ap.add_argument("--config", default="c4")
     ap.add_argument("--kernel", default="auto")
     ap.add_argument("--tb", type=int, default=0)
+    ap.add_argument("--k", type=int, default=1, help="sub-domain length (PAPER.md:82); k >= 2: per-level kernel only")
     ap.add_argument("--tc", type=int, default=0, help="1-D temporal kernel: values per lane")
     ap.add_argument("--rc", type=int, default=0, help="persistent kernels: values per lane")
     ap.add_argument("--hl", type=int, default=0, help="whole-chip persistent kernel: halo lanes per side")

@@ -16,6 +16,10 @@
  *     Eq (1)/(2) with the boundary value as new-level neighbour
  *     (PAPER.md:70-78, :142, :148).  The pattern alternates between levels
  *     (PAPER.md:92, :140-150).
+ *   - 1-D, group_k = k >= 2 (the paper's general scheme): node classes
+ *     c = (i - phase*k) mod 2k: c = 2k-1 / 0 are the left / right member of a pair (Eqs (3),(4)),
+ *     c = 1..k-1 follow by Saul'yev's Eq (1) in ascending order, c = k..2k-2 by Eq (2) in
+ *     descending order; sweeps that reach a boundary read it.
  *   - 2-D (reading R-2D; the paper only claims the extension,
  *     PAPER.md:134, :228): 2x2 four-point groups anchored at (1+phase, 1+phase)
  *     (mod 2) -- diagonal shift --, in-group links implicit, out-of-group links
@@ -62,7 +66,7 @@ typedef enum {
     GE_EINVAL = -1,           /* bad argument; nothing was enqueued                   */
     GE_ENOMEM = -2,           /* host or device allocation failed                     */
     GE_ECUDA = -3,            /* a CUDA call failed; ge_strerror appends its message  */
-    GE_EUNSUPPORTED = -4      /* valid request the GPU path does not implement (group_k >= 2) */
+    GE_EUNSUPPORTED = -4      /* valid request the GPU path does not implement (group_k > 2048) */
 } ge_status;
 
 typedef struct {
@@ -70,8 +74,9 @@ typedef struct {
     int64_t   nx, ny;     /* interior nodes per axis, >= 1 (ny must be 1 when dim == 1)                */
     int64_t   batch;      /* independent 1-D rods, >= 1 (must be 1 when dim == 2)                      */
     int32_t   dtype;      /* ge_dtype: arithmetic and storage type of u                                */
-    int32_t   group_k;    /* 1 = two-point groups (2x2 groups in 2-D); >= 2 = PAPER.md:82 sub-domain
-                             length k: GE_EUNSUPPORTED on the GPU            */
+    int32_t   group_k;    /* 1 = two-point groups (2x2 groups in 2-D); 2..2048 = PAPER.md:82 sub-domain
+                             length k (1-D only; the paper's runs use 16): confluence pairs every 2k nodes
+                             joined by Saul'yev sweeps; always strategy A (one launch per level)       */
     const double *r;      /* HOST array, `batch` entries (dim 2: 1 entry), finite, > 0; copied         */
     const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; copied  */
     const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; copied  */

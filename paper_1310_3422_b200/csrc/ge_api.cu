@@ -18,6 +18,7 @@
 #include "ge_resident.cuh"
 #include "ge_stream.cuh"
 #include "ge_strip2d.cuh"
+#include "ge_level_k.cuh"
 
 namespace {
 
@@ -151,10 +152,36 @@ int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStre
     return GE_OK;
 }
 
+// ---- strategy A for sub-domain length k >= 2 (ge_level_k.cuh) ----
+constexpr size_t kLevelKSmemBudget = 96 * 1024;
+constexpr int kMaxGroupK = 2048;          // a unit of 2k+1 values (twice) must fit the shared-memory budget
+
+template <typename T>
+int launch_level_k(ge_plan* p, const void* uin, void* uout, int phase, cudaStream_t s) {
+    const ge::LevelKGeom g = ge::level_k_geom(p->group_k, phase, p->nx, sizeof(T), kLevelKSmemBudget);
+    if (g.upc < 1) return GE_EUNSUPPORTED;
+    const size_t smem = ge::level_k_smem(g, sizeof(T));
+    static bool configured = false;
+    if (!configured) {
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_level_k_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(kLevelKSmemBudget + 64)));
+        configured = true;
+    }
+    dim3 grid((unsigned)((g.units + g.upc - 1) / g.upc), (unsigned)(p->batch < 65535 ? p->batch : 65535));
+    ge::ge1d_level_k_kernel<T><<<grid, ge::kLevelKThreads, smem, s>>>((const T*)uin, (T*)uout, p->nx, p->batch,
+                                                                      (const ge::Coef1<T>*)p->coef, g);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    return GE_OK;
+}
+
 int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     const int phase = (int)(p->level & 1);
     int rc;
-    if (p->dim == 1) rc = p->dtype == GE_F64 ? launch_level_1d<double>(p, uin, uout, phase, s)
+    if (p->dim == 1 && p->group_k >= 2)
+        rc = p->dtype == GE_F64 ? launch_level_k<double>(p, uin, uout, phase, s)
+                                : launch_level_k<float>(p, uin, uout, phase, s);
+    else if (p->dim == 1) rc = p->dtype == GE_F64 ? launch_level_1d<double>(p, uin, uout, phase, s)
                                              : launch_level_1d<float>(p, uin, uout, phase, s);
     else             rc = p->dtype == GE_F64 ? launch_level_2d<double>(p, uin, uout, phase, s)
                                              : launch_level_2d<float>(p, uin, uout, phase, s);
@@ -451,7 +478,7 @@ const char* ge_strerror(int status) {
         case GE_OK: return "ok";
         case GE_EINVAL: return "invalid argument";
         case GE_ENOMEM: return "out of memory";
-        case GE_EUNSUPPORTED: return "unsupported on the GPU path (group_k >= 2 is SURVEY.md 8(f) NEXT-1)";
+        case GE_EUNSUPPORTED: return "unsupported on the GPU path (group_k > 2048: a unit does not fit in shared memory)";
         case GE_ECUDA:
             std::snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s", cudaGetErrorString(g_last_cuda));
             return g_errbuf;
@@ -477,7 +504,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     const int64_t nb = d->dim == 1 ? d->batch : 2;
     for (int64_t b = 0; b < nb; ++b)
         if (!std::isfinite(d->bc_lo[b]) || !std::isfinite(d->bc_hi[b])) return GE_EINVAL;
-    if (d->group_k >= 2) return GE_EUNSUPPORTED;
+    if (d->group_k > kMaxGroupK) return GE_EUNSUPPORTED;
 
     ge_plan* p = new (std::nothrow) ge_plan();
     if (!p) return GE_ENOMEM;
@@ -506,6 +533,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
+    if (d->group_k >= 2) kernel = GE_KERNEL_PER_STEP;      // k >= 2: strategy A only (ge_level_k.cuh)
     if (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT) {
         p->res_tb = d->tb;
         rc = resident_configure(p, 0);

@@ -1,0 +1,161 @@
+// ge_level_k.cuh -- strategy A for the paper's general scheme, sub-domain length
+// k >= 2 (the paper's own runs use k = 16):
+// one kernel launch per level, one HBM round trip per level.
+//
+// Rule table.  Class of node i: c = (i - phase*k) mod 2k.
+//   c = 0      right member of the confluence pair (i-1, i)      Eq (4)
+//   c = 1..k-1 Saul'yev A, ascending i, uses new_{i-1}           Eq (1)
+//   c = k..2k-2 Saul'yev B, descending i, uses new_{i+1}         Eq (2)
+//   c = 2k-1   left member of the pair (i, i+1)                  Eq (3)
+// A pair with a boundary member gives its interior member Eq (1)/(2) with the
+// boundary value as new-level neighbour; sweeps that reach a boundary read it.
+//
+// Ownership is the paper's: a thread owns one UNIT = 2k
+// consecutive nodes c = 0 .. 2k-1 (the paper's "sub-domain couple" seen from its
+// left wall): it forms the right member of the pair at its left wall, sweeps A
+// k-1 nodes to the right, forms the left member of the pair at its right wall and
+// sweeps B k-1 nodes to the left -- two independent serial chains, everything
+// it reads beyond its own nodes are the two old values either side.  What is not
+// the paper's: threads share only OLD values (one barrier after every thread has
+// read its four, then the unit is updated in place), the CTA stages its units through shared memory so
+// that HBM sees coalesced 128-byte lines (a unit is padded to 2k+1 words, which
+// makes the strided per-thread accesses bank-conflict-free), and the arithmetic
+// is the "value + correction" form of ge_common.cuh:
+//   Eq (1): new_i = old_i + e ((new_{i-1} - old_i) + (old_{i+1} - old_i)),  e = r/(1+r)
+//   Eq (2): new_i = old_i + e ((new_{i+1} - old_i) + (old_{i-1} - old_i))
+//   pair  : pair_update (Eqs (3),(4) factored)
+#pragma once
+#include "ge_common.cuh"
+
+namespace ge {
+
+constexpr int kLevelKThreads = 128;
+
+struct LevelKGeom {
+    int k;
+    int phase;
+    int upc;               // units per CTA (<= kLevelKThreads)
+    int64_t s0;            // node where unit 0 starts: 0 (phase 0) or -k (phase 1)
+    int64_t units;         // units per rod
+};
+
+inline LevelKGeom level_k_geom(int k, int phase, int64_t nx, size_t elem, size_t smem_budget) {
+    LevelKGeom g;
+    g.k = k; g.phase = phase;
+    g.s0 = phase ? -(int64_t)k : 0;
+    g.units = (nx - g.s0) / (2 * (int64_t)k) + 1;          // all units with start <= N
+    int64_t upc = (int64_t)((smem_budget - 4 * elem) / ((size_t)(2 * k + 1) * elem));
+    if (upc > kLevelKThreads) upc = kLevelKThreads;
+    if (upc > g.units) upc = g.units;
+    g.upc = (int)upc;                                       // 0: k too large for shared memory
+    return g;
+}
+inline size_t level_k_smem(const LevelKGeom& g, size_t elem) {
+    return ((size_t)g.upc * (2 * g.k + 1) + 4) * elem;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kLevelKThreads)
+ge1d_level_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
+                    const Coef1<T>* __restrict__ coef, const LevelKGeom g) {
+    extern __shared__ __align__(16) unsigned char levelk_smem[];
+    const int k = g.k, two_k = 2 * g.k, pitch = 2 * g.k + 1;
+    const int span = g.upc * two_k;                        // nodes of this CTA's units
+    T* so = reinterpret_cast<T*>(levelk_smem);             // unit u at u*pitch; old values, then new in place
+    T* sh = so + (size_t)g.upc * pitch;                    // old values of nodes S-2, S-1, S+span, S+span+1
+    const int64_t S = g.s0 + (int64_t)blockIdx.x * span;   // first node of the CTA
+    const int64_t N = nx;
+    for (int64_t rod = blockIdx.y; rod < batch; rod += gridDim.y) {
+        const Coef1<T> c = coef[rod];
+        const T* __restrict__ in = uin + rod * nx;
+        T* __restrict__ out = uout + rod * nx;
+        auto node_value = [&](int64_t i) -> T {            // old value of node i, boundaries included
+            if (i < 0 || i > N + 1) return T(0);
+            if (i == 0) return c.lo;
+            if (i == N + 1) return c.hi;
+            return __ldg(in + (i - 1));
+        };
+        // ---- coalesced load into the padded layout ----
+        {
+            int q = threadIdx.x / two_k, rem = threadIdx.x % two_k;
+            const int dq = kLevelKThreads / two_k, dr = kLevelKThreads % two_k;
+            for (int j = threadIdx.x; j < span; j += kLevelKThreads) {
+                so[q * pitch + rem] = node_value(S + j);
+                q += dq; rem += dr;
+                if (rem >= two_k) { rem -= two_k; ++q; }
+            }
+            if (threadIdx.x < 4) {
+                const int64_t i = threadIdx.x < 2 ? S - 2 + threadIdx.x : S + span + (threadIdx.x - 2);
+                sh[threadIdx.x] = node_value(i);
+            }
+        }
+        __syncthreads();
+        // ---- one unit per thread, in place ----
+        const int t = threadIdx.x;
+        const int64_t s = S + (int64_t)t * two_k;          // node with c = 0
+        const bool mine = t < g.upc && s <= N;
+        T* o = so + t * pitch;
+        T om2 = T(0), om1 = T(0), op0 = T(0), op1 = T(0);  // old values just outside the unit
+        if (mine) {
+            om2 = t > 0 ? o[-pitch + two_k - 2] : sh[0];
+            om1 = t > 0 ? o[-pitch + two_k - 1] : sh[1];
+            op0 = t + 1 < g.upc ? o[pitch] : sh[2];
+            op1 = t + 1 < g.upc ? o[pitch + 1] : sh[3];
+        }
+        __syncthreads();                                   // neighbours have read my edge values: overwrite freely
+        if (mine) {
+            const int64_t e = s + two_k - 1;               // node with c = 2k-1
+            // (1) right member of the pair (s-1, s), (3) left member of the pair (e, e+1)
+            T prev = c.lo;                                 // new value of the node left of the A sweep
+            T next = c.hi;                                 // new value of the node right of the B sweep
+            const T o0 = o[0], o1 = o[1], oe1 = o[two_k - 2], oe = o[two_k - 1];
+            if (s >= 1) {
+                T lo_, hi_;
+                pair_update_bc(om2, om1, o0, o1, c, s - 1 == 0, false, lo_, hi_);
+                prev = hi_;
+            }
+            if (e >= 1 && e <= N) {
+                T lo_, hi_;
+                pair_update_bc(oe1, oe, op0, op1, c, false, e + 1 == N + 1, lo_, hi_);
+                next = lo_;
+            }
+            // (2) Saul'yev A ascending from the left wall and (4) Saul'yev B descending from the right
+            // wall, one node of each per iteration: two independent chains that meet in the middle.
+            // Every iteration reads its four old values before it writes, so the update is in place.
+            T a_old = o1;                                  // old value of the A node of this iteration
+            T b_old = oe1;                                 // old value of the B node of this iteration
+            o[0] = prev; o[two_k - 1] = next;
+#pragma unroll 4
+            for (int m = 1; m < k; ++m) {
+                const int ja = m, jb = two_k - 1 - m;
+                const T a_nxt = o[ja + 1];                 // old_{i+1} of the A node (jb when the chains meet)
+                const T b_nxt = o[jb - 1];                 // old_{i-1} of the B node
+                const int64_t ia = s + ja, ib = s + jb;
+                if (ia >= 1 && ia <= N) {
+                    prev = fma(c.e, (prev - a_old) + (a_nxt - a_old), a_old);
+                    o[ja] = prev;
+                }
+                if (ib >= 1 && ib <= N) {
+                    next = fma(c.e, (next - b_old) + (b_nxt - b_old), b_old);
+                    o[jb] = next;
+                }
+                a_old = a_nxt; b_old = b_nxt;
+            }
+        }
+        __syncthreads();
+        // ---- coalesced store of the interior nodes ----
+        {
+            int q = threadIdx.x / two_k, rem = threadIdx.x % two_k;
+            const int dq = kLevelKThreads / two_k, dr = kLevelKThreads % two_k;
+            for (int j = threadIdx.x; j < span; j += kLevelKThreads) {
+                const int64_t i = S + j;
+                if (i >= 1 && i <= N) out[i - 1] = so[q * pitch + rem];
+                q += dq; rem += dr;
+                if (rem >= two_k) { rem -= two_k; ++q; }
+            }
+        }
+        __syncthreads();                                   // the buffers are reused by the next rod
+    }
+}
+
+}  // namespace ge

@@ -5,14 +5,14 @@ _TORCH_DT = {"f32": "float32", "f64": "float64"}
 
 
 def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc=0, hl=0, sync=None, rtb=0,
-            chunks=None):
+            chunks=None, k=1):
     """Run `steps` levels on cuda:0 and return the final state as a numpy array."""
     import torch
     from paper_1310_3422_b200 import libge
     dev = torch.device("cuda:0")
     u = torch.from_numpy(np.ascontiguousarray(cfg["u0"])).to(dev)
     stream = torch.cuda.current_stream(dev).cuda_stream
-    with libge.Plan(cfg, kernel=kernel, tb=tb, stream=stream) as plan:
+    with libge.Plan(cfg, kernel=kernel, tb=tb, stream=stream, group_k=k) as plan:
         plan.level = level0
         if tc:
             plan.tune(libge.GE_TUNE_TEMPORAL_C, tc)
@@ -52,15 +52,15 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc
     return u.cpu().numpy(), info
 
 
-def run_oracle(oracle, cfg, steps, level0=0):
+def run_oracle(oracle, cfg, steps, level0=0, k=1):
     u0 = cfg["u0"].astype(np.float64)
     if cfg["dim"] == 2:
         bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1])
         return oracle.run_2d(u0, cfg["r"][0], steps, bc, level0=level0)
     if cfg["batch"] == 1:
         return oracle.run_1d(u0.reshape(-1), cfg["r"][0], steps, cfg["bc_lo"][0], cfg["bc_hi"][0],
-                             level0=level0).reshape(u0.shape)
-    return oracle.run_batched_1d(u0, cfg["r"], steps, cfg["bc_lo"], cfg["bc_hi"], level0=level0)
+                             k=k, level0=level0).reshape(u0.shape)
+    return oracle.run_batched_1d(u0, cfg["r"], steps, cfg["bc_lo"], cfg["bc_hi"], k=k, level0=level0)
 
 
 def rel_err(got, ref):

@@ -201,6 +201,39 @@ def test_auto_picks_the_resident_kernels_when_the_state_fits_on_chip():
         assert info["kernel"] == ("persistent" if path else "temporal")
 
 
+# ------------------------------------------------------------------ sub-domain length k >= 2 ------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("k,n", [(2, 1), (2, 2), (2, 3), (2, 6), (2, 7), (3, 10), (3, 64), (5, 1003), (16, 62), (16, 30),
+                                 (16, 8206), (16, 5000), (7, 4099), (64, 20000), (100, 150), (1000, 5000)])
+def test_general_k_per_level(oracle, dtype, k, n):
+    """The paper's general scheme: confluence pairs every 2k
+    nodes joined by Saul'yev sweeps.  Paper-shaped layouts ((N+2) mod 2k == 0, e.g. k = 16,
+    N = 8206 -- the paper's "8208" nodes), ragged ones, rods shorter than a sub-domain, both starting
+    phases, per-rod r and unequal boundary values."""
+    cfg = inputs.random_rods(3, n, dtype, seed=17 * k + n)
+    for level0, steps in ((0, 1), (1, 1), (0, 2), (1, 7), (0, 40)):
+        got, info = run_gpu(cfg, steps, level0=level0, k=k)
+        ref = run_oracle(oracle, cfg, steps, level0=level0, k=k)
+        assert info["kernel"] == "per_step" and info["launches"] == steps
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (k, n, level0, steps)
+
+
+def test_general_k_matches_the_closed_form(oracle):
+    """k = 16 on N = 254 (the paper's SDC width 32): the end state follows e^{-pi^2 t} sin(pi x) to the
+    oracle's own error (tests/golden P6: 5.35e-5 at t ~ 0.1, r = 1)."""
+    n, r = 254, 1.0
+    x = np.arange(1, n + 1) / (n + 1.0)
+    steps = int(round(0.1 * (n + 1) ** 2 / r))
+    cfg = dict(inputs.random_rods(1, n, "f64"), r=np.array([r]), bc_lo=np.array([0.0]), bc_hi=np.array([0.0]),
+               u0=np.sin(np.pi * x)[None, :].copy())
+    got, _ = run_gpu(cfg, steps, k=16)
+    ref = run_oracle(oracle, cfg, steps, k=16)
+    assert rel_err_rows(got, ref, cfg) <= TOL["f64"]
+    t = steps * r / (n + 1.0) ** 2
+    err = np.abs(got.reshape(-1) - np.exp(-np.pi ** 2 * t) * np.sin(np.pi * x)).max()
+    assert 3e-5 < err < 8e-5, err
+
+
 # ------------------------------------------------------------------ 2-D ------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("nx,ny", [(1, 1), (2, 2), (3, 3), (4, 4), (5, 4), (4, 7), (8, 8), (64, 32), (130, 67), (131, 66), (256, 256)])
