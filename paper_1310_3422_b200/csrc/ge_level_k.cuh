@@ -75,12 +75,23 @@ ge1d_level_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx,
             if (i == N + 1) return c.hi;
             return __ldg(in + (i - 1));
         };
-        // ---- coalesced load into the padded layout ----
+        // ---- coalesced load into the padded layout: one cp.async per node (HBM -> shared memory without
+        //      a register in between, all of a thread's copies in flight together) ----
         {
             int q = threadIdx.x / two_k, rem = threadIdx.x % two_k;
             const int dq = kLevelKThreads / two_k, dr = kLevelKThreads % two_k;
             for (int j = threadIdx.x; j < span; j += kLevelKThreads) {
-                so[q * pitch + rem] = node_value(S + j);
+                const int64_t i = S + j;
+                T* dst = so + q * pitch + rem;
+                if (i >= 1 && i <= N) {
+                    const uint32_t d32 = (uint32_t)__cvta_generic_to_shared(dst);
+                    if constexpr (sizeof(T) == 8)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d32), "l"(in + (i - 1)) : "memory");
+                    else
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d32), "l"(in + (i - 1)) : "memory");
+                } else {
+                    *dst = node_value(i);
+                }
                 q += dq; rem += dr;
                 if (rem >= two_k) { rem -= two_k; ++q; }
             }
@@ -88,6 +99,7 @@ ge1d_level_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx,
                 const int64_t i = threadIdx.x < 2 ? S - 2 + threadIdx.x : S + span + (threadIdx.x - 2);
                 sh[threadIdx.x] = node_value(i);
             }
+            asm volatile("cp.async.wait_all;" ::: "memory");
         }
         __syncthreads();
         // ---- one unit per thread, in place ----
