@@ -407,7 +407,7 @@ def roofline(cfg, info, total_ms, launches, steps):
         names["per_step"] = "ge%dd_level_k_kernel"
     if kernel == "persistent":
         name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
-    elif kernel == "temporal" and info.get("temporal_c") in (18, 36):
+    elif kernel == "temporal" and info.get("temporal_c") in (18, 22, 26, 36, 44, 52):
         name = "ge1d_stream_kernel"                      # the TMA-staged form of strategy B
     elif kernel == "temporal" and cfg["dim"] == 2 and cfg["nx"] % 4 == 0 and cfg["nx"] >= 128:
         name = "ge2d_strip_kernel"                       # the drift-free form of strategy B in 2-D

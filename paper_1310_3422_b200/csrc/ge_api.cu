@@ -189,6 +189,24 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     return rc;
 }
 
+// persistent grid of the TMA-staged kernel: queried once per plan and tile width
+template <typename T, int C>
+cudaError_t stream_dispatch(ge_plan* p, const T* in, T* out, const ge::Coef1<T>* c, int tb, int phase, cudaStream_t s) {
+    if (p->stream_ctas == 0) {
+        int per_sm = 0;
+        auto* fn = &ge::ge1d_stream_kernel<T, C>;
+        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (e == cudaSuccess && ge::stream_smem_bytes<T, C>() > 48 * 1024)
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ge::stream_smem_bytes<T, C>());
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ge::kStreamWarps * 32, ge::stream_smem_bytes<T, C>());
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorInvalidConfiguration;
+        p->stream_ctas = per_sm * p->sm_count;
+    }
+    return ge::stream1d_launch<T, C>(in, out, p->nx, p->batch, c, tb, phase, p->stream_ctas, s);
+}
+
 // ---- strategy B launch (1-D): tb levels from the plan's current level (any phase) ----
 template <typename T>
 int launch_temporal_1d(ge_plan* p, const void* uin, void* uout, int tb, cudaStream_t s) {
@@ -200,20 +218,14 @@ int launch_temporal_1d(ge_plan* p, const void* uin, void* uout, int tb, cudaStre
     constexpr int C0 = 16 / (int)sizeof(T) * 4;     // 8 (f64) / 16 (f32)
     // rods of at least one tile take the drift-free kernels, shorter ones the generic (drifting) one
     const bool df = p->nx >= 32 * (int64_t)p->tc;
-    constexpr int CS = 144 / (int)sizeof(T);         // 18 (f64) / 36 (f32): the TMA-staged kernel
+    // the TMA-staged kernel: lane strides of 144 / 176 / 208 bytes (odd multiples of 16: conflict-free)
+    constexpr int CS = 144 / (int)sizeof(T), CS2 = 176 / (int)sizeof(T), CS3 = 208 / (int)sizeof(T);
     switch (p->tc) {
-        case CS: {
+        case CS: case CS2: case CS3: {
             if (!df) return GE_EINVAL;
-            if (p->stream_ctas == 0) {
-                int per_sm = 0;
-                auto* fn = &ge::ge1d_stream_kernel<T, CS>;
-                GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-                GE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ge::kStreamWarps * 32,
-                                                                      ge::stream_smem_bytes<T, CS>()));
-                p->stream_ctas = per_sm * p->sm_count;
-                if (p->stream_ctas < 1) return GE_ECUDA;
-            }
-            e = ge::stream1d_launch<T, CS>(in, out, p->nx, p->batch, c, tb, phase, p->stream_ctas, s);
+            e = p->tc == CS ? stream_dispatch<T, CS>(p, in, out, c, tb, phase, s)
+              : p->tc == CS2 ? stream_dispatch<T, CS2>(p, in, out, c, tb, phase, s)
+                             : stream_dispatch<T, CS3>(p, in, out, c, tb, phase, s);
             break;
         }
         case C0:
@@ -284,10 +296,11 @@ bool temporal_ok(const ge_plan* p, const void* u) {
     return p->nx % V == 0 && ((uintptr_t)u % 16 == 0) && ((uintptr_t)p->scratch % 16 == 0);
 }
 
-int stream_tc(int dtype) { return dtype == GE_F64 ? 18 : 36; }
-// the TMA-staged kernel when the rod holds at least a few tiles, else the warp-per-tile one
+int stream_tc(int dtype) { return dtype == GE_F64 ? 22 : 52; }     // measured on C4 / C3
+bool is_stream_tc(int dtype, int64_t tc) { const int64_t b = dtype == GE_F64 ? 8 : 4; return tc * b == 144 || tc * b == 176 || tc * b == 208; }
+// the TMA-staged kernel when the rod holds at least two tiles, else the warp-per-tile one
 int default_tc(int dtype, int64_t nx) {
-    return nx >= 4 * 32 * (int64_t)stream_tc(dtype) ? stream_tc(dtype) : (dtype == GE_F64 ? 16 : 32);
+    return nx >= 2 * 32 * (int64_t)stream_tc(dtype) ? stream_tc(dtype) : (dtype == GE_F64 ? 16 : 32);
 }
 int clamp_tb(const ge_plan* p, int64_t tb) {
     const int mx = ge::temporal1d_max_tb(p->tc);
@@ -543,7 +556,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->kernel = kernel;
     const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
     // measured on C4: the TMA-staged kernel is fp64-bound from tb ~ 12 on, best near 20
-    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (p->tc == stream_tc(p->dtype) ? 20 : 16));
+    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (is_stream_tc(p->dtype, p->tc) ? 20 : 16));
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
@@ -600,9 +613,22 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                 left -= 1;
             }
         } else if (temporal) {
-            // equal-sized blocks: ceil(left / tb) launches of (almost) the same number of levels
-            const int64_t nl = (left + p->tb - 1) / p->tb;
-            const int tbn = (int)((left + nl - 1) / nl);
+            int tbn;
+            if (p->tb % 2 == 0 && p->tb >= 4) {
+                // blocks that start at an odd level and have an even length are pure R/L pairs: a run from
+                // an even level opens with one block of tb-1 levels (in-lane level I first), a tail of one
+                // or two levels joins the last block (which may then end with R + shift back)
+                const int64_t nl = left > 2 ? (left - 2 + p->tb - 1) / p->tb : 1;   // launches to go (a block may take tb+2)
+                int64_t q = (left + nl - 1) / nl;
+                q += q & 1;
+                tbn = (int)((p->level & 1) ? q : q - 1);
+                if (tbn > left) tbn = (int)left;
+                if (left - tbn <= 2 && left <= ge::temporal1d_max_tb(p->tc)) tbn = (int)left;
+            } else {
+                // equal-sized blocks: ceil(left / tb) launches of (almost) the same number of levels
+                const int64_t nl = (left + p->tb - 1) / p->tb;
+                tbn = (int)((left + nl - 1) / nl);
+            }
             rc = p->dtype == GE_F64 ? launch_temporal_1d<double>(p, cur, oth, tbn, s)
                                     : launch_temporal_1d<float>(p, cur, oth, tbn, s);
             left -= tbn;
@@ -689,7 +715,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_TEMPORAL_C: {
             if (p->dim != 1) return GE_EINVAL;
             const int c0 = p->dtype == GE_F64 ? 8 : 16;
-            if (value == stream_tc(p->dtype)) { if (p->nx < 32 * value) return GE_EINVAL; }
+            if (is_stream_tc(p->dtype, value)) { if (p->nx < 32 * value) return GE_EINVAL; p->stream_ctas = 0; }
             else if (value != c0 && value != 2 * c0 && value != 4 * c0) return GE_EINVAL;
             p->tc = (int32_t)value;
             if (p->kernel == GE_KERNEL_TEMPORAL) p->tb = clamp_tb(p, p->tb);

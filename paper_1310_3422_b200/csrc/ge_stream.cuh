@@ -14,11 +14,11 @@
 //     tile i+1 is in flight into the warp's second buffer, and the bulk store of
 //     tile i-1 drains from it.  Two buffers and two mbarriers per warp; no
 //     __syncthreads anywhere.
-//   * a lane's chunk is C values with C*sizeof(T) = 144 bytes (C = 18 fp64,
-//     36 fp32): the lane stride is an odd multiple of 16 bytes, so the 16-byte
+//   * a lane's chunk is C values with C*sizeof(T) = 144, 176 or 208 bytes (C =
+//     18, 22, 26 fp64; 36, 44, 52 fp32): the lane stride is an odd multiple of 16 bytes, so the 16-byte
 //     shared-memory accesses of a quarter-warp fall into 8 different bank
 //     groups -- conflict-free without padding, and the tile stays ONE linear
-//     4608-byte block that a single 1-D bulk copy moves.
+//     block (5632 bytes at the default C) that a single 1-D bulk copy moves.
 //   * tile layout, level code and arithmetic are those of the drift-free
 //     warp-per-tile kernel (ge_temporal.cuh temporal1d_tile_df; level code in
 //     ge_resident.cuh): tile 0 left-aligned, last tile right-aligned, tb stale

@@ -70,15 +70,15 @@ def test_step_rejects_bad_arguments():
 
 # ------------------------------------------------------------------ strategy B, 1-D ------
 @pytest.mark.parametrize("dtype,tb,tc", [("f64", 0, 0), ("f64", 1, 8), ("f64", 2, 16), ("f64", 7, 8), ("f64", 13, 16),
-                                         ("f64", 32, 8), ("f64", 100, 16), ("f64", 24, 32), ("f64", 16, 18), ("f64", 7, 18), ("f64", 61, 18), ("f32", 0, 0), ("f32", 50, 64),
-                                         ("f32", 16, 36), ("f32", 9, 36), ("f32", 120, 36), ("f32", 1, 32), ("f32", 3, 16),
+                                         ("f64", 32, 8), ("f64", 100, 16), ("f64", 24, 32), ("f64", 16, 18), ("f64", 7, 18), ("f64", 61, 18), ("f64", 20, 22), ("f64", 9, 26), ("f32", 0, 0), ("f32", 50, 64),
+                                         ("f32", 16, 36), ("f32", 9, 36), ("f32", 120, 36), ("f32", 20, 44), ("f32", 33, 52), ("f32", 1, 32), ("f32", 3, 16),
                                          ("f32", 6, 32), ("f32", 8, 16), ("f32", 21, 32), ("f32", 40, 16), ("f32", 200, 32)])
 @pytest.mark.parametrize("n", [8, 224, 232, 2048, 10000, 3 * 4096 + 8])
 def test_temporal_1d(oracle, dtype, tb, tc, n):
     """Strategy B against the oracle: every starting phase, odd and even block lengths (pre/post
     realignment shifts), tiles with both ghosts, ragged last tile; the warp-per-tile kernels (generic
-    and drift-free) and the TMA-staged persistent kernel (tc = 18 / 36)."""
-    if tc in (18, 36) and n < 32 * tc:
+    and drift-free) and the TMA-staged persistent kernel (tc = 18, 22, 26 / 36, 44, 52)."""
+    if tc in (18, 22, 26, 36, 44, 52) and n < 32 * tc:
         pytest.skip("the TMA-staged kernel needs a rod of at least one tile")
     cfg = inputs.random_rods(2, n, dtype, seed=7 * n + tb)
     for level0, steps in ((0, 1), (1, 16), (0, 40), (1, 37), (0, 101)):
