@@ -267,8 +267,14 @@ int launch_temporal_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) 
     return GE_OK;
 }
 // ---- strategy B launch (2-D, drift-free strips): plan->tb levels from the current PHASE-1 level ----
-constexpr int kStripC = 4;
-bool strip2d_ok(const ge_plan* p) { return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * kStripC; }
+#ifndef GE_STRIP_C_F32
+#define GE_STRIP_C_F32 4
+#endif
+template <typename T> struct StripC { static constexpr int c = sizeof(T) == 8 ? 4 : GE_STRIP_C_F32; };
+bool strip2d_ok(const ge_plan* p) {
+    const int c = p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c;
+    return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * c;
+}
 
 template <typename T>
 int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
@@ -277,9 +283,9 @@ int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     auto* c = (const ge::Coef2<T>*)p->coef;
     cudaError_t e;
     switch (p->tb) {
-        case 4: e = ge::strip2d_launch<T, kStripC, 4>(in, out, p->nx, p->ny, c, p->hp, s); break;
-        case 6: e = ge::strip2d_launch<T, kStripC, 6>(in, out, p->nx, p->ny, c, p->hp, s); break;
-        case 8: e = ge::strip2d_launch<T, kStripC, 8>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 4: e = ge::strip2d_launch<T, StripC<T>::c, 4>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 6: e = ge::strip2d_launch<T, StripC<T>::c, 6>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 8: e = ge::strip2d_launch<T, StripC<T>::c, 8>(in, out, p->nx, p->ny, c, p->hp, s); break;
         default: return GE_EINVAL;
     }
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
@@ -542,7 +548,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     // the chip (1-D only), else the temporally blocked ones
     p->tb = 0;
     p->tc = default_tc(p->dtype, p->nx);
-    p->hp = 64;
+    p->hp = 56;                    // measured on C5
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
