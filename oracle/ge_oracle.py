@@ -43,6 +43,8 @@ def _load():
         lib = ctypes.CDLL(build())
         lib.ge_ref_level_1d.argtypes = [_f64p, _f64p, _i64, _f64, _i64, _i64]
         lib.ge_ref_level_1d.restype = None
+        lib.ge_ref_level_1d_src.argtypes = [_f64p, _f64p, _i64, _f64, _i64, _i64, ctypes.c_void_p, _f64, _f64]
+        lib.ge_ref_level_1d_src.restype = None
         lib.ge_ref_run_1d.argtypes = [_f64p, _i64, _f64, _i64, _f64, _f64, _i64, _i64]
         lib.ge_ref_run_1d.restype = ctypes.c_int
         lib.ge_ref_run_batched_1d.argtypes = [_f64p, _i64, _i64, _f64p, _i64, _f64p, _f64p, _i64, _i64]
@@ -64,6 +66,24 @@ def level_1d(u, r, phase, bc_lo=0.0, bc_hi=0.0, k=1):
     old[1:-1] = u
     new = np.empty_like(old)
     _load().ge_ref_level_1d(old, new, n, float(r), int(k), int(phase))
+    return new[1:-1].copy()
+
+
+def level_1d_src(u, r, phase, bc_old, bc_new, s=None, k=1):
+    """One level with a source term and moving boundary values (reading R-N3): bc_old = (lo, hi)
+    at the old level, bc_new at the new level, s[i] = tau*f at interior node i+1 (or None)."""
+    u = np.asarray(u, dtype=np.float64)
+    n = u.shape[0]
+    old = np.empty(n + 2, dtype=np.float64)
+    old[0], old[-1] = bc_old
+    old[1:-1] = u
+    new = np.empty_like(old)
+    sp = None
+    if s is not None:
+        sp = np.zeros(n + 2, dtype=np.float64)
+        sp[1:-1] = np.asarray(s, dtype=np.float64)
+    _load().ge_ref_level_1d_src(old, new, n, float(r), int(k), int(phase),
+                                sp.ctypes.data if sp is not None else None, float(bc_new[0]), float(bc_new[1]))
     return new[1:-1].copy()
 
 

@@ -93,6 +93,58 @@ void ge_ref_level_1d(const double *old_, double *new_, int64_t N, double r,
 }
 
 /*
+ * One level in 1-D with a source term and time-dependent boundary values
+ * (reading R-N3; SURVEY.md 8(f) NEXT-3 -- the paper's model problem has
+ * neither; PAPER.md:37 only mentions the diffusion step inside
+ * an operator splitting):   u_t = u_xx + f(x,t),  u(0,t) = lo(t),  u(1,t) = hi(t).
+ * Saul'yev's asymmetric equations gain tau*f at their node,
+ *   Eq (1): (1+r) new_i = r new_{i-1} + (1-r) old_i + r old_{i+1} + s_i
+ *   Eq (2): (1+r) new_i = r new_{i+1} + (1-r) old_i + r old_{i-1} + s_i
+ * and a confluence pair is the 2x2 system of Eq (2) at i with Eq (1) at i+1,
+ * whose solution is the bracket of Eq (3)/(4) plus (1+r) s_i + r s_{i+1}
+ * (resp. r s_i + (1+r) s_{i+1}), all over 1+2r.  Old-level reads of a boundary
+ * node take its OLD value (old_[0], old_[N+1]); the new-level neighbour of a
+ * truncated pair or of a sweep is the NEW value (lo_new, hi_new).
+ * s: length N+2, s[i] = tau * f(x_i, t*) for i = 1..N (t* is the caller's
+ * choice), or NULL for no source.
+ */
+void ge_ref_level_1d_src(const double *old_, double *new_, int64_t N, double r,
+                         int64_t k, int64_t phase, const double *s,
+                         double lo_new, double hi_new)
+{
+    const int64_t two_k = 2 * k;
+    int64_t i;
+    new_[0] = lo_new;
+    new_[N + 1] = hi_new;
+    for (i = 0; i <= N; ++i) {
+        if (pmod(i - phase * k, two_k) != two_k - 1) continue;
+        if (i >= 1 && i + 1 <= N) {
+            const double si = s ? s[i] : 0.0, sj = s ? s[i + 1] : 0.0;
+            new_[i] = ((r + r * r) * old_[i - 1] + (1.0 - r * r) * old_[i]
+                       + (r - r * r) * old_[i + 1] + r * r * old_[i + 2]
+                       + (1.0 + r) * si + r * sj) / (1.0 + 2.0 * r);
+            new_[i + 1] = (r * r * old_[i - 1] + (r - r * r) * old_[i]
+                           + (1.0 - r * r) * old_[i + 1] + (r + r * r) * old_[i + 2]
+                           + r * si + (1.0 + r) * sj) / (1.0 + 2.0 * r);
+        } else if (i == 0 && N >= 1) {
+            new_[1] = (r * new_[0] + (1.0 - r) * old_[1] + r * old_[2] + (s ? s[1] : 0.0)) / (1.0 + r);
+        } else if (i == N && N >= 1) {
+            new_[N] = (r * new_[N + 1] + (1.0 - r) * old_[N] + r * old_[N - 1] + (s ? s[N] : 0.0)) / (1.0 + r);
+        }
+    }
+    for (i = 1; i <= N; ++i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= 1 && c <= k - 1)
+            new_[i] = (r * new_[i - 1] + (1.0 - r) * old_[i] + r * old_[i + 1] + (s ? s[i] : 0.0)) / (1.0 + r);
+    }
+    for (i = N; i >= 1; --i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= k && c <= two_k - 2)
+            new_[i] = (r * new_[i + 1] + (1.0 - r) * old_[i] + r * old_[i - 1] + (s ? s[i] : 0.0)) / (1.0 + r);
+    }
+}
+
+/*
  * `steps` levels of one rod starting at level counter `level0` (phase =
  * level mod 2, phase 0 first: DESIGN.md reading R-A3).  u holds the N
  * interior values and is overwritten by the final level.  Returns 0, or -1 if

@@ -53,6 +53,32 @@ def system_1d(n, r, k, phase, bc_lo, bc_hi, num=float):
     return A, B, c
 
 
+def level_1d_dense_src(u, r, k, phase, bc_old, bc_new, s=None):
+    """Implicit statement with a source term and moving boundary values (reading R-N3): a boundary
+    neighbour taken at the new level contributes its NEW value, one taken at the old level its OLD value."""
+    n = len(u)
+    r = float(r)
+    A = np.zeros((n, n)); B = np.zeros((n, n)); c = np.zeros(n)
+    side = classes_1d(n, k, phase)
+    old_b = {0: bc_old[0], n + 1: bc_old[1]}
+    new_b = {0: bc_new[0], n + 1: bc_new[1]}
+    for i in range(1, n + 1):
+        A[i - 1, i - 1] = 1 + r
+        B[i - 1, i - 1] = 1 - r
+        jn, jo = i + side[i], i - side[i]
+        if jn in new_b:
+            c[i - 1] += r * new_b[jn]
+        else:
+            A[i - 1, jn - 1] -= r
+        if jo in old_b:
+            c[i - 1] += r * old_b[jo]
+        else:
+            B[i - 1, jo - 1] += r
+    if s is not None:
+        c = c + np.asarray(s, dtype=np.float64)
+    return np.linalg.solve(A, B @ np.asarray(u, dtype=np.float64) + c)
+
+
 def solve_exact(A, b):
     """Gaussian elimination over Fractions."""
     n = len(A)
