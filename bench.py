@@ -363,6 +363,57 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_src(args):
+    """NEXT-3 measurement: `levels` launches of ge_step_1d_src (source array + moving boundary values) on
+    the C4-shaped rod; HBM-bound, 3*sizeof(T) algorithmic bytes per update (u in, tau*f in, u out)."""
+    import torch
+    from paper_1310_3422_b200 import build as gebuild, libge
+    gebuild.build()
+    libge.load()
+    dev = torch.device("cuda", 0)
+    cfg = make_cfg(args.config)
+    levels = args.levels or cfg["steps"]
+    es = ESIZE[cfg["dtype"]]
+    stream_obj = torch.cuda.current_stream(dev)
+    stream = stream_obj.cuda_stream
+    u = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
+    v = torch.empty_like(u)
+    src = torch.full_like(u, 1e-9)
+    plan = libge.Plan(cfg, kernel="per_step", stream=stream)
+
+    def step():
+        a, b = u, v
+        for n in range(levels):
+            t = 1e-3 * n
+            plan.step_src(a.data_ptr(), b.data_ptr(), src.data_ptr(), (t, t + 1e-3, -t, -t - 1e-3), stream)
+            a, b = b, a
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream_obj)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream_obj)
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    peaks, srcp = measured_peaks()
+    upd = cfg["nx"] * levels * args.steps
+    gbs = 3.0 * es * upd / (ms * 1e-3) / 1e9
+    print(json.dumps({
+        "metric": METRIC, "value": upd / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
+        "config": {"workload": workload_desc(cfg) + ", source term + moving boundary values (NEXT-3)",
+                   "levels_per_step": levels, "kernel": "per_step"},
+        "gpu_launches": levels * args.steps, "finite": bool(torch.isfinite(u).all().item()),
+        "roofline": {"kernel": "ge1d_level_src_kernel<%s>" % cfg["dtype"], "bound": "hbm", "achieved": gbs,
+                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"], "traffic": None,
+                     "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * cfg["nx"]},
+        "e2e": None, "cpu_baseline": None}), flush=True)
+    plan.close()
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -450,6 +501,7 @@ def main():
     ap.add_argument("--rtb", type=int, default=0, help="whole-chip persistent kernel: levels between meetings")
     ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines"], help="whole-chip persistent kernel: meeting kind")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
+    ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-scale", type=float, default=1 / 64, help="grid fraction of the cpu_baseline sample")
@@ -457,7 +509,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         sys.stderr.write("bench.py: warning: fewer than 3 warm-up steps; the number is not reportable\n")
-    if args.impl == "reference":
+    if args.src:
+        run_src(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -99,6 +99,18 @@ int ge_plan_create(ge_plan **out, const ge_desc *desc, ge_stream_t stream);
 int ge_step_1d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 int ge_step_2d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 
+/* One level of a single rod (batch == 1, group_k == 1) with NON-CONSTANT problem data (SURVEY.md 8(f)
+ * NEXT-3, reading R-N3; the paper's model problem has neither):
+ * u_t = u_xx + f(x,t) with boundary values that move in time.
+ *   tau_f: device pointer, nx elements of dtype, tau_f[i] = tau * f(x_{i+1}, t*) (the time point t*
+ *          is the caller's choice, e.g. the middle of the level), or NULL for no source;
+ *   bc4:   HOST array {lo_old, lo_new, hi_old, hi_new}: the values of nodes 0 and N+1 at the old and
+ *          at the new level (the plan's constant boundary values are not used).
+ * Otherwise as ge_step_1d (phase = level & 1, level += 1, one launch).  GE_EINVAL for batch > 1 or
+ * dim == 2, GE_EUNSUPPORTED for group_k >= 2. */
+int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f, const double *bc4,
+                   ge_stream_t stream);
+
 /* `steps` >= 0 levels in place: on completion of the enqueued work u holds level (level0+steps) and
  * the plan's level counter has advanced by `steps`.  The plan's scratch level is used for
  * ping-ponging; the strategy is the plan's (AUTO/PER_STEP/TEMPORAL/PERSISTENT).  steps == 0 is a no-op. */

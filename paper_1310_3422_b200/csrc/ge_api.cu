@@ -19,6 +19,7 @@
 #include "ge_stream.cuh"
 #include "ge_strip2d.cuh"
 #include "ge_level_k.cuh"
+#include "ge_level_src.cuh"
 
 namespace {
 
@@ -574,6 +575,35 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
 
 int ge_step_1d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
     return step_common(p, 1, u_in, u_out, (cudaStream_t)stream);
+}
+
+int ge_step_1d_src(ge_plan* p, const void* u_in, void* u_out, const void* tau_f, const double* bc4,
+                   ge_stream_t stream) {
+    if (!p || !u_in || !u_out || u_in == u_out || !bc4 || p->dim != 1 || p->batch != 1) return GE_EINVAL;
+    if (p->group_k != 1) return GE_EUNSUPPORTED;
+    for (int i = 0; i < 4; ++i) if (!std::isfinite(bc4[i])) return GE_EINVAL;
+    const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)u_in % es || (uintptr_t)u_out % es || (uintptr_t)tau_f % es) return GE_EINVAL;
+    const char* a = (const char*)u_in; const char* b = (const char*)u_out;
+    const size_t bytes = (size_t)p->count * es;
+    if ((a < b + bytes) && (b < a + bytes)) return GE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    p->last_stream = s;
+    const int phase = (int)(p->level & 1);
+    cudaError_t e;
+    if (p->dtype == GE_F64) {
+        const ge::SrcBc<double> bc{bc4[0], bc4[1], bc4[2], bc4[3]};
+        e = ge::level_src_launch<double>((const double*)u_in, (double*)u_out, (const double*)tau_f, p->nx,
+                                         (const ge::Coef1<double>*)p->coef, bc, phase, s);
+    } else {
+        const ge::SrcBc<float> bc{(float)bc4[0], (float)bc4[1], (float)bc4[2], (float)bc4[3]};
+        e = ge::level_src_launch<float>((const float*)u_in, (float*)u_out, (const float*)tau_f, p->nx,
+                                        (const ge::Coef1<float>*)p->coef, bc, phase, s);
+    }
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += 1;
+    return GE_OK;
 }
 
 int ge_step_2d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {

@@ -33,7 +33,7 @@ _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
 _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 
 # every symbol include/ge.h declares
-EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_2d", "ge_run", "ge_run_host",
+EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_step_2d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
            "ge_strerror", "ge_version")
 
@@ -76,6 +76,7 @@ def load() -> ctypes.CDLL:
     lib.ge_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ge_desc), vp]
     lib.ge_step_1d.argtypes = [vp, vp, vp, vp]
     lib.ge_step_2d.argtypes = [vp, vp, vp, vp]
+    lib.ge_step_1d_src.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run.argtypes = [vp, vp, i64, vp]
     lib.ge_run_host.argtypes = [vp, vp, i64, vp]
     lib.ge_plan_get_level.argtypes = [vp, ctypes.POINTER(i64)]
@@ -134,6 +135,14 @@ def _check(rc: int, where: str):
 
 def ge_step_1d(plan: int, u_in: int, u_out: int, stream: int = 0):
     _check(load().ge_step_1d(plan, u_in, u_out, stream), "ge_step_1d")
+
+
+def ge_step_1d_src(plan: int, u_in: int, u_out: int, tau_f: int, bc4: Sequence[float], stream: int = 0):
+    """bc4 = (lo_old, lo_new, hi_old, hi_new); tau_f = device pointer or 0."""
+    arr = _darr(bc4)
+    if len(arr) != 4:
+        raise GeError(GE_EINVAL, "ge_step_1d_src (bc4 needs four values)")
+    _check(load().ge_step_1d_src(plan, u_in, u_out, tau_f or None, arr, stream), "ge_step_1d_src")
 
 
 def ge_step_2d(plan: int, u_in: int, u_out: int, stream: int = 0):
@@ -195,6 +204,9 @@ class Plan:
 
     def step(self, u_in: int, u_out: int, stream: int = 0):
         (ge_step_1d if self.cfg["dim"] == 1 else ge_step_2d)(self.handle, u_in, u_out, stream)
+
+    def step_src(self, u_in: int, u_out: int, tau_f: int, bc4, stream: int = 0):
+        ge_step_1d_src(self.handle, u_in, u_out, tau_f, bc4, stream)
 
     def run(self, u: int, steps: int, stream: int = 0):
         ge_run(self.handle, u, steps, stream)

@@ -1,0 +1,100 @@
+"""GPU parity for ge_step_1d_src (source term + time-dependent boundary values; SURVEY.md 8(f) NEXT-3,
+DESIGN.md reading R-N3) against oracle/ge_ref.c ge_ref_level_1d_src, element by element."""
+import numpy as np
+import pytest
+
+from gpu_util import TOL, run_gpu
+from paper_1310_3422_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+_NP = {"f32": np.float32, "f64": np.float64}
+
+
+def _march(oracle, cfg, steps, level0, srcs, bcs, use_src=True):
+    """GPU and oracle side by side on the same per-level data; returns (gpu, oracle) final levels."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    dt = _NP[cfg["dtype"]]
+    dev = torch.device("cuda:0")
+    u = torch.from_numpy(cfg["u0"].reshape(-1).copy()).to(dev)
+    v = torch.empty_like(u)
+    s = torch.cuda.current_stream(dev).cuda_stream
+    ref = cfg["u0"].reshape(-1).astype(np.float64)
+    r = float(cfg["r"][0])
+    with libge.Plan(cfg, kernel="per_step", stream=s) as plan:
+        plan.level = level0
+        for n in range(steps):
+            src = srcs[n].astype(dt)
+            lo_o, lo_n, hi_o, hi_n = [float(dt(x)) for x in bcs[n]]       # what the GPU will see
+            d_src = torch.from_numpy(src).to(dev)
+            plan.step_src(u.data_ptr(), v.data_ptr(), d_src.data_ptr() if use_src else 0, (lo_o, lo_n, hi_o, hi_n), s)
+            torch.cuda.synchronize(dev)
+            u, v = v, u
+            ref = oracle.level_1d_src(ref, r, (level0 + n) % 2, (lo_o, hi_o), (lo_n, hi_n),
+                                      src.astype(np.float64) if use_src else None)
+        assert plan.level == level0 + steps and plan.info()["launches"] == steps
+    return u.cpu().numpy().astype(np.float64), ref
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("n", [1, 2, 3, 8, 9, 1000, 4099, 65536])
+def test_step_src_matches_the_oracle(oracle, dtype, n):
+    cfg = inputs.random_rods(1, n, dtype, seed=n)
+    rng = np.random.default_rng(n + 5)
+    for level0 in (0, 1):
+        steps = 6
+        srcs = [rng.uniform(-0.1, 0.1, n) for _ in range(steps)]
+        walk = rng.uniform(-1, 1, (steps + 1, 2))                       # boundary values level by level
+        bcs = [(walk[i, 0], walk[i + 1, 0], walk[i, 1], walk[i + 1, 1]) for i in range(steps)]
+        got, ref = _march(oracle, cfg, steps, level0, srcs, bcs)
+        scale = max(np.abs(ref).max(), np.abs(walk).max())
+        assert np.abs(got - ref).max() / scale <= TOL[dtype], (n, level0)
+
+
+def test_step_src_without_source_and_with_fixed_boundaries_is_the_plain_level(oracle):
+    for dtype in ("f64", "f32"):
+        cfg = inputs.random_rods(1, 5000, dtype, seed=3)
+        lo, hi = float(cfg["bc_lo"][0]), float(cfg["bc_hi"][0])
+        for level0 in (0, 1):
+            got, _ = _march(oracle, cfg, 5, level0, [np.zeros(5000)] * 5, [(lo, lo, hi, hi)] * 5, use_src=False)
+            same, _ = run_gpu(cfg, 5, kernel="per_step", level0=level0)
+            np.testing.assert_array_equal(got, same.reshape(-1).astype(np.float64))
+
+
+def test_manufactured_solution_on_the_gpu(oracle):
+    """u = e^{-pi^2 t} sin(pi x) + x t^2 + (1-x) sin t on N = 127, r = 1, to t ~ 0.1: the GPU follows the
+    oracle to 1e-12 and the exact solution to the scheme's O(h^2) error."""
+    n, r = 127, 1.0
+    h = 1.0 / (n + 1)
+    x = np.arange(1, n + 1) * h
+    tau = r * h * h
+    steps = int(round(0.1 / tau)); steps += steps % 2
+    exact = lambda t: np.exp(-np.pi ** 2 * t) * np.sin(np.pi * x) + x * t * t + (1 - x) * np.sin(t)
+    f = lambda t: 2 * x * t + (1 - x) * np.cos(t)
+    cfg = dict(inputs.random_rods(1, n, "f64"), r=np.array([r]), u0=exact(0.0)[None, :].copy())
+    ts = [i * tau for i in range(steps + 1)]
+    srcs = [tau * f(t + tau / 2) for t in ts[:-1]]
+    bcs = [(np.sin(t), np.sin(t + tau), t * t, (t + tau) ** 2) for t in ts[:-1]]
+    got, ref = _march(oracle, cfg, steps, 0, srcs, bcs)
+    assert np.abs(got - ref).max() <= 1e-12
+    err = np.abs(got - exact(ts[-1])).max()
+    assert err < 3e-4, err
+
+
+def test_step_src_argument_errors():
+    import torch
+    from paper_1310_3422_b200 import libge
+    u = torch.zeros(256, dtype=torch.float64, device="cuda:0")
+    with libge.Plan(inputs.random_rods(2, 64, "f64")) as plan:            # batched rods: not supported
+        with pytest.raises(libge.GeError) as ei:
+            plan.step_src(u.data_ptr(), u.data_ptr() + 8 * 128, 0, (0, 0, 0, 0))
+        assert ei.value.status == libge.GE_EINVAL
+    with libge.Plan(inputs.random_rods(1, 64, "f64"), group_k=2) as plan:
+        with pytest.raises(libge.GeError) as ei:
+            plan.step_src(u.data_ptr(), u.data_ptr() + 8 * 64, 0, (0, 0, 0, 0))
+        assert ei.value.status == libge.GE_EUNSUPPORTED
+    with libge.Plan(inputs.random_rods(1, 64, "f64")) as plan:
+        with pytest.raises(libge.GeError):
+            plan.step_src(u.data_ptr(), u.data_ptr() + 8 * 64, 0, (0, float("nan"), 0, 0))
+        with pytest.raises(libge.GeError):
+            plan.step_src(u.data_ptr(), u.data_ptr(), 0, (0, 0, 0, 0))
