@@ -53,6 +53,10 @@ def _load():
         lib.ge_ref_level_2d.restype = None
         lib.ge_ref_run_2d.argtypes = [_f64p, _i64, _i64, _f64, _f64p, _i64, _i64]
         lib.ge_ref_run_2d.restype = ctypes.c_int
+        lib.ge_ref_level_3d.argtypes = [_f64p, _f64p, _i64, _i64, _i64, _f64, _i64]
+        lib.ge_ref_level_3d.restype = None
+        lib.ge_ref_run_3d.argtypes = [_f64p, _i64, _i64, _i64, _f64, _f64p, _i64, _i64]
+        lib.ge_ref_run_3d.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -139,3 +143,27 @@ def run_2d(u0, r, steps, bc=(0.0, 0.0, 0.0, 0.0), level0=0):
     if rc:
         raise MemoryError("ge_ref_run_2d")
     return u
+
+
+def run_3d(u0, r, steps, bc=(0.0,) * 6, level0=0):
+    """`steps` 3-D levels (reading R-3D); u0: [Nz][Ny][Nx] interior, bc = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi)."""
+    u = np.array(u0, dtype=np.float64, order="C", copy=True)
+    nz, ny, nx = u.shape
+    bcv = np.asarray(bc, dtype=np.float64).copy()
+    rc = _load().ge_ref_run_3d(u, nx, ny, nz, float(r), bcv, int(level0), int(steps))
+    if rc:
+        raise MemoryError("ge_ref_run_3d")
+    return u
+
+
+def level_3d(u, r, phase, bc=(0.0,) * 6):
+    return run_3d(u, r, 1, bc, level0=phase)
+
+
+def level_3d_padded(old, r, phase):
+    """One 3-D level on a padded array [Nz+2][Ny+2][Nx+2] whose faces hold arbitrary boundary data."""
+    old = np.ascontiguousarray(old, dtype=np.float64)
+    nz, ny, nx = (d - 2 for d in old.shape)
+    new = np.empty_like(old)
+    _load().ge_ref_level_3d(old, new, nx, ny, nz, float(r), int(phase))
+    return new

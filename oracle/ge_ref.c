@@ -300,3 +300,137 @@ int ge_ref_run_2d(double *u, int64_t Nx, int64_t Ny, double r, const double *bc,
     free(a); free(b);
     return 0;
 }
+
+/*
+ * One level in 3-D, 2x2x2 eight-point groups (reading R-3D; SURVEY.md
+ * 8(f) NEXT-4 -- the paper only claims "capacity of extension to higher order
+ * dimensions").  The construction is that of the 2-D
+ * reading: group anchors at (1+phase) mod 2 in every axis (shift (1,1,1)
+ * between levels), in-group links at the new level, out-of-group links at the
+ * old level; for an interior member P with its three in-group neighbours G and
+ * its three out-of-group neighbours O
+ *     (1+3r) new_P - r sum_G new_G = (1-3r) old_P + r sum_O old_O ,
+ * a boundary in-group neighbour contributing r*beta to the right side.  Groups
+ * cut by a face, an edge or a corner keep their interior members (4, 2, 1).
+ * The m x m system of a group (m <= 8) is solved by plain Gaussian elimination
+ * with partial pivoting -- no closed form is used here.
+ *
+ * Arrays: (Nz+2) x (Ny+2) x (Nx+2), x fastest; the six faces hold the boundary
+ * values (constant in time), edge and corner nodes of the box are never read.
+ */
+#define AT3(a, i, j, k) ((a)[((size_t)(k) * (size_t)sy + (size_t)(j)) * (size_t)sx + (size_t)(i)])
+
+static void solve_small(int m, double A[8][8], double *b)
+{
+    int c, rr, cc;
+    for (c = 0; c < m; ++c) {
+        int piv = c;
+        double best = A[c][c] < 0 ? -A[c][c] : A[c][c];
+        for (rr = c + 1; rr < m; ++rr) {
+            double v = A[rr][c] < 0 ? -A[rr][c] : A[rr][c];
+            if (v > best) { best = v; piv = rr; }
+        }
+        if (piv != c) {
+            double t;
+            for (cc = 0; cc < m; ++cc) { t = A[c][cc]; A[c][cc] = A[piv][cc]; A[piv][cc] = t; }
+            t = b[c]; b[c] = b[piv]; b[piv] = t;
+        }
+        for (rr = c + 1; rr < m; ++rr) {
+            const double f = A[rr][c] / A[c][c];
+            for (cc = c; cc < m; ++cc) A[rr][cc] -= f * A[c][cc];
+            b[rr] -= f * b[c];
+        }
+    }
+    for (c = m - 1; c >= 0; --c) {
+        double s = b[c];
+        for (cc = c + 1; cc < m; ++cc) s -= A[c][cc] * b[cc];
+        b[c] = s / A[c][c];
+    }
+}
+
+void ge_ref_level_3d(const double *old_, double *new_, int64_t Nx, int64_t Ny, int64_t Nz,
+                     double r, int64_t phase)
+{
+    const int64_t sx = Nx + 2, sy = Ny + 2;
+    const int64_t N[3] = {Nx, Ny, Nz};
+    int64_t g[3];
+    memcpy(new_, old_, (size_t)(Nx + 2) * (size_t)(Ny + 2) * (size_t)(Nz + 2) * sizeof(double));
+    for (g[2] = 1 - phase; g[2] <= Nz; g[2] += 2)
+        for (g[1] = 1 - phase; g[1] <= Ny; g[1] += 2)
+            for (g[0] = 1 - phase; g[0] <= Nx; g[0] += 2) {
+                int idx[8], m = 0, d, q, ax;
+                double A[8][8], b[8];
+                int64_t pos[8][3];
+                for (d = 0; d < 8; ++d) {                 /* member d: offsets (d&1, d>>1&1, d>>2&1) */
+                    int inside = 1;
+                    for (ax = 0; ax < 3; ++ax) {
+                        const int64_t p = g[ax] + ((d >> ax) & 1);
+                        if (p < 1 || p > N[ax]) inside = 0;
+                    }
+                    idx[d] = inside ? m : -1;
+                    if (inside) {
+                        for (ax = 0; ax < 3; ++ax) pos[m][ax] = g[ax] + ((d >> ax) & 1);
+                        ++m;
+                    }
+                }
+                if (m == 0) continue;
+                for (d = 0; d < 8; ++d) {
+                    int row;
+                    int64_t p[3];
+                    if (idx[d] < 0) continue;
+                    row = idx[d];
+                    for (ax = 0; ax < 3; ++ax) p[ax] = g[ax] + ((d >> ax) & 1);
+                    for (q = 0; q < m; ++q) A[row][q] = 0.0;
+                    A[row][row] = 1.0 + 3.0 * r;
+                    b[row] = (1.0 - 3.0 * r) * AT3(old_, p[0], p[1], p[2]);
+                    for (ax = 0; ax < 3; ++ax) {
+                        const int bit = (d >> ax) & 1;
+                        int64_t in[3] = {p[0], p[1], p[2]}, out[3] = {p[0], p[1], p[2]};
+                        const int partner = d ^ (1 << ax);
+                        in[ax] += bit ? -1 : 1;           /* in-group neighbour along this axis  */
+                        out[ax] += bit ? 1 : -1;          /* out-of-group neighbour              */
+                        b[row] += r * AT3(old_, out[0], out[1], out[2]);
+                        if (idx[partner] >= 0) A[row][idx[partner]] -= r;
+                        else b[row] += r * AT3(old_, in[0], in[1], in[2]);   /* boundary node: known */
+                    }
+                }
+                solve_small(m, A, b);
+                for (q = 0; q < m; ++q) AT3(new_, pos[q][0], pos[q][1], pos[q][2]) = b[q];
+            }
+}
+
+/*
+ * `steps` levels in 3-D.  u: Nz x Ny x Nx interior values, [k][j][i], overwritten
+ * by the final level.  bc = {x_lo, x_hi, y_lo, y_hi, z_lo, z_hi}.
+ */
+int ge_ref_run_3d(double *u, int64_t Nx, int64_t Ny, int64_t Nz, double r, const double *bc,
+                  int64_t level0, int64_t steps)
+{
+    const int64_t sx = Nx + 2, sy = Ny + 2;
+    const size_t tot = (size_t)(Nx + 2) * (size_t)(Ny + 2) * (size_t)(Nz + 2);
+    double *a = (double *)calloc(tot, sizeof(double));
+    double *b = (double *)calloc(tot, sizeof(double));
+    int64_t i, j, k, s;
+    if (!a || !b) { free(a); free(b); return -1; }
+    for (k = 0; k <= Nz + 1; ++k)
+        for (j = 0; j <= Ny + 1; ++j)
+            for (i = 0; i <= Nx + 1; ++i) {
+                double v = 0.0;
+                const int onx = (i == 0 || i == Nx + 1), ony = (j == 0 || j == Ny + 1), onz = (k == 0 || k == Nz + 1);
+                if (onx + ony + onz == 0) v = u[((size_t)(k - 1) * (size_t)Ny + (size_t)(j - 1)) * (size_t)Nx + (size_t)(i - 1)];
+                else if (onx + ony + onz == 1)
+                    v = onx ? bc[i == 0 ? 0 : 1] : (ony ? bc[j == 0 ? 2 : 3] : bc[k == 0 ? 4 : 5]);
+                AT3(a, i, j, k) = v;
+            }
+    for (s = 0; s < steps; ++s) {
+        double *t;
+        ge_ref_level_3d(a, b, Nx, Ny, Nz, r, pmod(level0 + s, 2));
+        t = a; a = b; b = t;
+    }
+    for (k = 1; k <= Nz; ++k)
+        for (j = 1; j <= Ny; ++j)
+            memcpy(u + ((size_t)(k - 1) * (size_t)Ny + (size_t)(j - 1)) * (size_t)Nx, &AT3(a, 1, j, k),
+                   (size_t)Nx * sizeof(double));
+    free(a); free(b);
+    return 0;
+}

@@ -177,3 +177,59 @@ def level_2d_dense(u, r, phase, bc=(0.0, 0.0, 0.0, 0.0)):
 def operator_2d(nx, ny, r, phase):
     A, B, _ = system_2d(nx, ny, float(r), phase, (0.0, 0.0, 0.0, 0.0))
     return np.linalg.solve(np.array(A), np.array(B))
+
+
+def system_3d(nx, ny, nz, r, phase, bc, num=float):
+    """3-D (reading R-3D): in-group neighbours at the new level, out-of-group at the old level.
+    Unknown index ((k-1)*ny + (j-1))*nx + (i-1); bc = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi)."""
+    zero, one = num(0), num(1)
+    n = nx * ny * nz
+    A = [[zero] * n for _ in range(n)]
+    B = [[zero] * n for _ in range(n)]
+    c = [zero] * n
+    dims = (nx, ny, nz)
+
+    def gid(p):
+        return tuple(((q - 1) // 2 if phase == 0 else q // 2) for q in p)
+
+    def bvalue(p):
+        for ax in range(3):
+            if p[ax] == 0:
+                return num(bc[2 * ax])
+            if p[ax] == dims[ax] + 1:
+                return num(bc[2 * ax + 1])
+        return None
+
+    def index(p):
+        return ((p[2] - 1) * ny + (p[1] - 1)) * nx + (p[0] - 1)
+
+    for k in range(1, nz + 1):
+        for j in range(1, ny + 1):
+            for i in range(1, nx + 1):
+                p = (i, j, k)
+                row = index(p)
+                A[row][row] = one + 3 * r
+                B[row][row] = one - 3 * r
+                for ax in range(3):
+                    for d in (-1, 1):
+                        q = list(p); q[ax] += d; q = tuple(q)
+                        bv = bvalue(q)
+                        if bv is not None:
+                            c[row] += r * bv
+                        elif gid(q) == gid(p):
+                            A[row][index(q)] -= r
+                        else:
+                            B[row][index(q)] += r
+    return A, B, c
+
+
+def level_3d_dense(u, r, phase, bc=(0.0,) * 6):
+    u = np.asarray(u, dtype=np.float64)
+    nz, ny, nx = u.shape
+    A, B, c = system_3d(nx, ny, nz, float(r), phase, bc)
+    return np.linalg.solve(np.array(A), np.array(B) @ u.ravel() + np.array(c)).reshape(nz, ny, nx)
+
+
+def operator_3d(nx, ny, nz, r, phase):
+    A, B, _ = system_3d(nx, ny, nz, float(r), phase, (0.0,) * 6)
+    return np.linalg.solve(np.array(A), np.array(B))

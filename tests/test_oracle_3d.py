@@ -1,0 +1,90 @@
+"""Pins for the 3-D oracle (oracle/ge_ref.c ge_ref_level_3d; reading R-3D, SURVEY.md 8(f)
+NEXT-4) -- CPU only.  PAPER.md defines no 3-D scheme (PAPER.md:134, :228 only claim the extension), so
+the reading is pinned by mathematics: invariants, dense brute force from the implicit statement,
+exact rationals, spectral radius of the two-level cycle, convergence to the closed form."""
+from fractions import Fraction as F
+
+import numpy as np
+import pytest
+
+import dense_ref as D
+
+
+@pytest.mark.parametrize("phase", [0, 1])
+@pytest.mark.parametrize("shape", [(1, 1, 1), (2, 2, 2), (3, 2, 4), (4, 4, 4), (5, 3, 2)])
+def test_constants_and_linear_data_are_fixed_points(oracle, phase, shape):
+    nz, ny, nx = shape
+    for r in (0.5, 2.0, 9.0):
+        c = np.full(shape, 1.75)
+        np.testing.assert_allclose(oracle.level_3d(c, r, phase, (1.75,) * 6), c, rtol=1e-14)
+        k, j, i = np.meshgrid(np.arange(nz + 2), np.arange(ny + 2), np.arange(nx + 2), indexing="ij")
+        lin = 0.5 - 0.125 * i + 0.25 * j + 0.0625 * k        # second differences vanish in every axis
+        new = oracle.level_3d_padded(lin, r, phase)
+        np.testing.assert_allclose(new[1:-1, 1:-1, 1:-1], lin[1:-1, 1:-1, 1:-1], rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("phase", [0, 1])
+@pytest.mark.parametrize("shape", [(1, 1, 1), (2, 2, 2), (2, 3, 1), (3, 3, 3), (4, 4, 4), (4, 2, 5), (3, 5, 4)])
+def test_brute_force_from_the_implicit_statement(oracle, phase, shape):
+    """Global dense A^-1 (B old + c), assembled node by node; the oracle solves group by group."""
+    rng = np.random.default_rng(sum(shape) + phase)
+    for r in (0.5, 1.0, 4.0, 30.0):
+        u = rng.uniform(-1, 1, shape)
+        bc = tuple(rng.uniform(-1, 1, 6))
+        got = oracle.level_3d(u, r, phase, bc)
+        ref = D.level_3d_dense(u, r, phase, bc)
+        np.testing.assert_allclose(got, ref, rtol=0, atol=3e-13 * max(1.0, r))
+
+
+def test_exact_rational_full_group():
+    """N = 2, phase 0: one full 2x2x2 group, zero boundary values, r = 1: (1+3r) I - r Q3 solved in
+    exact rationals; by symmetry u0 = 1 everywhere gives R = 1 - 3r = -2 and new = -2 / (1+3r-3r) = -2."""
+    A, B, c = D.system_3d(2, 2, 2, F(1), 0, (0,) * 6, num=F)
+    rhs = [sum(B[i][j] for j in range(8)) + c[i] for i in range(8)]
+    sol = D.solve_exact(A, rhs)
+    assert all(v == F(-2) for v in sol)
+    # a single hot corner: eigen-decomposition of the cube graph gives the exact weights
+    rhs = [B[i][0] for i in range(8)]
+    sol = D.solve_exact(A, rhs)
+    lam = {0: F(1), 1: F(3), 2: F(5), 3: F(7)}           # 1 + 3r - r*(3 - 2*popcount) at r = 1
+    for d in range(8):
+        w = sum(F((-1) ** bin(d & m).count("1")) / lam[bin(m).count("1")] for m in range(8)) / 8
+        assert sol[d] == (1 - 3) * w                      # B[0][0] = 1 - 3r = -2
+
+
+def test_exact_rational_matches_oracle(oracle):
+    u = np.arange(1, 9, dtype=np.float64).reshape(2, 2, 2)
+    A, B, c = D.system_3d(2, 2, 2, F(2), 0, (1, 0, 0, 3, 0, 0), num=F)
+    flat = [F(int(v)) for v in u.ravel()]
+    rhs = [sum(B[i][j] * flat[j] for j in range(8)) + c[i] for i in range(8)]
+    sol = np.array([float(v) for v in D.solve_exact(A, rhs)]).reshape(2, 2, 2)
+    np.testing.assert_allclose(oracle.level_3d(u, 2.0, 0, (1, 0, 0, 3, 0, 0)), sol, rtol=0, atol=1e-13)
+    # phase 1 on N = 2: eight single-member corner groups
+    A, B, c = D.system_3d(2, 2, 2, F(2), 1, (1, 0, 0, 3, 0, 0), num=F)
+    rhs = [sum(B[i][j] * flat[j] for j in range(8)) + c[i] for i in range(8)]
+    sol = np.array([float(v) for v in D.solve_exact(A, rhs)]).reshape(2, 2, 2)
+    np.testing.assert_allclose(oracle.level_3d(u, 2.0, 1, (1, 0, 0, 3, 0, 0)), sol, rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("n", [3, 4])
+def test_two_level_cycle_is_unconditionally_stable(n):
+    for r in (0.5, 1.0, 2.0, 10.0, 100.0):
+        T0, T1 = D.operator_3d(n, n, n, r, 0), D.operator_3d(n, n, n, r, 1)
+        rho = max(abs(np.linalg.eigvals(T1 @ T0)))
+        assert rho <= 1.0 + 1e-10, (n, r, rho)
+    # a single level is NOT stable beyond r ~ 1: nobody should "fix" the alternation
+    assert max(abs(np.linalg.eigvals(D.operator_3d(4, 4, 4, 4.0, 0)))) > 1.0
+
+
+def test_convergence_to_the_closed_form(oracle):
+    """u = e^{-3 pi^2 t} sin(pi x) sin(pi y) sin(pi z), zero boundary values, r = 1, t ~ 0.03."""
+    errs = []
+    for n in (7, 15, 31):
+        h = 1.0 / (n + 1)
+        x = np.arange(1, n + 1) * h
+        u0 = np.sin(np.pi * x)[None, None, :] * np.sin(np.pi * x)[None, :, None] * np.sin(np.pi * x)[:, None, None]
+        steps = int(round(0.03 / (h * h))); steps += steps % 2
+        t = steps * h * h
+        u = oracle.run_3d(u0, 1.0, steps)
+        errs.append(float(np.abs(u - np.exp(-3 * np.pi ** 2 * t) * u0).max()))
+    assert errs[0] / errs[1] > 3.0 and errs[1] / errs[2] > 3.3, errs
