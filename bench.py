@@ -52,17 +52,22 @@ def make_cfg(name, scale=1.0):
     if name in ("c5_f32", "c5_f64"):
         n = int(8192 * scale ** 0.5)
         return inputs.make_c5(n=n - n % 2, dtype=name[3:])
+    if name in ("box_f32", "box_f64"):        # 3-D (NEXT-4), not a BASELINE.json config
+        n = int(512 * scale ** (1.0 / 3.0))
+        return inputs.make_box(n=n - n % 2, dtype=name[4:])
     raise SystemExit("unknown --config %s" % name)
 
 
 def units(cfg, levels=None):
     """grid-point updates of one step"""
     lv = cfg["steps"] if levels is None else levels
-    return cfg["nx"] * cfg["ny"] * cfg["batch"] * lv
+    return cfg["nx"] * cfg["ny"] * cfg.get("nz", 1) * cfg["batch"] * lv
 
 
 def workload_desc(cfg):
-    if cfg["dim"] == 2:
+    if cfg["dim"] == 3:
+        shape = "%dx%dx%d" % (cfg["nz"], cfg["ny"], cfg["nx"])
+    elif cfg["dim"] == 2:
         shape = "%dx%d" % (cfg["ny"], cfg["nx"])
     elif cfg["batch"] > 1:
         shape = "%d rods x %d" % (cfg["batch"], cfg["nx"])
@@ -78,7 +83,9 @@ def oracle_time(cfg):
     from oracle import ge_oracle          # allowed here only: cpu_baseline / --impl reference legs
     u0 = cfg["u0"].astype(np.float64)
     t0 = time.perf_counter()
-    if cfg["dim"] == 2:
+    if cfg["dim"] == 3:
+        ge_oracle.run_3d(u0, cfg["r"][0], cfg["steps"])
+    elif cfg["dim"] == 2:
         ge_oracle.run_2d(u0, cfg["r"][0], cfg["steps"],
                          (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1]))
     elif cfg["batch"] == 1:
@@ -127,7 +134,9 @@ def make_cfg_meta(name):
             "c3": "c3: 1-D GE, 4096 rods x 4096 interior, f32, 2000 levels per step",
             "c4": "c4: 1-D GE, N=268435456 interior, f64, 200 levels per step",
             "c5_f32": "c5_f32: 2-D GE, 8192x8192 interior, f32, 1000 levels per step",
-            "c5_f64": "c5_f64: 2-D GE, 8192x8192 interior, f64, 1000 levels per step"}
+            "c5_f64": "c5_f64: 2-D GE, 8192x8192 interior, f64, 1000 levels per step",
+            "box_f32": "box_f32: 3-D GE, 512x512x512 interior, f32, 100 levels per step",
+            "box_f64": "box_f64: 3-D GE, 512x512x512 interior, f64, 100 levels per step"}
     return meta[name]
 
 
@@ -233,7 +242,7 @@ def run_ours(args):
         cfg["steps"] = args.levels
     levels = cfg["steps"]
     es = ESIZE[cfg["dtype"]]
-    nelem = cfg["nx"] * cfg["ny"] * cfg["batch"]
+    nelem = cfg["nx"] * cfg["ny"] * cfg.get("nz", 1) * cfg["batch"]
     stream_obj = torch.cuda.current_stream(dev)
     stream = stream_obj.cuda_stream
 
@@ -447,7 +456,7 @@ def roofline(cfg, info, total_ms, launches, steps):
     rate.  Temporally blocked and resident kernels: bound by the plain fp32/fp64 pipes, achieved =
     flops of the factored form per second against 2 x lanes x SMs x max clock."""
     es = ESIZE[cfg["dtype"]]
-    nelem = cfg["nx"] * cfg["ny"] * cfg["batch"]
+    nelem = cfg["nx"] * cfg["ny"] * cfg.get("nz", 1) * cfg["batch"]
     peaks, src = measured_peaks()
     kernel = info["kernel"]
     ms = total_ms / max(launches, 1)

@@ -20,6 +20,8 @@
  *     c = (i - phase*k) mod 2k: c = 2k-1 / 0 are the left / right member of a pair (Eqs (3),(4)),
  *     c = 1..k-1 follow by Saul'yev's Eq (1) in ascending order, c = k..2k-2 by Eq (2) in
  *     descending order; sweeps that reach a boundary read it.
+ *   - 3-D (reading R-3D, same construction as 2-D): 2x2x2 eight-point groups anchored at
+ *     (1+phase) mod 2 in every axis, 8x8 block solved in closed form (Walsh modes of the cube).
  *   - 2-D (reading R-2D; the paper only claims the extension,
  *     PAPER.md:134, :228): 2x2 four-point groups anchored at (1+phase, 1+phase)
  *     (mod 2) -- diagonal shift --, in-group links implicit, out-of-group links
@@ -70,7 +72,7 @@ typedef enum {
 } ge_status;
 
 typedef struct {
-    int32_t   dim;        /* 1 or 2                                                                    */
+    int32_t   dim;        /* 1, 2 or 3 (3: 2x2x2 groups, strategy A only)       */
     int64_t   nx, ny;     /* interior nodes per axis, >= 1 (ny must be 1 when dim == 1)                */
     int64_t   batch;      /* independent 1-D rods, >= 1 (must be 1 when dim == 2)                      */
     int32_t   dtype;      /* ge_dtype: arithmetic and storage type of u                                */
@@ -78,12 +80,13 @@ typedef struct {
                              length k (1-D only; the paper's runs use 16): confluence pairs every 2k nodes
                              joined by Saul'yev sweeps; always strategy A (one launch per level)       */
     const double *r;      /* HOST array, `batch` entries (dim 2: 1 entry), finite, > 0; copied         */
-    const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; copied  */
-    const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; copied  */
+    const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; 3-D {x_lo, y_lo, z_lo} */
+    const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; 3-D {x_hi, y_hi, z_hi} */
     int32_t   kernel;     /* ge_kernel                                                                 */
     int32_t   tb;         /* levels per launch for TEMPORAL (0 = auto; any value >= 1, both starting
                              phases are handled in-kernel); levels between two meetings of the tiles for
                              PERSISTENT on one long rod (0 = the largest the halo allows)              */
+    int64_t   nz;         /* interior nodes along z (dim == 3; must be 0 or 1 otherwise); layout [nz][ny][nx] */
 } ge_desc;
 
 /* Create a plan: validates desc, uploads per-rod coefficients (r, r/(1+2r), r/(1+r), ... computed in
@@ -98,6 +101,7 @@ int ge_plan_create(ge_plan **out, const ge_desc *desc, ge_stream_t stream);
  * GE_EINVAL if the plan's dim does not match or a pointer is null/misaligned for dtype. */
 int ge_step_1d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 int ge_step_2d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
+int ge_step_3d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 
 /* One level of a single rod (batch == 1, group_k == 1) with NON-CONSTANT problem data (SURVEY.md 8(f)
  * NEXT-3, reading R-N3; the paper's model problem has neither):

@@ -20,6 +20,7 @@
 #include "ge_strip2d.cuh"
 #include "ge_level_k.cuh"
 #include "ge_level_src.cuh"
+#include "ge_level3d.cuh"
 
 namespace {
 
@@ -44,7 +45,7 @@ struct ge_plan {
     int32_t tc;               // values per lane of the temporal kernel (18 f64 / 36 f32: the TMA-staged one)
     int32_t stream_ctas;      // persistent grid of the TMA-staged kernel (0: not queried yet)
     int32_t hp;               // 2-D temporal kernel: output row pairs per segment
-    int64_t nx, ny, batch;
+    int64_t nx, ny, nz, batch;
     int64_t count;            // elements of the state
     int64_t level;
     int64_t launches;
@@ -86,6 +87,18 @@ int upload_coef(ge_plan* p, const ge_desc* d, cudaStream_t s) {
         GE_CUDA(cudaMalloc(&p->coef, h.size() * sizeof(ge::Coef1<T>)));
         GE_CUDA(cudaMemcpyAsync(p->coef, h.data(), h.size() * sizeof(ge::Coef1<T>), cudaMemcpyHostToDevice, s));
         GE_CUDA(cudaStreamSynchronize(s));   // h is a stack-owned staging buffer
+    } else if (p->dim == 3) {
+        ge::Coef3<T> h;
+        std::memset(&h, 0, sizeof(h));
+        const double r = d->r[0];
+        h.r = (T)r;
+        h.c1 = (T)(2.0 * r / (1.0 + 2.0 * r) / 8.0);
+        h.c2 = (T)(4.0 * r / (1.0 + 4.0 * r) / 8.0);
+        h.c3 = (T)(6.0 * r / (1.0 + 6.0 * r) / 8.0);
+        for (int ax = 0; ax < 3; ++ax) { h.lo[ax] = (T)d->bc_lo[ax]; h.hi[ax] = (T)d->bc_hi[ax]; }
+        GE_CUDA(cudaMalloc(&p->coef, sizeof(h)));
+        GE_CUDA(cudaMemcpyAsync(p->coef, &h, sizeof(h), cudaMemcpyHostToDevice, s));
+        GE_CUDA(cudaStreamSynchronize(s));
     } else {
         ge::Coef2<T> h;
         std::memset(&h, 0, sizeof(h));
@@ -182,6 +195,14 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     if (p->dim == 1 && p->group_k >= 2)
         rc = p->dtype == GE_F64 ? launch_level_k<double>(p, uin, uout, phase, s)
                                 : launch_level_k<float>(p, uin, uout, phase, s);
+    else if (p->dim == 3) {
+        cudaError_t e = p->dtype == GE_F64
+            ? ge::level3d_launch<double>((const double*)uin, (double*)uout, p->nx, p->ny, p->nz, (const ge::Coef3<double>*)p->coef, phase, s)
+            : ge::level3d_launch<float>((const float*)uin, (float*)uout, p->nx, p->ny, p->nz, (const ge::Coef3<float>*)p->coef, phase, s);
+        if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+        p->launches += 1;
+        rc = GE_OK;
+    }
     else if (p->dim == 1) rc = p->dtype == GE_F64 ? launch_level_1d<double>(p, uin, uout, phase, s)
                                              : launch_level_1d<float>(p, uin, uout, phase, s);
     else             rc = p->dtype == GE_F64 ? launch_level_2d<double>(p, uin, uout, phase, s)
@@ -508,20 +529,22 @@ const char* ge_strerror(int status) {
 
 int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (!out || !d) return GE_EINVAL;
-    if (d->dim != 1 && d->dim != 2) return GE_EINVAL;
+    if (d->dim != 1 && d->dim != 2 && d->dim != 3) return GE_EINVAL;
     if (d->nx < 1 || d->ny < 1 || d->batch < 1) return GE_EINVAL;
+    if (d->dim == 3 && (d->nz < 1 || d->batch != 1 || d->nx >= (1 << 30) || d->ny >= (1 << 30) || d->nz >= (1 << 30))) return GE_EINVAL;
+    if (d->dim != 3 && d->nz > 1) return GE_EINVAL;
     if (d->dim == 1 && d->ny != 1) return GE_EINVAL;
     if (d->dim == 2 && d->batch != 1) return GE_EINVAL;
     if (d->dtype != GE_F32 && d->dtype != GE_F64) return GE_EINVAL;
     if (d->group_k < 1) return GE_EINVAL;
-    if (d->group_k >= 2 && d->dim == 2) return GE_EINVAL;
+    if (d->group_k >= 2 && d->dim >= 2) return GE_EINVAL;
     if (d->kernel < GE_KERNEL_AUTO || d->kernel > GE_KERNEL_PERSISTENT) return GE_EINVAL;
     if (d->tb < 0) return GE_EINVAL;
     if (!d->r || !d->bc_lo || !d->bc_hi) return GE_EINVAL;
     const int64_t nr = d->dim == 1 ? d->batch : 1;
     for (int64_t b = 0; b < nr; ++b)
         if (!(d->r[b] > 0.0) || !std::isfinite(d->r[b])) return GE_EINVAL;
-    const int64_t nb = d->dim == 1 ? d->batch : 2;
+    const int64_t nb = d->dim == 1 ? d->batch : d->dim;
     for (int64_t b = 0; b < nb; ++b)
         if (!std::isfinite(d->bc_lo[b]) || !std::isfinite(d->bc_hi[b])) return GE_EINVAL;
     if (d->group_k > kMaxGroupK) return GE_EUNSUPPORTED;
@@ -530,8 +553,8 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (!p) return GE_ENOMEM;
     std::memset(p, 0, sizeof(*p));
     p->dim = d->dim; p->dtype = d->dtype; p->group_k = d->group_k;
-    p->nx = d->nx; p->ny = d->ny; p->batch = d->batch;
-    p->count = d->dim == 1 ? d->batch * d->nx : d->ny * d->nx;
+    p->nx = d->nx; p->ny = d->ny; p->nz = d->dim == 3 ? d->nz : 1; p->batch = d->batch;
+    p->count = d->dim == 1 ? d->batch * d->nx : d->ny * d->nx * p->nz;
     p->last_stream = (cudaStream_t)stream;
     int rc = GE_OK;
     cudaError_t ce = cudaGetDevice(&p->device);
@@ -554,6 +577,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
     if (d->group_k >= 2) kernel = GE_KERNEL_PER_STEP;      // k >= 2: strategy A only (ge_level_k.cuh)
+    if (d->dim == 3) kernel = GE_KERNEL_PER_STEP;          // 3-D: strategy A only (ge_level3d.cuh)
     if (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT) {
         p->res_tb = d->tb;
         rc = resident_configure(p, 0);
@@ -608,6 +632,10 @@ int ge_step_1d_src(ge_plan* p, const void* u_in, void* u_out, const void* tau_f,
 
 int ge_step_2d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
     return step_common(p, 2, u_in, u_out, (cudaStream_t)stream);
+}
+
+int ge_step_3d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
+    return step_common(p, 3, u_in, u_out, (cudaStream_t)stream);
 }
 
 int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {

@@ -102,3 +102,26 @@ def random_grid(nx, ny, dtype="f64", seed=4321, r=2.0):
     u0 = rng.uniform(-1.0, 1.0, size=(ny, nx)).astype(t)
     b = rng.uniform(-1.0, 1.0, size=4).astype(t).astype(np.float64)
     return _cfg("grid", 2, nx, ny, 1, dtype, 0, [r], [b[0], b[2]], [b[1], b[3]], u0)
+
+
+def random_box(nx, ny, nz, dtype="f64", seed=999, r=2.0):
+    """Generic seeded 3-D case with six different face values; u0 is [nz][ny][nx]."""
+    rng = np.random.default_rng(seed)
+    t = _DT[dtype]
+    u0 = rng.uniform(-1.0, 1.0, size=(nz, ny, nx)).astype(t)
+    b = rng.uniform(-1.0, 1.0, size=6).astype(t).astype(np.float64)
+    cfg = _cfg("box", 3, nx, ny, 1, dtype, 0, [r], [b[0], b[2], b[4]], [b[1], b[3], b[5]], u0)
+    cfg["nz"] = int(nz)
+    return cfg
+
+
+def make_box(n=512, steps=100, r=2.0, dtype="f32", seed=4):
+    """3-D measurement workload (not a BASELINE.json config): n^3 interior, u0 = sin(pi x) sin(pi y)
+    sin(pi z) + 0.01 N(0,1) from `seed`, zero boundary values."""
+    rng = np.random.default_rng(seed)
+    x = np.sin(np.pi * _x(n))
+    u0 = x[None, None, :] * x[None, :, None] * x[:, None, None]
+    u0 = u0 + 0.01 * rng.standard_normal((n, n, n))
+    cfg = _cfg("box", 3, n, n, 1, dtype, steps, [r], [0.0, 0.0, 0.0], [0.0, 0.0, 0.0], u0)
+    cfg["nz"] = int(n)
+    return cfg

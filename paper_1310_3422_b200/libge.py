@@ -33,7 +33,7 @@ _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
 _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 
 # every symbol include/ge.h declares
-EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_step_2d", "ge_run", "ge_run_host",
+EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
            "ge_strerror", "ge_version")
 
@@ -50,6 +50,7 @@ class ge_desc(ctypes.Structure):
         ("bc_hi", ctypes.POINTER(ctypes.c_double)),
         ("kernel", ctypes.c_int32),
         ("tb", ctypes.c_int32),
+        ("nz", ctypes.c_int64),
     ]
 
 
@@ -76,6 +77,7 @@ def load() -> ctypes.CDLL:
     lib.ge_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ge_desc), vp]
     lib.ge_step_1d.argtypes = [vp, vp, vp, vp]
     lib.ge_step_2d.argtypes = [vp, vp, vp, vp]
+    lib.ge_step_3d.argtypes = [vp, vp, vp, vp]
     lib.ge_step_1d_src.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run.argtypes = [vp, vp, i64, vp]
     lib.ge_run_host.argtypes = [vp, vp, i64, vp]
@@ -109,18 +111,18 @@ def _darr(values: Sequence[float]):
 
 def ge_plan_create(dim: int, nx: int, ny: int = 1, batch: int = 1, dtype="f64", r=(1.0,),
                    bc_lo=(0.0,), bc_hi=(0.0,), group_k: int = 1, kernel="auto", tb: int = 0,
-                   stream: int = 0) -> int:
+                   stream: int = 0, nz: int = 1) -> int:
     """Returns the opaque plan handle (an integer address)."""
     lib = load()
     ra, lo, hi = _darr(r), _darr(bc_lo), _darr(bc_hi)
     need = batch if dim == 1 else 1
-    needb = batch if dim == 1 else 2
+    needb = batch if dim == 1 else dim
     if len(ra) < need or len(lo) < needb or len(hi) < needb:
         raise GeError(GE_EINVAL, "ge_plan_create (host arrays too short)")
     d = ge_desc(dim=dim, nx=nx, ny=ny, batch=batch,
                 dtype=_DTYPES[dtype] if isinstance(dtype, str) else int(dtype),
                 group_k=group_k, r=ra, bc_lo=lo, bc_hi=hi,
-                kernel=_KERNEL_IDS[kernel] if isinstance(kernel, str) else int(kernel), tb=tb)
+                kernel=_KERNEL_IDS[kernel] if isinstance(kernel, str) else int(kernel), tb=tb, nz=nz)
     out = ctypes.c_void_p()
     rc = lib.ge_plan_create(ctypes.byref(out), ctypes.byref(d), ctypes.c_void_p(stream))
     if rc != GE_OK:
@@ -147,6 +149,10 @@ def ge_step_1d_src(plan: int, u_in: int, u_out: int, tau_f: int, bc4: Sequence[f
 
 def ge_step_2d(plan: int, u_in: int, u_out: int, stream: int = 0):
     _check(load().ge_step_2d(plan, u_in, u_out, stream), "ge_step_2d")
+
+
+def ge_step_3d(plan: int, u_in: int, u_out: int, stream: int = 0):
+    _check(load().ge_step_3d(plan, u_in, u_out, stream), "ge_step_3d")
 
 
 def ge_run(plan: int, u: int, steps: int, stream: int = 0):
@@ -189,7 +195,7 @@ class Plan:
         self.cfg = cfg
         self.handle = ge_plan_create(cfg["dim"], cfg["nx"], cfg["ny"], cfg["batch"], cfg["dtype"],
                                      list(cfg["r"]), list(cfg["bc_lo"]), list(cfg["bc_hi"]),
-                                     group_k=group_k, kernel=kernel, tb=tb, stream=stream)
+                                     group_k=group_k, kernel=kernel, tb=tb, stream=stream, nz=cfg.get("nz", 1))
 
     def __enter__(self):
         return self
@@ -203,7 +209,7 @@ class Plan:
             self.handle = None
 
     def step(self, u_in: int, u_out: int, stream: int = 0):
-        (ge_step_1d if self.cfg["dim"] == 1 else ge_step_2d)(self.handle, u_in, u_out, stream)
+        {1: ge_step_1d, 2: ge_step_2d, 3: ge_step_3d}[self.cfg["dim"]](self.handle, u_in, u_out, stream)
 
     def step_src(self, u_in: int, u_out: int, tau_f: int, bc4, stream: int = 0):
         ge_step_1d_src(self.handle, u_in, u_out, tau_f, bc4, stream)

@@ -54,6 +54,9 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc
 
 def run_oracle(oracle, cfg, steps, level0=0, k=1):
     u0 = cfg["u0"].astype(np.float64)
+    if cfg["dim"] == 3:
+        bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1], cfg["bc_lo"][2], cfg["bc_hi"][2])
+        return oracle.run_3d(u0, cfg["r"][0], steps, bc, level0=level0)
     if cfg["dim"] == 2:
         bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1])
         return oracle.run_2d(u0, cfg["r"][0], steps, bc, level0=level0)

@@ -42,7 +42,7 @@ def test_version_and_strerror(lib):
 def test_validation_needs_no_gpu(lib):
     from paper_1310_3422_b200 import libge
     # argument errors are reported before any CUDA call
-    for kw in (dict(dim=3, nx=8), dict(dim=1, nx=0), dict(dim=1, nx=8, r=(-1.0,)),
+    for kw in (dict(dim=4, nx=8), dict(dim=3, nx=8, ny=8, nz=0, bc_lo=(0, 0, 0), bc_hi=(0, 0, 0)), dict(dim=2, nx=8, ny=8, nz=4, bc_lo=(0, 0), bc_hi=(0, 0)), dict(dim=1, nx=0), dict(dim=1, nx=8, r=(-1.0,)),
                dict(dim=1, nx=8, r=(float("nan"),)), dict(dim=2, nx=8, ny=8, batch=2, bc_lo=(0, 0), bc_hi=(0, 0)),
                dict(dim=1, nx=8, ny=2), dict(dim=1, nx=8, group_k=0), dict(dim=1, nx=8, tb=-1),
                dict(dim=2, nx=8, ny=8, group_k=2, bc_lo=(0, 0), bc_hi=(0, 0))):
@@ -62,7 +62,8 @@ def test_desc_struct_layout_matches_header():
     assert libge.ge_desc.nx.offset == 8 and libge.ge_desc.batch.offset == 24
     assert libge.ge_desc.dtype.offset == 32 and libge.ge_desc.group_k.offset == 36
     assert libge.ge_desc.r.offset == 40 and libge.ge_desc.kernel.offset == 64
-    assert ctypes.sizeof(libge.ge_desc) == 72
+    assert libge.ge_desc.nz.offset == 72
+    assert ctypes.sizeof(libge.ge_desc) == 80
 
 
 def test_product_does_not_import_oracle():
