@@ -67,6 +67,8 @@ struct ge_plan {
     unsigned* res_flags;      // device: one flag per tile, + the fault word at [res_tiles]
     unsigned res_epoch;       // value every flag holds between launches
     int64_t meetings;         // meetings of the persistent kernel so far (info)
+    int32_t strip_attr_tb;    // block length whose strip-kernel function attributes are set on this device (0: none)
+    bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
 };
 
 namespace {
@@ -175,11 +177,10 @@ int launch_level_k(ge_plan* p, const void* uin, void* uout, int phase, cudaStrea
     const ge::LevelKGeom g = ge::level_k_geom(p->group_k, phase, p->nx, sizeof(T), kLevelKSmemBudget);
     if (g.upc < 1) return GE_EUNSUPPORTED;
     const size_t smem = ge::level_k_smem(g, sizeof(T));
-    static bool configured = false;
-    if (!configured) {
+    if (!p->levelk_attr) {
         GE_CUDA(cudaFuncSetAttribute(ge::ge1d_level_k_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)(kLevelKSmemBudget + 64)));
-        configured = true;
+        p->levelk_attr = true;
     }
     dim3 grid((unsigned)((g.units + g.upc - 1) / g.upc), (unsigned)(p->batch < 65535 ? p->batch : 65535));
     ge::ge1d_level_k_kernel<T><<<grid, ge::kLevelKThreads, smem, s>>>((const T*)uin, (T*)uout, p->nx, p->batch,
@@ -304,12 +305,14 @@ int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
     auto* out = (T*)uout;
     auto* c = (const ge::Coef2<T>*)p->coef;
     cudaError_t e;
+    bool configured = p->strip_attr_tb == p->tb;
     switch (p->tb) {
-        case 4: e = ge::strip2d_launch<T, StripC<T>::c, 4>(in, out, p->nx, p->ny, c, p->hp, s); break;
-        case 6: e = ge::strip2d_launch<T, StripC<T>::c, 6>(in, out, p->nx, p->ny, c, p->hp, s); break;
-        case 8: e = ge::strip2d_launch<T, StripC<T>::c, 8>(in, out, p->nx, p->ny, c, p->hp, s); break;
+        case 4: e = ge::strip2d_launch<T, StripC<T>::c, 4>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
+        case 6: e = ge::strip2d_launch<T, StripC<T>::c, 6>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
+        case 8: e = ge::strip2d_launch<T, StripC<T>::c, 8>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
         default: return GE_EINVAL;
     }
+    if (configured) p->strip_attr_tb = p->tb;
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     p->launches += 1;
     p->level += p->tb;

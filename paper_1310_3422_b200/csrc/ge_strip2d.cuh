@@ -442,15 +442,16 @@ ge2d_strip_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
     else               strip_run<T, C, TB, false>(uin, uout, nx, ny, coef, sp, a0, out_lo, out_hi, false, false, ys, ye, lane);
 }
 
-// Host launcher: TB levels starting at a PHASE-1 level.  Requires nx % V == 0, nx even, nx >= 32*C,
+// Host launcher: TB levels starting at a PHASE-1 level; `configured` is the caller's per-plan flag for
+// this instantiation's function attributes.  Requires nx % V == 0, nx even, nx >= 32*C,
 // 16-byte aligned buffers and nx, ny < 2^30.
 template <typename T, int C, int TB>
 inline cudaError_t strip2d_launch(const T* uin, T* uout, int64_t nx, int64_t ny, const Coef2<T>* coef, int hp,
-                                  cudaStream_t s) {
+                                  bool& configured, cudaStream_t s) {
     const Strip2dGeom g = strip2d_geom(C, VecOf<T>::V, TB, nx, ny, hp);
     dim3 grid((unsigned)((g.nstrips + kStripWarps - 1) / kStripWarps), (unsigned)g.segs);
     constexpr size_t smem = (size_t)kStripWarps * (TB + kStripRing) * 2 * 32 * C * sizeof(T);
-    static bool configured = false;               // per instantiation: allow > 48 KB and the full carve-out
+    // once per plan (= per device) and instantiation: allow > 48 KB and the full carve-out
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(ge2d_strip_kernel<T, C, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(ge2d_strip_kernel<T, C, TB>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
