@@ -78,14 +78,10 @@ __device__ __forceinline__ void truncated_group3d(const T (&R)[8], const bool (&
     for (int d = 0; d < 8; ++d) nw[d] = idx[d] >= 0 ? b[idx[d]] : T(0);
 }
 
-template <typename T, int PH>
-__global__ void __launch_bounds__(kLevel3dBx * kLevel3dBy * kLevel3dBz)
-ge3d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
-                  const Coef3<T>* __restrict__ coef) {
-    const Coef3<T> k = *coef;
-    const int g0 = 2 * (blockIdx.x * kLevel3dBx + threadIdx.x) - PH;      // anchor, 0-based element indices
-    const int g1 = 2 * (blockIdx.y * kLevel3dBy + threadIdx.y) - PH;
-    const int g2 = 2 * (blockIdx.z * kLevel3dBz + threadIdx.z) - PH;
+// one group, anchored at element (g0, g1, g2)
+template <typename T>
+__device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
+                                        const Coef3<T>& k, int g0, int g1, int g2) {
     if (g0 >= nx || g1 >= ny || g2 >= nz) return;
     // value of node (x,y,z): interior from memory, one step outside = the face value
     auto val = [&](int x, int y, int z) -> T {
@@ -162,12 +158,27 @@ ge3d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
     }
 }
 
+constexpr int kLevel3dGy = 1;       // groups per thread, consecutive in y (2 measured: no gain, the register allocation serialises them)
+
+template <typename T, int PH>
+__global__ void __launch_bounds__(kLevel3dBx * kLevel3dBy * kLevel3dBz)
+ge3d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
+                  const Coef3<T>* __restrict__ coef) {
+    const Coef3<T> k = *coef;
+    const int g0 = 2 * (blockIdx.x * kLevel3dBx + threadIdx.x) - PH;      // anchor, 0-based element indices
+    const int g1 = 2 * kLevel3dGy * (blockIdx.y * kLevel3dBy + threadIdx.y) - PH;
+    const int g2 = 2 * (blockIdx.z * kLevel3dBz + threadIdx.z) - PH;
+#pragma unroll
+    for (int s = 0; s < kLevel3dGy; ++s) group3d<T>(uin, uout, nx, ny, nz, k, g0, g1 + 2 * s, g2);
+}
+
 template <typename T>
 inline cudaError_t level3d_launch(const T* uin, T* uout, int64_t nx, int64_t ny, int64_t nz, const Coef3<T>* coef,
                                   int phase, cudaStream_t s) {
     auto groups = [&](int64_t n) { return (n + phase) / 2 + 1; };      // anchors -phase, 2-phase, ... <= n-1
     dim3 block(kLevel3dBx, kLevel3dBy, kLevel3dBz);
-    dim3 grid((unsigned)((groups(nx) + kLevel3dBx - 1) / kLevel3dBx), (unsigned)((groups(ny) + kLevel3dBy - 1) / kLevel3dBy),
+    dim3 grid((unsigned)((groups(nx) + kLevel3dBx - 1) / kLevel3dBx),
+              (unsigned)((groups(ny) + kLevel3dBy * kLevel3dGy - 1) / (kLevel3dBy * kLevel3dGy)),
               (unsigned)((groups(nz) + kLevel3dBz - 1) / kLevel3dBz));
     if (phase == 0) ge3d_level_kernel<T, 0><<<grid, block, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
     else            ge3d_level_kernel<T, 1><<<grid, block, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
