@@ -67,6 +67,11 @@ struct ge_plan {
     unsigned* res_flags;      // device: one flag per tile, + the fault word at [res_tiles]
     unsigned res_epoch;       // value every flag holds between launches
     int64_t meetings;         // meetings of the persistent kernel so far (info)
+    // ge_run_host pipeline (one long rod): per slot a stream, a device buffer and cached sub-plans
+    struct HostSlot { cudaStream_t stream; void* buf; size_t cap; cudaEvent_t h2d_done; ge_plan* sub[4]; int64_t sub_len[4]; };
+    HostSlot* slots;          // kHostSlots entries (lazy)
+    ge_desc host_desc;        // shape of this plan for the sub-plans (r, boundary values below)
+    double host_r, host_lo, host_hi;
     int32_t strip_attr_tb;    // block length whose strip-kernel function attributes are set on this device (0: none)
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
 };
@@ -556,6 +561,8 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (!p) return GE_ENOMEM;
     std::memset(p, 0, sizeof(*p));
     p->dim = d->dim; p->dtype = d->dtype; p->group_k = d->group_k;
+    p->host_r = d->r[0]; p->host_lo = d->bc_lo[0]; p->host_hi = d->bc_hi[0];
+    p->host_desc = *d;
     p->nx = d->nx; p->ny = d->ny; p->nz = d->dim == 3 ? d->nz : 1; p->batch = d->batch;
     p->count = d->dim == 1 ? d->batch * d->nx : d->ny * d->nx * p->nz;
     p->last_stream = (cudaStream_t)stream;
@@ -710,10 +717,97 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     return GE_OK;
 }
 
+// ge_run_host for one long rod: the rod is cut into chunks that are marched INDEPENDENTLY -- a chunk
+// carries 2*steps+8 extra nodes per side, more than the dependency cone of `steps` levels (a two-point
+// group reads u_{i-1}..u_{i+2}), so its interior comes out exactly as in the whole-rod
+// run -- and the chunks travel through a three-slot pipeline: while chunk c is computed, chunk c+1 is
+// on its way to the device and chunk c-1 on its way back.
+constexpr int kHostSlots = 3;
+constexpr int64_t kHostChunk = (int64_t)1 << 24;
+
+static int host_pipeline(ge_plan* p, void* u_host, int64_t steps, cudaStream_t user) {
+    const size_t es = elem_size(p->dtype);
+    const int64_t halo = (2 * steps + 8 + 3) & ~(int64_t)3, nx = p->nx;    // a multiple of 4: chunks keep the vector kernels
+    if (!p->slots) {
+        p->slots = new (std::nothrow) ge_plan::HostSlot[kHostSlots]();
+        if (!p->slots) return GE_ENOMEM;
+        for (int i = 0; i < kHostSlots; ++i) {
+            GE_CUDA(cudaStreamCreateWithFlags(&p->slots[i].stream, cudaStreamNonBlocking));
+            GE_CUDA(cudaEventCreateWithFlags(&p->slots[i].h2d_done, cudaEventDisableTiming));
+        }
+    }
+    cudaEvent_t start;
+    GE_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+    GE_CUDA(cudaEventRecord(start, user));
+    for (int i = 0; i < kHostSlots; ++i) GE_CUDA(cudaStreamWaitEvent(p->slots[i].stream, start, 0));
+    const int64_t nchunks = (nx + kHostChunk - 1) / kHostChunk;
+    auto range = [&](int64_t c, int64_t& i0, int64_t& i1, int64_t& o0, int64_t& o1) {
+        o0 = c * kHostChunk; o1 = o0 + kHostChunk < nx ? o0 + kHostChunk : nx;
+        i0 = o0 - halo > 0 ? o0 - halo : 0; i1 = o1 + halo < nx ? o1 + halo : nx;
+    };
+    auto upload = [&](int64_t c) -> int {
+        ge_plan::HostSlot& sl = p->slots[c % kHostSlots];
+        int64_t i0, i1, o0, o1; range(c, i0, i1, o0, o1);
+        const size_t bytes = (size_t)(i1 - i0) * es;
+        if (sl.cap < bytes) { cudaFree(sl.buf); sl.buf = nullptr; sl.cap = 0; GE_CUDA(cudaMalloc(&sl.buf, bytes)); sl.cap = bytes; }
+        GE_CUDA(cudaMemcpyAsync(sl.buf, (const char*)u_host + (size_t)i0 * es, bytes, cudaMemcpyHostToDevice, sl.stream));
+        GE_CUDA(cudaEventRecord(sl.h2d_done, sl.stream));
+        return GE_OK;
+    };
+    int rc = upload(0);
+    for (int64_t c = 0; c < nchunks && rc == GE_OK; ++c) {
+        ge_plan::HostSlot& sl = p->slots[c % kHostSlots];
+        int64_t i0, i1, o0, o1; range(c, i0, i1, o0, o1);
+        // sub-plan of this slot for this chunk shape: real boundary value where the chunk touches the rod's end
+        const int kind = (i0 == 0 ? 1 : 0) | (i1 == nx ? 2 : 0);
+        if (sl.sub[kind] && sl.sub_len[kind] != i1 - i0) { ge_plan_destroy(sl.sub[kind]); sl.sub[kind] = nullptr; }
+        if (!sl.sub[kind]) {
+            ge_desc d = p->host_desc;
+            const double r = p->host_r, lo = (kind & 1) ? p->host_lo : 0.0, hi = (kind & 2) ? p->host_hi : 0.0;
+            d.nx = i1 - i0; d.r = &r; d.bc_lo = &lo; d.bc_hi = &hi; d.kernel = p->kernel == GE_KERNEL_PER_STEP ? GE_KERNEL_PER_STEP : GE_KERNEL_TEMPORAL;
+            d.tb = p->tb > 0 ? p->tb : 0;
+            rc = ge_plan_create(&sl.sub[kind], &d, (ge_stream_t)sl.stream);
+            if (rc != GE_OK) break;
+            sl.sub_len[kind] = i1 - i0;
+        }
+        ge_plan* sub = sl.sub[kind];
+        sub->level = p->level;
+        rc = ge_run(sub, sl.buf, steps, (ge_stream_t)sl.stream);
+        if (rc != GE_OK) break;
+        p->launches += sub->launches; sub->launches = 0;
+        // the next chunk reads host nodes this chunk is about to overwrite: upload it first
+        if (c + 1 < nchunks) {
+            // its slot's previous download (chunk c-2) is ordered before by the slot's stream
+            rc = upload(c + 1);
+            if (rc != GE_OK) break;
+            GE_CUDA(cudaStreamWaitEvent(sl.stream, p->slots[(c + 1) % kHostSlots].h2d_done, 0));
+        }
+        // ... and so did the previous chunk (its upload is long done; make the order explicit)
+        if (c >= 1) GE_CUDA(cudaStreamWaitEvent(sl.stream, p->slots[(c - 1) % kHostSlots].h2d_done, 0));
+        GE_CUDA(cudaMemcpyAsync((char*)u_host + (size_t)o0 * es, (const char*)sl.buf + (size_t)(o0 - i0) * es,
+                                (size_t)(o1 - o0) * es, cudaMemcpyDeviceToHost, sl.stream));
+    }
+    for (int i = 0; i < kHostSlots; ++i) {
+        const cudaError_t e = cudaStreamSynchronize(p->slots[i].stream);
+        if (e != cudaSuccess && rc == GE_OK) { g_last_cuda = e; rc = GE_ECUDA; }
+    }
+    cudaEventDestroy(start);
+    if (rc == GE_OK) p->level += steps;
+    return rc;
+}
+
 int ge_run_host(ge_plan* p, void* u_host, int64_t steps, ge_stream_t stream) {
     if (!p || !u_host || steps < 0) return GE_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t bytes = (size_t)p->count * elem_size(p->dtype);
+    if (p->dim == 1 && p->batch == 1 && p->group_k == 1 && steps > 0 && p->nx >= 2 * kHostChunk &&
+        2 * steps + 8 <= kHostChunk / 8) {
+        p->last_stream = s;
+        const int rc = host_pipeline(p, u_host, steps, s);
+        if (rc != GE_OK) return rc;
+        GE_CUDA(cudaStreamSynchronize(s));
+        return GE_OK;
+    }
     if (!p->hostpath) GE_CUDA(cudaMalloc(&p->hostpath, bytes));
     GE_CUDA(cudaMemcpyAsync(p->hostpath, u_host, bytes, cudaMemcpyHostToDevice, s));
     int rc = ge_run(p, p->hostpath, steps, stream);
@@ -850,6 +944,15 @@ int ge_plan_destroy(ge_plan* p) {
     cudaFree(p->hostpath);
     cudaFree(p->res_xbuf);
     cudaFree(p->res_flags);
+    if (p->slots) {
+        for (int i = 0; i < kHostSlots; ++i) {
+            for (int kd = 0; kd < 4; ++kd) if (p->slots[i].sub[kd]) ge_plan_destroy(p->slots[i].sub[kd]);
+            cudaFree(p->slots[i].buf);
+            if (p->slots[i].stream) cudaStreamDestroy(p->slots[i].stream);
+            if (p->slots[i].h2d_done) cudaEventDestroy(p->slots[i].h2d_done);
+        }
+        delete[] p->slots;
+    }
     delete p;
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     return GE_OK;

@@ -95,3 +95,14 @@ def test_c5_full_size(oracle, dtype):
     assert ia["launches"] < ib["launches"] == cfg["steps"]
     assert np.isfinite(a).all()
     np.testing.assert_array_equal(a, b)
+
+
+@pytest.mark.parametrize("dtype,steps,level0", [("f64", 40, 0), ("f32", 33, 1)])
+def test_run_host_pipeline_is_bit_identical(dtype, steps, level0):
+    """ge_run_host on a rod of several chunks (halo-redundant chunks through a three-slot pipeline) against
+    ge_run on the whole rod: bit for bit, including a ragged last chunk and an odd level count."""
+    cfg = inputs.random_rods(1, 3 * 2 ** 24 + 40960, dtype, seed=13)
+    a, ia = run_gpu(cfg, steps, via="host", level0=level0)
+    b, _ = run_gpu(cfg, steps, via="run", level0=level0)
+    assert ia["launches"] > 0
+    np.testing.assert_array_equal(a, b)
