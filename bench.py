@@ -417,7 +417,8 @@ def run_src(args):
                    "levels_per_step": levels, "kernel": "per_step"},
         "gpu_launches": levels * args.steps, "finite": bool(torch.isfinite(u).all().item()),
         "roofline": {"kernel": "ge1d_level_src_kernel<%s>" % cfg["dtype"], "bound": "hbm", "achieved": gbs,
-                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"], "traffic": None,
+                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                     "traffic": traffic_of("%s/ge1d_level_src_kernel<%s>" % (cfg["name"], cfg["dtype"])),
                      "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * cfg["nx"]},
         "e2e": None, "cpu_baseline": None}), flush=True)
     plan.close()
