@@ -151,9 +151,11 @@ int launch_level_1d(ge_plan* p, const void* uin, void* uout, int phase, cudaStre
 
 template <typename T>
 int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStream_t s) {
-    constexpr int V = ge::VecOf<T>::V;
-    const bool vec = (p->nx % V == 0) && (((uintptr_t)uin | (uintptr_t)uout) % 16 == 0);
-    const int64_t nvec = vec ? p->nx / V : p->nx;
+    constexpr int NV = ge::VecOf<T>::V;
+    constexpr int V = 4;                               // columns per thread: one float4, two double2
+    const bool aligned = (((uintptr_t)uin | (uintptr_t)uout) % 16 == 0);
+    const int v = aligned && p->nx % V == 0 ? V : (aligned && p->nx % NV == 0 ? NV : 1);
+    const int64_t nvec = p->nx / v;
     const int64_t npair = (p->ny + phase) / 2 + 1;      // anchor rows -phase, 2-phase, ... <= ny-1
     dim3 grid((unsigned)((nvec + ge::kLevel2dBx - 1) / ge::kLevel2dBx),
               (unsigned)((npair + ge::kLevel2dBy - 1) / ge::kLevel2dBy));
@@ -161,9 +163,12 @@ int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStre
     auto* c = (const ge::Coef2<T>*)p->coef;
     auto* in = (const T*)uin;
     auto* out = (T*)uout;
-    if (vec) {
+    if (v == V) {
         if (phase == 0) ge::ge2d_level_kernel<T, V, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
         else            ge::ge2d_level_kernel<T, V, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+    } else if (v == NV) {
+        if (phase == 0) ge::ge2d_level_kernel<T, NV, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+        else            ge::ge2d_level_kernel<T, NV, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
     } else {
         if (phase == 0) ge::ge2d_level_kernel<T, 1, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
         else            ge::ge2d_level_kernel<T, 1, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);

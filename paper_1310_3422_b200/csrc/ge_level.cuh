@@ -151,13 +151,17 @@ ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, i
         const int64_t y = j0 - 1 + rr;
         const bool yin = y >= 0 && y < ny;
         if constexpr (V > 1) {
-            T t[V];
+            constexpr int NV = VecOf<T>::V;            // native 16-byte vector; V is a multiple of it
+            T t[NV];
             if (yin) {
                 const T* __restrict__ row = uin + y * nx;
-                ld_vec(row + e0, t);
 #pragma unroll
-                for (int j = 0; j < V; ++j) w[rr][2 + j] = t[j];
-                if (e0 >= V) { ld_vec(row + e0 - V, t); w[rr][0] = t[V - 2]; w[rr][1] = t[V - 1]; }
+                for (int c = 0; c < V / NV; ++c) {
+                    ld_vec(row + e0 + c * NV, t);
+#pragma unroll
+                    for (int j = 0; j < NV; ++j) w[rr][2 + c * NV + j] = t[j];
+                }
+                if (e0 >= NV) { ld_vec(row + e0 - NV, t); w[rr][0] = t[NV - 2]; w[rr][1] = t[NV - 1]; }
                 else { w[rr][0] = T(0); w[rr][1] = k.xlo; }
                 if (e0 + V < nx) { ld_vec(row + e0 + V, t); w[rr][V + 2] = t[0]; w[rr][V + 3] = t[1]; }
                 else { w[rr][V + 2] = k.xhi; w[rr][V + 3] = T(0); }
@@ -193,11 +197,22 @@ ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, i
         if (m >= 0) { o[0][m] = na; o[1][m] = nc; }
         if (m + 1 < V) { o[0][m + 1] = nb; o[1][m + 1] = nd; }
     }
-    if (j0 >= 0) {
-        if constexpr (V > 1) st_vec(uout + j0 * nx + e0, o[0]); else uout[j0 * nx + e0] = o[0][0];
-    }
-    if (j0 + 1 < ny) {
-        if constexpr (V > 1) st_vec(uout + (j0 + 1) * nx + e0, o[1]); else uout[(j0 + 1) * nx + e0] = o[1][0];
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+        const int64_t y = j0 + rr;
+        if (y < 0 || y >= ny) continue;
+        if constexpr (V > 1) {
+            constexpr int NV = VecOf<T>::V;
+#pragma unroll
+            for (int c = 0; c < V / NV; ++c) {
+                T t[NV];
+#pragma unroll
+                for (int j = 0; j < NV; ++j) t[j] = o[rr][c * NV + j];
+                st_vec(uout + y * nx + e0 + c * NV, t);
+            }
+        } else {
+            uout[y * nx + e0] = o[rr][0];
+        }
     }
 }
 
