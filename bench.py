@@ -52,6 +52,8 @@ def make_cfg(name, scale=1.0):
     if name in ("c5_f32", "c5_f64"):
         n = int(8192 * scale ** 0.5)
         return inputs.make_c5(n=n - n % 2, dtype=name[3:])
+    if name == "paper":                       # PAPER.md:204-218 run shape; use with --k 16
+        return inputs.make_paper()
     if name in ("box_f32", "box_f64"):        # 3-D (NEXT-4), not a BASELINE.json config
         n = int(512 * scale ** (1.0 / 3.0))
         return inputs.make_box(n=n - n % 2, dtype=name[4:])
@@ -89,7 +91,7 @@ def oracle_time(cfg):
         ge_oracle.run_2d(u0, cfg["r"][0], cfg["steps"],
                          (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1]))
     elif cfg["batch"] == 1:
-        ge_oracle.run_1d(u0.reshape(-1), cfg["r"][0], cfg["steps"], cfg["bc_lo"][0], cfg["bc_hi"][0])
+        ge_oracle.run_1d(u0.reshape(-1), cfg["r"][0], cfg["steps"], cfg["bc_lo"][0], cfg["bc_hi"][0], k=cfg.get("k", 1))
     else:
         ge_oracle.run_batched_1d(u0, cfg["r"], cfg["steps"], cfg["bc_lo"], cfg["bc_hi"])
     return time.perf_counter() - t0
@@ -135,6 +137,7 @@ def make_cfg_meta(name):
             "c4": "c4: 1-D GE, N=268435456 interior, f64, 200 levels per step",
             "c5_f32": "c5_f32: 2-D GE, 8192x8192 interior, f32, 1000 levels per step",
             "c5_f64": "c5_f64: 2-D GE, 8192x8192 interior, f64, 1000 levels per step",
+            "paper": "paper: 1-D GE, N=8206 interior, f32, 1200 levels per step",
             "box_f32": "box_f32: 3-D GE, 512x512x512 interior, f32, 100 levels per step",
             "box_f64": "box_f64: 3-D GE, 512x512x512 interior, f64, 100 levels per step"}
     return meta[name]
@@ -338,6 +341,7 @@ def run_ours(args):
         ge_oracle.build()
         scale = args.cpu_scale
         scfg = make_cfg(args.config, scale)
+        scfg["k"] = args.k
         if args.levels:
             scfg["steps"] = args.levels
         t = oracle_time(scfg)

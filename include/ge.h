@@ -78,7 +78,8 @@ typedef struct {
     int32_t   dtype;      /* ge_dtype: arithmetic and storage type of u                                */
     int32_t   group_k;    /* 1 = two-point groups (2x2 groups in 2-D); 2..2048 = PAPER.md:82 sub-domain
                              length k (1-D only; the paper's runs use 16): confluence pairs every 2k nodes
-                             joined by Saul'yev sweeps; always strategy A (one launch per level)       */
+                             joined by Saul'yev sweeps; strategy A (one launch per level), or C when a
+                             rod fits in one CTA's shared memory (AUTO / PERSISTENT)                  */
     const double *r;      /* HOST array, `batch` entries (dim 2: 1 entry), finite, > 0; copied         */
     const double *bc_lo;  /* HOST array: 1-D `batch` entries, u at node 0;   2-D {x_lo, y_lo}; 3-D {x_lo, y_lo, z_lo} */
     const double *bc_hi;  /* HOST array: 1-D `batch` entries, u at node N+1; 2-D {x_hi, y_hi}; 3-D {x_hi, y_hi, z_hi} */
@@ -139,7 +140,8 @@ enum {
     GE_INFO_LAUNCHES = 2,      /* kernels launched through this plan so far                       */
     GE_INFO_TILE_VALID = 3,    /* valid outputs per tile of the temporal kernel (per axis)        */
     GE_INFO_TILE_LOADED = 4,   /* elements loaded per tile of the temporal kernel (per axis)      */
-    GE_INFO_RESIDENT_PATH = 5, /* strategy C: 0 not in use, 1 rod per CTA, 2 one rod on the whole chip */
+    GE_INFO_RESIDENT_PATH = 5, /* strategy C: 0 not in use, 1 rod per CTA, 2 one rod on the whole chip,
+                                  3 group_k >= 2: rod per CTA, resident in shared memory               */
     GE_INFO_RESIDENT_C = 6,    /* strategy C: values per lane                                     */
     GE_INFO_RESIDENT_WARPS = 7,/* path 1: warps per rod; path 2: tiles (warps) in the launch      */
     GE_INFO_RESIDENT_CAPACITY = 8, /* path 2: co-resident tiles the device offers                 */

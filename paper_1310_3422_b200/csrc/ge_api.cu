@@ -74,6 +74,7 @@ struct ge_plan {
     double host_r, host_lo, host_hi;
     int32_t strip_attr_tb;    // block length whose strip-kernel function attributes are set on this device (0: none)
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
+    bool rodk_attr;           // ... and of its shared-memory-resident form
 };
 
 namespace {
@@ -197,6 +198,31 @@ int launch_level_k(ge_plan* p, const void* uin, void* uout, int phase, cudaStrea
                                                                       (const ge::Coef1<T>*)p->coef, g);
     GE_CUDA(cudaGetLastError());
     p->launches += 1;
+    return GE_OK;
+}
+
+// strategy C for k >= 2: the rod resident in shared memory, one launch for the whole run (res_path 3)
+constexpr size_t kRodKSmemMax = 200 * 1024;
+bool rod_k_fits(const ge_plan* p) {
+    if (p->dim != 1 || p->group_k < 2 || p->nx >= (1 << 24)) return false;
+    const ge::RodKGeom g = ge::rod_k_geom(p->group_k, p->nx, elem_size(p->dtype));
+    return g.threads > 0 && g.smem <= kRodKSmemMax;
+}
+template <typename T>
+int launch_rod_k_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
+    const ge::RodKGeom g = ge::rod_k_geom(p->group_k, p->nx, sizeof(T));
+    if (!p->rodk_attr) {
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_rod_k_resident_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)kRodKSmemMax));
+        p->rodk_attr = true;
+    }
+    const unsigned grid = (unsigned)(p->batch < (1 << 30) ? p->batch : (1 << 30));
+    ge::ge1d_rod_k_resident_kernel<T><<<grid, g.threads, g.smem, s>>>((T*)u, p->nx, p->batch,
+                                                                      (const ge::Coef1<T>*)p->coef, p->group_k,
+                                                                      (int)(p->level & 1), steps);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    p->level += steps;
     return GE_OK;
 }
 
@@ -591,9 +617,13 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
-    if (d->group_k >= 2) kernel = GE_KERNEL_PER_STEP;      // k >= 2: strategy A only (ge_level_k.cuh)
+    if (d->group_k >= 2) {                                  // k >= 2 (ge_level_k.cuh): strategy A, or C when the rod fits in shared memory
+        const bool want_c = kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT;
+        kernel = GE_KERNEL_PER_STEP;
+        if (want_c && rod_k_fits(p)) { kernel = GE_KERNEL_PERSISTENT; p->res_path = 3; }
+    }
     if (d->dim == 3) kernel = GE_KERNEL_PER_STEP;          // 3-D: strategy A only (ge_level3d.cuh)
-    if (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT) {
+    if (d->group_k == 1 && (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT)) {
         p->res_tb = d->tb;
         rc = resident_configure(p, 0);
         if (rc != GE_OK) { cudaFree(p->coef); cudaFree(p->scratch); cudaFree(p->res_xbuf); cudaFree(p->res_flags); cudaGetLastError(); delete p; return rc; }
@@ -663,6 +693,11 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     void* oth = p->scratch;
     int64_t left = steps;
     int rc = GE_OK;
+    if (p->kernel == GE_KERNEL_PERSISTENT && p->res_path == 3) {
+        if (steps == 0) return GE_OK;
+        return p->dtype == GE_F64 ? launch_rod_k_resident<double>(p, u, steps, s)
+                                  : launch_rod_k_resident<float>(p, u, steps, s);
+    }
     if (p->kernel == GE_KERNEL_PERSISTENT && resident_ok(p, u)) {
         // strategy C: the whole run is one launch, in place
         if (steps == 0) return GE_OK;

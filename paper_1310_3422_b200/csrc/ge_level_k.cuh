@@ -171,3 +171,97 @@ ge1d_level_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx,
 }
 
 }  // namespace ge
+
+// ------------------------------------------------------------------------------------------------
+// Strategy C for k >= 2: the whole run of a rod in ONE launch, the rod resident in shared memory
+// (the paper's own run shape -- 8208 nodes, sub-domain couples of 32, <= 1200 levels, PAPER.md:204-218
+// -- is launch-bound at one launch per level: 6 us per level for 0.1 us of work).
+// One CTA per rod, one thread per unit as above; per level every thread reads the two old values either
+// side of its unit, the CTA synchronises, the unit is updated in place, the CTA synchronises -- the
+// paper's two barriers per level PAIR become two per level, but they are CTA barriers that cost ~50 ns
+// and there is no block-to-block ordering left to luck.  The unit decomposition shifts by
+// k nodes between levels, so the layout is linear in the node index, skewed by one word per 32 (node i
+// at i + i/32): threads 2k nodes apart fall into different banks whatever the phase.
+namespace ge {
+
+struct RodKGeom {
+    int k;
+    int threads;           // >= units of either phase, multiple of 32, <= 1024
+    size_t smem;           // bytes
+};
+inline RodKGeom rod_k_geom(int k, int64_t nx, size_t elem) {
+    RodKGeom g;
+    g.k = k;
+    const int64_t units = (nx + k) / (2 * (int64_t)k) + 1;            // phase 1 has the most
+    g.threads = units <= 1024 ? (int)((units + 31) / 32 * 32) : 0;
+    const int64_t words = (nx + 2) + (nx + 2) / 32 + 1;
+    g.smem = (size_t)words * elem;
+    return g;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(1024)
+ge1d_rod_k_resident_kernel(T* u, int64_t nx, int64_t batch, const Coef1<T>* __restrict__ coef, int k,
+                           int phase0, int64_t steps) {
+    extern __shared__ __align__(16) unsigned char rodk_smem[];
+    T* sm = reinterpret_cast<T*>(rodk_smem);
+    const int N = (int)nx, two_k = 2 * k;
+    auto at = [&](int i) -> T& { return sm[i + (i >> 5)]; };           // node i, 0 <= i <= N+1
+    auto rd = [&](int i) -> T { return (i >= 0 && i <= N + 1) ? sm[i + (i >> 5)] : T(0); };
+    const int t = threadIdx.x;
+    for (int64_t rod = blockIdx.x; rod < batch; rod += gridDim.x) {
+        const Coef1<T> c = coef[rod];
+        T* row = u + rod * nx;
+        for (int i = t; i <= N + 1; i += blockDim.x) at(i) = i == 0 ? c.lo : (i == N + 1 ? c.hi : row[i - 1]);
+        __syncthreads();
+#pragma unroll 1
+        for (int64_t lev = 0; lev < steps; ++lev) {
+            const int phase = (int)((phase0 + lev) & 1);
+            const int s = (phase ? -k : 0) + t * two_k;               // node with c = 0
+            const int e = s + two_k - 1;                               // node with c = 2k-1
+            const bool mine = s <= N;
+            T om2 = T(0), om1 = T(0), op0 = T(0), op1 = T(0), o0 = T(0), o1 = T(0), oe1 = T(0), oe = T(0);
+            if (mine) {
+                om2 = rd(s - 2); om1 = rd(s - 1); o0 = rd(s); o1 = rd(s + 1);
+                oe1 = rd(e - 1); oe = rd(e); op0 = rd(e + 1); op1 = rd(e + 2);
+            }
+            __syncthreads();                                           // everybody has its old wall values
+            if (mine) {
+                T prev = c.lo, next = c.hi;
+                if (s >= 1) {
+                    T lo_, hi_;
+                    pair_update_bc(om2, om1, o0, o1, c, s - 1 == 0, false, lo_, hi_);
+                    prev = hi_;
+                    at(s) = prev;
+                }
+                if (e >= 1 && e <= N) {
+                    T lo_, hi_;
+                    pair_update_bc(oe1, oe, op0, op1, c, false, e + 1 == N + 1, lo_, hi_);
+                    next = lo_;
+                    at(e) = next;
+                }
+                T a_old = o1, b_old = oe1;
+#pragma unroll 4
+                for (int m = 1; m < k; ++m) {
+                    const int ia = s + m, ib = e - m;
+                    const T a_nxt = rd(ia + 1);
+                    const T b_nxt = rd(ib - 1);
+                    if (ia >= 1 && ia <= N) {
+                        prev = fma(c.e, (prev - a_old) + (a_nxt - a_old), a_old);
+                        at(ia) = prev;
+                    }
+                    if (ib >= 1 && ib <= N) {
+                        next = fma(c.e, (next - b_old) + (b_nxt - b_old), b_old);
+                        at(ib) = next;
+                    }
+                    a_old = a_nxt; b_old = b_nxt;
+                }
+            }
+            __syncthreads();
+        }
+        for (int i = t; i < N; i += blockDim.x) row[i] = at(i + 1);
+        __syncthreads();
+    }
+}
+
+}  // namespace ge

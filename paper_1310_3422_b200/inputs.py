@@ -125,3 +125,10 @@ def make_box(n=512, steps=100, r=2.0, dtype="f32", seed=4):
     cfg = _cfg("box", 3, n, n, 1, dtype, steps, [r], [0.0, 0.0, 0.0], [0.0, 0.0, 0.0], u0)
     cfg["nz"] = int(n)
     return cfg
+
+
+def make_paper(n=8206, steps=1200, r=1.0, dtype="f32"):
+    """The paper's own run shape: 8208 nodes including the two boundary nodes, sub-domain
+    couples of 32 nodes (k = 16, passed to the plan as group_k), up to ~1200 levels; the paper states
+    neither r nor phi: r = 1, u0 = sin(pi x), zero boundary values are this repository's choice."""
+    return _cfg("paper", 1, n, 1, 1, dtype, steps, [r], [0.0], [0.0], np.sin(np.pi * _x(n)))

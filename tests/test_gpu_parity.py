@@ -212,10 +212,23 @@ def test_general_k_per_level(oracle, dtype, k, n):
     phases, per-rod r and unequal boundary values."""
     cfg = inputs.random_rods(3, n, dtype, seed=17 * k + n)
     for level0, steps in ((0, 1), (1, 1), (0, 2), (1, 7), (0, 40)):
-        got, info = run_gpu(cfg, steps, level0=level0, k=k)
+        got, info = run_gpu(cfg, steps, level0=level0, k=k, kernel="per_step")
         ref = run_oracle(oracle, cfg, steps, level0=level0, k=k)
         assert info["kernel"] == "per_step" and info["launches"] == steps
         assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (k, n, level0, steps)
+        # strategy C (the rod resident in shared memory, one launch): AUTO picks it when the rod fits
+        res, info = run_gpu(cfg, steps, level0=level0, k=k)
+        assert info["kernel"] == "persistent" and info["resident_path"] == 3 and info["launches"] == 1, info
+        np.testing.assert_array_equal(res, got)
+
+
+def test_general_k_resident_needs_the_rod_to_fit():
+    cfg = inputs.random_rods(1, 100000, "f64", seed=1)           # 800 KB: more than a CTA's shared memory
+    _, info = run_gpu(cfg, 3, k=16)
+    assert info["kernel"] == "per_step" and info["resident_path"] == 0 and info["launches"] == 3
+    cfg = inputs.random_rods(1, 40000, "f32", seed=1)            # fits, but 10 001 units > 1024 threads at k = 2
+    _, info = run_gpu(cfg, 3, k=2)
+    assert info["kernel"] == "per_step"
 
 
 def test_general_k_matches_the_closed_form(oracle):
