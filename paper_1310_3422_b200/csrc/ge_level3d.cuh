@@ -27,7 +27,19 @@ struct Coef3 {
     T pad[6];
 };
 
-constexpr int kLevel3dBx = 32, kLevel3dBy = 4, kLevel3dBz = 2;
+#ifndef GE_L3D_BX
+#define GE_L3D_BX 32
+#endif
+#ifndef GE_L3D_BY
+#define GE_L3D_BY 4
+#endif
+#ifndef GE_L3D_BZ
+#define GE_L3D_BZ 1
+#endif
+#ifndef GE_L3D_MINB
+#define GE_L3D_MINB 1
+#endif
+constexpr int kLevel3dBx = GE_L3D_BX, kLevel3dBy = GE_L3D_BY, kLevel3dBz = GE_L3D_BZ;   // block of groups (sweeps: GE_NVCC_EXTRA)
 
 template <typename T>
 __device__ __forceinline__ void wht8(T (&v)[8]) {
@@ -161,7 +173,7 @@ __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict
 constexpr int kLevel3dGy = 1;       // groups per thread, consecutive in y (2 measured: no gain, the register allocation serialises them)
 
 template <typename T, int PH>
-__global__ void __launch_bounds__(kLevel3dBx * kLevel3dBy * kLevel3dBz)
+__global__ void __launch_bounds__(kLevel3dBx * kLevel3dBy * kLevel3dBz, GE_L3D_MINB)
 ge3d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
                   const Coef3<T>* __restrict__ coef) {
     const Coef3<T> k = *coef;
