@@ -15,6 +15,8 @@
 // side) is solved by elimination -- only the outermost layer of groups takes this path.
 // One thread per group, x fastest: a warp reads 64 consecutive nodes of a row.
 #pragma once
+#include <type_traits>
+
 #include "ge_common.cuh"
 
 namespace ge {
@@ -91,7 +93,7 @@ __device__ __forceinline__ void truncated_group3d(const T (&R)[8], const bool (&
 }
 
 // one group, anchored at element (g0, g1, g2)
-template <typename T>
+template <typename T, int PH>
 __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
                                         const Coef3<T>& k, int g0, int g1, int g2) {
     if (g0 >= nx || g1 >= ny || g2 >= nz) return;
@@ -111,16 +113,22 @@ __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict
     T R[8];
     bool in[8];
     if (deep) {
+        // twelve row pointers (rows y-1 .. y+2 of planes z, z+1; rows y, y+1 of planes z-1, z+2), every load
+        // at a constant offset from one of them: the address arithmetic is paid per row, not per load
         const int64_t sy = nx, sz = (int64_t)nx * ny;
         const T* __restrict__ base = uin + ((int64_t)g2 * ny + g1) * nx + g0;
+        const T* __restrict__ rp[4][4];
+#pragma unroll
+        for (int zz = 0; zz < 4; ++zz)
+#pragma unroll
+            for (int yy = 0; yy < 4; ++yy) rp[zz][yy] = base + (zz - 1) * sz + (yy - 1) * sy;
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
             const int dx = d & 1, dy = (d >> 1) & 1, dz = (d >> 2) & 1;
-            const T* __restrict__ q = base + dz * sz + dy * sy + dx;
-            const T o = __ldg(q);
-            const T ox = __ldg(q + (dx ? 1 : -1));
-            const T oy = __ldg(q + (dy ? sy : -sy));
-            const T oz = __ldg(q + (dz ? sz : -sz));
+            const T o = __ldg(rp[dz + 1][dy + 1] + dx);
+            const T ox = __ldg(rp[dz + 1][dy + 1] + (dx ? 2 : -1));
+            const T oy = __ldg(rp[dz + 1][dy ? 3 : 0] + dx);
+            const T oz = __ldg(rp[dz ? 3 : 0][dy + 1] + dx);
             in[d] = true;
             R[d] = fma(k.r, ((ox - o) + (oy - o)) + (oz - o), o);
         }
@@ -158,8 +166,19 @@ __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict
     if (full) {
         T* __restrict__ ob = uout + ((int64_t)g2 * ny + g1) * nx + g0;
         const int64_t sy = nx, sz = (int64_t)nx * ny;
+        // phase 0: the anchor column is even, a row's two members are one aligned 8- / 16-byte store (nx even)
+        const bool pairs = PH == 0 && (nx & 1) == 0 && ((uintptr_t)uout % (2 * sizeof(T))) == 0;
+        if (pairs) {
+            using P2 = typename std::conditional<sizeof(T) == 8, double2, float2>::type;
 #pragma unroll
-        for (int d = 0; d < 8; ++d) ob[((d >> 2) & 1) * sz + ((d >> 1) & 1) * sy + (d & 1)] = nw[d];
+            for (int d = 0; d < 8; d += 2) {
+                P2 v; v.x = nw[d]; v.y = nw[d + 1];
+                *reinterpret_cast<P2*>(ob + ((d >> 2) & 1) * sz + ((d >> 1) & 1) * sy) = v;
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < 8; ++d) ob[((d >> 2) & 1) * sz + ((d >> 1) & 1) * sy + (d & 1)] = nw[d];
+        }
     } else {
 #pragma unroll
         for (int d = 0; d < 8; ++d)
@@ -181,7 +200,7 @@ ge3d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
     const int g1 = 2 * kLevel3dGy * (blockIdx.y * kLevel3dBy + threadIdx.y) - PH;
     const int g2 = 2 * (blockIdx.z * kLevel3dBz + threadIdx.z) - PH;
 #pragma unroll
-    for (int s = 0; s < kLevel3dGy; ++s) group3d<T>(uin, uout, nx, ny, nz, k, g0, g1 + 2 * s, g2);
+    for (int s = 0; s < kLevel3dGy; ++s) group3d<T, PH>(uin, uout, nx, ny, nz, k, g0, g1 + 2 * s, g2);
 }
 
 template <typename T>
