@@ -518,7 +518,7 @@ def main():
     ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--cpu-scale", type=float, default=1 / 64, help="grid fraction of the cpu_baseline sample")
+    ap.add_argument("--cpu-scale", type=float, default=1 / 32, help="grid fraction of the cpu_baseline sample")
     ap.add_argument("--ref-scale", type=float, default=1 / 256, help="grid fraction of the --impl reference sample")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
