@@ -126,7 +126,8 @@ int ge_run(ge_plan *p, void *u, int64_t steps, ge_stream_t stream);
  * synchronises `stream` before returning.  One long rod (dim 1, batch 1, nx >= 2^25) is cut into chunks
  * of 2^24 nodes that carry 2*steps+8 extra nodes per side -- more than the dependency cone of `steps`
  * levels -- and are marched independently through a three-slot pipeline (upload, compute and download of
- * neighbouring chunks overlap; u_host should be pinned for that); the result is bit-identical. */
+ * neighbouring chunks overlap; u_host should be pinned for that); the result is bit-identical.  Batched rods
+ * (batch >= 64, >= 8 MiB) travel through the same pipeline in eight groups of rods. */
 int ge_run_host(ge_plan *p, void *u_host, int64_t steps, ge_stream_t stream);
 
 /* Level counter (checkpoint/resume: state = (u, level)). */

@@ -836,6 +836,56 @@ static int host_pipeline(ge_plan* p, void* u_host, int64_t steps, cudaStream_t u
     return rc;
 }
 
+// ge_run_host for batched rods: the rods are independent, so the batch travels in groups of rods through the
+// same three-slot pipeline (upload of group c+1 and download of group c-1 overlap the levels of group c).
+// A group is run by pointing the plan at its slice of the state, the coefficient table and the scratch level.
+static int host_pipeline_rods(ge_plan* p, void* u_host, int64_t steps, cudaStream_t user) {
+    const size_t es = elem_size(p->dtype);
+    const size_t coef_sz = p->dtype == GE_F64 ? sizeof(ge::Coef1<double>) : sizeof(ge::Coef1<float>);
+    const int64_t groups = 8, per = (p->batch + groups - 1) / groups;
+    if (!p->slots) {
+        p->slots = new (std::nothrow) ge_plan::HostSlot[kHostSlots]();
+        if (!p->slots) return GE_ENOMEM;
+        for (int i = 0; i < kHostSlots; ++i) {
+            GE_CUDA(cudaStreamCreateWithFlags(&p->slots[i].stream, cudaStreamNonBlocking));
+            GE_CUDA(cudaEventCreateWithFlags(&p->slots[i].h2d_done, cudaEventDisableTiming));
+        }
+    }
+    const size_t bytes = (size_t)p->count * es;
+    if (!p->hostpath) GE_CUDA(cudaMalloc(&p->hostpath, bytes));
+    cudaEvent_t start;
+    GE_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+    GE_CUDA(cudaEventRecord(start, user));
+    for (int i = 0; i < kHostSlots; ++i) GE_CUDA(cudaStreamWaitEvent(p->slots[i].stream, start, 0));
+    // the plan is pointed at one group at a time
+    const int64_t batch0 = p->batch, count0 = p->count, level0 = p->level;
+    void* const coef0 = p->coef; void* const scratch0 = p->scratch;
+    int rc = GE_OK;
+    int64_t c = 0;
+    for (int64_t rod0 = 0; rod0 < batch0 && rc == GE_OK; rod0 += per, ++c) {
+        const int64_t n = rod0 + per <= batch0 ? per : batch0 - rod0;
+        cudaStream_t st = p->slots[c % kHostSlots].stream;
+        const size_t off = (size_t)rod0 * p->nx * es, len = (size_t)n * p->nx * es;
+        cudaError_t e = cudaMemcpyAsync((char*)p->hostpath + off, (const char*)u_host + off, len, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { g_last_cuda = e; rc = GE_ECUDA; break; }
+        p->batch = n; p->count = n * p->nx; p->level = level0;
+        p->coef = (char*)coef0 + (size_t)rod0 * coef_sz;
+        p->scratch = (char*)scratch0 + off;
+        rc = ge_run(p, (char*)p->hostpath + off, steps, (ge_stream_t)st);
+        if (rc != GE_OK) break;
+        e = cudaMemcpyAsync((char*)u_host + off, (const char*)p->hostpath + off, len, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) { g_last_cuda = e; rc = GE_ECUDA; }
+    }
+    p->batch = batch0; p->count = count0; p->coef = coef0; p->scratch = scratch0;
+    for (int i = 0; i < kHostSlots; ++i) {
+        const cudaError_t e = cudaStreamSynchronize(p->slots[i].stream);
+        if (e != cudaSuccess && rc == GE_OK) { g_last_cuda = e; rc = GE_ECUDA; }
+    }
+    cudaEventDestroy(start);
+    p->level = rc == GE_OK ? level0 + steps : level0;
+    return rc;
+}
+
 int ge_run_host(ge_plan* p, void* u_host, int64_t steps, ge_stream_t stream) {
     if (!p || !u_host || steps < 0) return GE_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -844,6 +894,13 @@ int ge_run_host(ge_plan* p, void* u_host, int64_t steps, ge_stream_t stream) {
         2 * steps + 8 <= kHostChunk / 8) {
         p->last_stream = s;
         const int rc = host_pipeline(p, u_host, steps, s);
+        if (rc != GE_OK) return rc;
+        GE_CUDA(cudaStreamSynchronize(s));
+        return GE_OK;
+    }
+    if (p->dim == 1 && p->batch >= 64 && steps > 0 && bytes >= ((size_t)8 << 20) && p->res_path != 2) {
+        p->last_stream = s;
+        const int rc = host_pipeline_rods(p, u_host, steps, s);
         if (rc != GE_OK) return rc;
         GE_CUDA(cudaStreamSynchronize(s));
         return GE_OK;

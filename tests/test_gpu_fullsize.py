@@ -106,3 +106,14 @@ def test_run_host_pipeline_is_bit_identical(dtype, steps, level0):
     b, _ = run_gpu(cfg, steps, via="run", level0=level0)
     assert ia["launches"] > 0
     np.testing.assert_array_equal(a, b)
+
+
+@pytest.mark.parametrize("dtype,kernel", [("f32", "auto"), ("f64", "temporal"), ("f32", "per_step")])
+def test_run_host_rod_groups_are_bit_identical(dtype, kernel):
+    """ge_run_host on batched rods (eight groups of rods through the three-slot pipeline, ragged last group)
+    against ge_run on the whole batch."""
+    cfg = inputs.random_rods(1003, 4096, dtype, seed=21)
+    a, ia = run_gpu(cfg, 33, via="host", level0=1, kernel=kernel)
+    b, ib = run_gpu(cfg, 33, via="run", level0=1, kernel=kernel)
+    assert ia["kernel"] == ib["kernel"] and ia["launches"] >= ib["launches"]
+    np.testing.assert_array_equal(a, b)
