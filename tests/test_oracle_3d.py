@@ -88,3 +88,19 @@ def test_convergence_to_the_closed_form(oracle):
         u = oracle.run_3d(u0, 1.0, steps)
         errs.append(float(np.abs(u - np.exp(-3 * np.pi ** 2 * t) * u0).max()))
     assert errs[0] / errs[1] > 3.0 and errs[1] / errs[2] > 3.3, errs
+
+
+def test_exact_rational_fixture(oracle):
+    """tests/golden/p11_3d_exact.txt: two levels in exact rationals from the implicit statement."""
+    from conftest import golden_lines
+    for ln in golden_lines("p11_3d_exact.txt"):
+        head, bc, u0, u1, u2 = [p.strip() for p in ln.split(";")]
+        n, r = int(head.split()[0]), float(F(head.split()[1]))
+        bc = tuple(float(F(t)) for t in bc.split())
+        a0 = np.array([float(F(t)) for t in u0.split()]).reshape(n, n, n)
+        a1 = np.array([float(F(t)) for t in u1.split()]).reshape(n, n, n)
+        a2 = np.array([float(F(t)) for t in u2.split()]).reshape(n, n, n)
+        g1 = oracle.level_3d(a0, r, 0, bc)
+        np.testing.assert_allclose(g1, a1, rtol=0, atol=1e-12)
+        np.testing.assert_allclose(oracle.level_3d(g1, r, 1, bc), a2, rtol=0, atol=1e-12)
+        np.testing.assert_allclose(oracle.run_3d(a0, r, 2, bc), a2, rtol=0, atol=1e-12)

@@ -75,3 +75,18 @@ def test_manufactured_solution_converges_at_second_order(oracle):
     errs = [_manufactured(oracle, n, 1.0, 0.1) for n in (31, 63, 127)]
     assert errs[0] / errs[1] > 3.5 and errs[1] / errs[2] > 3.5, errs
     assert errs[2] < 3e-4
+
+
+def test_exact_rational_fixture(oracle):
+    """tests/golden/p12_src_exact.txt: two levels with a source term and moving boundary values, exact rationals."""
+    from fractions import Fraction as F
+    from conftest import golden_lines
+    for ln in golden_lines("p12_src_exact.txt"):
+        head, lo, hi, u0, s1, s2, u1, u2 = [p.strip() for p in ln.split(";")]
+        k, r = int(head.split()[0]), float(F(head.split()[1]))
+        vec = lambda t: np.array([float(F(x)) for x in t.split()])
+        lo, hi, u0, s1, s2, u1, u2 = map(vec, (lo, hi, u0, s1, s2, u1, u2))
+        g1 = oracle.level_1d_src(u0, r, 0, (lo[0], hi[0]), (lo[1], hi[1]), s1, k=k)
+        np.testing.assert_allclose(g1, u1, rtol=0, atol=1e-13)
+        g2 = oracle.level_1d_src(g1, r, 1, (lo[1], hi[1]), (lo[2], hi[2]), s2, k=k)
+        np.testing.assert_allclose(g2, u2, rtol=0, atol=1e-13)
