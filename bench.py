@@ -264,7 +264,7 @@ def run_ours(args):
     if args.hl:
         plan.tune(libge.GE_TUNE_HALO_LANES, args.hl)
     if args.sync:
-        plan.tune(libge.GE_TUNE_SYNC_MODE, {"flags": libge.GE_SYNC_FLAGS, "grid": libge.GE_SYNC_GRID, "lines": libge.GE_SYNC_LINES}[args.sync])
+        plan.tune(libge.GE_TUNE_SYNC_MODE, {"flags": libge.GE_SYNC_FLAGS, "grid": libge.GE_SYNC_GRID, "lines": libge.GE_SYNC_LINES, "stagger": libge.GE_SYNC_STAGGER}[args.sync])
     if args.rtb:
         plan.tune(libge.GE_TUNE_TB, args.rtb)
     info0 = plan.info()
@@ -513,7 +513,7 @@ def main():
     ap.add_argument("--rc", type=int, default=0, help="persistent kernels: values per lane")
     ap.add_argument("--hl", type=int, default=0, help="whole-chip persistent kernel: halo lanes per side")
     ap.add_argument("--rtb", type=int, default=0, help="whole-chip persistent kernel: levels between meetings")
-    ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines"], help="whole-chip persistent kernel: meeting kind")
+    ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines", "stagger"], help="whole-chip persistent kernel: meeting kind")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
     ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")

@@ -168,7 +168,9 @@ enum {
     GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */
     GE_TUNE_SYNC_MODE = 5      /* path 2, how the tiles meet: 0 = neighbour flags (data, release fence, flag per
                                   tile, acquire), 1 = grid-wide barrier (cooperative groups), 2 = neighbour
-                                  flag-in-data lines (no fence, no separate flag); default 1, the fastest measured               */
+                                  flag-in-data lines (no fence, no separate flag), 3 = the same lines published
+                                  every tb/2 levels and consumed every other time, the CTAs that share an SM
+                                  taking opposite turns (needs tb >= 8); default 1, the fastest measured            */
 };
 int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
 

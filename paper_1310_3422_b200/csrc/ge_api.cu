@@ -480,11 +480,12 @@ int grid_resident_configure(ge_plan* p) {
     cudaFree(p->res_xbuf); cudaFree(p->res_flags);
     p->res_xbuf = nullptr; p->res_flags = nullptr;
     // sized for the flag-in-data lines: 16 bytes per fp64 value (8 per fp32 value)
-    const size_t xb = (size_t)2 * tiles * 2 * p->res_hl * p->res_c * 2 * elem_size(p->dtype);
+    const size_t xb = (size_t)ge::kLineSlots * tiles * 2 * p->res_hl * p->res_c * 2 * elem_size(p->dtype);
     GE_CUDA(cudaMalloc(&p->res_xbuf, xb));
     GE_CUDA(cudaMemset(p->res_xbuf, 0, xb));
-    GE_CUDA(cudaMalloc((void**)&p->res_flags, (size_t)(tiles + 1) * sizeof(unsigned)));
-    GE_CUDA(cudaMemset(p->res_flags, 0, (size_t)(tiles + 1) * sizeof(unsigned)));
+    // flags[tiles], the fault word, and 256 per-SM arrival counters of the staggered mode
+    GE_CUDA(cudaMalloc((void**)&p->res_flags, (size_t)(tiles + 1 + 256) * sizeof(unsigned)));
+    GE_CUDA(cudaMemset(p->res_flags, 0, (size_t)(tiles + 1 + 256) * sizeof(unsigned)));
     p->res_epoch = 0;
     p->res_tiles = tiles;
     p->res_tb = tb;
@@ -500,6 +501,8 @@ int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     void* coef = p->coef;
     unsigned* flags = p->res_flags;
     unsigned* fault = p->res_flags + p->res_tiles;
+    if (p->res_sync == ge::kSyncStagger)
+        GE_CUDA(cudaMemsetAsync(p->res_flags + p->res_tiles + 1, 0, 256 * sizeof(unsigned), s));
     void* args[] = {&u, &xbuf, &coef, &flags, &fault, &a};
     const void* fn = grid_resident_fn_for(p->dtype, p->res_c);
     const unsigned ctas = (unsigned)((p->res_tiles + ge::kGridWarps - 1) / ge::kGridWarps);
@@ -508,7 +511,7 @@ int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     const int64_t meet = ge::grid_resident_meetings(steps, a.phase0, a.tb);
     // every launch moves the epoch past all flag values / line tags it used (one extra meeting is held
     // by the flag-in-data mode when the run has none)
-    p->res_epoch += (unsigned)(2 + meet);
+    p->res_epoch += (unsigned)(2 + (p->res_sync == ge::kSyncStagger ? ge::grid_resident_halves(steps, a.phase0, a.tb) : meet));
     p->meetings += meet;
     p->launches += 1;
     p->level += steps;
@@ -1008,7 +1011,8 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         }
         case GE_TUNE_SYNC_MODE:
             if (p->kernel != GE_KERNEL_PERSISTENT || p->res_path != 2) return GE_EINVAL;
-            if (value != ge::kSyncFlags && value != ge::kSyncGrid && value != ge::kSyncLL) return GE_EINVAL;
+            if (value < ge::kSyncFlags || value > ge::kSyncStagger) return GE_EINVAL;
+            if (value == ge::kSyncStagger && p->res_tb < 8) return GE_EINVAL;
             p->res_sync = (int32_t)value;
             return GE_OK;
         case GE_TUNE_TB:
@@ -1016,7 +1020,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             if (p->kernel == GE_KERNEL_PERSISTENT && p->res_path == 2) {
                 int64_t tb = value > (int64_t)p->res_hl * p->res_c ? (int64_t)p->res_hl * p->res_c : value;
                 tb -= tb % 2;
-                if (tb < 2) return GE_EINVAL;
+                if (tb < 2 || (p->res_sync == ge::kSyncStagger && tb < 8)) return GE_EINVAL;
                 p->res_tb = (int32_t)tb;
                 return GE_OK;
             }

@@ -281,8 +281,10 @@ inline cudaError_t rod_resident_launch(T* u, int64_t nx, int64_t batch, const Co
 // ------------------------------------------------------------------ (ii) one rod on the whole chip ------
 constexpr int kGridWarps = 4;              // warps (tiles) per CTA
 // how the tiles meet: 0 = per-tile flag with a release fence (neighbours only), 1 = grid-wide barrier,
-// 2 = flag-in-data lines, no fence and no separate flag (neighbours only; the default)
-constexpr int kSyncFlags = 0, kSyncGrid = 1, kSyncLL = 2;
+// 2 = flag-in-data lines, no fence and no separate flag (neighbours only), 3 = the same, published every
+// tb/2 levels and consumed in opposite turns by the CTAs that share an SM
+constexpr int kSyncFlags = 0, kSyncGrid = 1, kSyncLL = 2, kSyncStagger = 3;
+constexpr int kLineSlots = 4;          // exchange slots of the flag-in-data modes (2 are used by kSyncLL)
 
 struct GridResidentArgs {
     int64_t nx;
@@ -306,6 +308,20 @@ __host__ __device__ inline int64_t grid_resident_meetings(int64_t steps, int pha
     }
     if (left) { if (usedl + 2 > tb) { ++n; usedl = 0; } }
     return n;
+}
+
+// publications of a staggered run (the same loop as in the kernel) + the final one
+__host__ __device__ inline int64_t grid_resident_halves(int64_t steps, int phase0, int tb) {
+    const int tbh = tb / 2 - (tb / 2) % 2;
+    int64_t left = steps, n = 0;
+    int usedh = 0;
+    if (phase0 == 0 && left > 0) { usedh = 2; --left; }
+    while (left >= 2) {
+        if (usedh + 2 > tbh) { ++n; usedh = 0; }
+        usedh += 2; left -= 2;
+    }
+    if (left) { if (usedh + 2 > tbh) { ++n; usedh = 0; } }
+    return n + 1;
 }
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -408,7 +424,7 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
     const size_t side = (size_t)hl * C;                               // elements per published side
     auto signal = [&]() {
         if (a.sync_mode == kSyncGrid) { grid.sync(); return; }
-        if (a.sync_mode == kSyncLL || !active) return;
+        if (a.sync_mode == kSyncLL || a.sync_mode == kSyncStagger || !active) return;
         // release: the warp's stores are ordered before lane 0's fence by __syncwarp, the fence is cumulative
         __syncwarp();
         if (lane == 0) { __threadfence(); st_relaxed_u32(flags + tile, stage); }
@@ -424,47 +440,54 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
 
     int parity = 0;
     constexpr int NQ = C / Line<T>::per;                              // lines per lane
-    auto meet_lines = [&]() {
-        // flag-in-data: publish tagged lines, then poll the neighbours' lines until every tag matches
-        ++stage;
-        if (active) {
-            uint4* xl = reinterpret_cast<uint4*>(xbuf);
-            const size_t lside = (size_t)hl * NQ;
-            if (own_l || own_r) {
-                uint4* dst = xl + ((size_t)parity * a.ntiles + tile) * 2 * lside +
-                             (own_l ? (size_t)(lane - hl) * NQ : lside + (size_t)(lane - (32 - 2 * hl)) * NQ);
+    // flag-in-data: publish tagged lines into slot `slot` (of kLineSlots); consume = poll the neighbours' lines
+    // of that slot until every tag matches
+    auto publish_lines = [&](int slot, unsigned tag) {
+        if (!active || !(own_l || own_r)) return;
+        uint4* xl = reinterpret_cast<uint4*>(xbuf);
+        const size_t lside = (size_t)hl * NQ;
+        uint4* dst = xl + ((size_t)slot * a.ntiles + tile) * 2 * lside +
+                     (own_l ? (size_t)(lane - hl) * NQ : lside + (size_t)(lane - (32 - 2 * hl)) * NQ);
 #pragma unroll
-                for (int j = 0; j < NQ; ++j) Line<T>::put(dst + j, &v[j * Line<T>::per], stage);
+        for (int j = 0; j < NQ; ++j) Line<T>::put(dst + j, &v[j * Line<T>::per], tag);
+    };
+    auto consume_lines = [&](int slot, unsigned tag) {
+        if (!active) return;
+        const uint4* xl = reinterpret_cast<const uint4*>(xbuf);
+        const size_t lside = (size_t)hl * NQ;
+        const uint4* src = nullptr;
+        if (halo_l && has_l)
+            src = xl + ((size_t)slot * a.ntiles + tile - 1) * 2 * lside + lside + (size_t)lane * NQ;
+        else if (halo_r && has_r)
+            src = xl + ((size_t)slot * a.ntiles + tile + 1) * 2 * lside + (size_t)(lane - (32 - hl)) * NQ;
+        if (src) {
+            uint4 q[NQ];
+            bool ok = false;
+            // watch the line written last with a back-off (a spinning lane would take issue slots from
+            // the warp that shares this scheduler and is still computing), then fetch all of them
+            for (unsigned it = 0; it < (1u << 22); ++it) {
+                const uint4 w = ld_line(src + NQ - 1);
+                if (w.y == tag && w.w == tag) break;
+                __nanosleep(it < 64 ? 20 : 200);
             }
-            const uint4* src = nullptr;
-            if (halo_l && has_l)
-                src = xl + ((size_t)parity * a.ntiles + tile - 1) * 2 * lside + lside + (size_t)lane * NQ;
-            else if (halo_r && has_r)
-                src = xl + ((size_t)parity * a.ntiles + tile + 1) * 2 * lside + (size_t)(lane - (32 - hl)) * NQ;
-            if (src) {
-                uint4 q[NQ];
-                bool ok = false;
-                // watch the line written last with a back-off (a spinning lane would take issue slots from
-                // the warp that shares this scheduler and is still computing), then fetch all of them
-                for (unsigned it = 0; it < (1u << 22); ++it) {
-                    const uint4 w = ld_line(src + NQ - 1);
-                    if (w.y == stage && w.w == stage) break;
-                    __nanosleep(it < 64 ? 20 : 200);
-                }
-                for (unsigned it = 0; it < (1u << 20) && !ok; ++it) {
+            for (unsigned it = 0; it < (1u << 20) && !ok; ++it) {
 #pragma unroll
-                    for (int j = 0; j < NQ; ++j) q[j] = ld_line(src + j);
-                    ok = true;
+                for (int j = 0; j < NQ; ++j) q[j] = ld_line(src + j);
+                ok = true;
 #pragma unroll
-                    for (int j = 0; j < NQ; ++j) ok = ok && q[j].y == stage && q[j].w == stage;
-                    if (!ok) __nanosleep(100);
-                }
-                if (!ok) atomicExch(fault, 1u);
-#pragma unroll
-                for (int j = 0; j < NQ; ++j) Line<T>::get(q[j], &v[j * Line<T>::per]);
+                for (int j = 0; j < NQ; ++j) ok = ok && q[j].y == tag && q[j].w == tag;
+                if (!ok) __nanosleep(100);
             }
-            __syncwarp();
+            if (!ok) atomicExch(fault, 1u);
+#pragma unroll
+            for (int j = 0; j < NQ; ++j) Line<T>::get(q[j], &v[j * Line<T>::per]);
         }
+        __syncwarp();
+    };
+    auto meet_lines = [&]() {
+        ++stage;
+        publish_lines(parity, stage);
+        consume_lines(parity, stage);
         parity ^= 1;
     };
     auto meet = [&]() {
@@ -504,6 +527,59 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
         }
         parity ^= 1;
     };
+
+    if (a.sync_mode == kSyncStagger) {
+        // Staggered flag-in-data meetings.  Every tile publishes its edge lanes every tb/2 levels, but refreshes
+        // its own halo only every second time: the two CTAs that share an SM take opposite turns (the turn is
+        // the order in which they arrived on the SM), so while one warp of a scheduler waits for its neighbours'
+        // lines the other one computes.  Any assignment of turns is correct -- a tile only ever reads lines of
+        // the level it is at.
+        __shared__ int turn_s;
+        if (threadIdx.x == 0) {
+            unsigned smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            turn_s = (int)(atomicAdd(flags + a.ntiles + 1 + (smid & 255u), 1u) & 1u);
+        }
+        __syncthreads();
+        const int turn = turn_s;
+        const int tbh = a.tb / 2 - (a.tb / 2) % 2;             // levels between two publications (even)
+        int64_t left = a.steps;
+        int usedh = 0, h = 0;
+        auto half = [&]() {
+            const unsigned tag = a.epoch0 + 1 + (unsigned)h;
+            publish_lines(h & (kLineSlots - 1), tag);
+            if ((h & 1) != turn) consume_lines(h & (kLineSlots - 1), tag);
+            ++h; usedh = 0;
+        };
+        if (a.phase0 == 0 && left > 0) { level_I<T, C, false>(v, c, 0); usedh = 2; --left; }
+#pragma unroll 1
+        while (left >= 2) {
+            if (usedh + 2 > tbh) half();
+            level_R<T, C, false>(v, x0, c, 0);
+            level_L<T, C, false>(v, x0, c, 0);
+            usedh += 2; left -= 2;
+        }
+        if (left) {
+            if (usedh + 2 > tbh) half();
+            level_R<T, C, false>(v, x0, c, 0);
+            unshift<T, C, false>(v, x0, c, 0);
+        }
+        {   // before u is overwritten every neighbour must have loaded it: one last exchange that everybody consumes
+            const unsigned tag = a.epoch0 + 1 + (unsigned)h;
+            publish_lines(h & (kLineSlots - 1), tag);
+            consume_lines(h & (kLineSlots - 1), tag);
+        }
+        if (inside && lane >= hl && lane < 32 - hl) {
+#pragma unroll
+            for (int j = 0; j < C / V; ++j) {
+                T t[V];
+#pragma unroll
+                for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
+                st_vec(u + e0 + j * V, t);
+            }
+        }
+        return;
+    }
 
     int64_t left = a.steps;
     int usedl = 0;

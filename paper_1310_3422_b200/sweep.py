@@ -37,7 +37,7 @@ def main():
     stream = stream_obj.cuda_stream
     u0 = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
     sync_names = {libge.GE_SYNC_FLAGS: "flag + fence", libge.GE_SYNC_GRID: "grid barrier",
-                  libge.GE_SYNC_LINES: "flag-in-data"}
+                  libge.GE_SYNC_LINES: "flag-in-data", libge.GE_SYNC_STAGGER: "staggered flag-in-data"}
     settings = [("A: launch per level", dict(kernel="per_step"), {}),
                 ("B: warp-per-tile, tb 16", dict(kernel="temporal", tb=16), {libge.GE_TUNE_TEMPORAL_C: 16}),
                 ("B: TMA-staged, tb 20", dict(kernel="temporal", tb=20), {})]
@@ -52,6 +52,10 @@ def main():
             settings.append(("C: C=32, halo 2, %s, tb %d" % (sync_names[sync], tb), dict(kernel="persistent"),
                              {libge.GE_TUNE_RESIDENT_C: 32, libge.GE_TUNE_HALO_LANES: 2,
                               libge.GE_TUNE_SYNC_MODE: sync, libge.GE_TUNE_TB: tb}))
+    for c, hl in ((32, 2), (32, 1), (64, 2)):
+        settings.append(("C: C=%d, halo %d, %s" % (c, hl, sync_names[libge.GE_SYNC_STAGGER]), dict(kernel="persistent"),
+                         {libge.GE_TUNE_RESIDENT_C: c, libge.GE_TUNE_HALO_LANES: hl,
+                          libge.GE_TUNE_SYNC_MODE: libge.GE_SYNC_STAGGER}))
     rows, first = [], None
     for name, kw, tune in settings:
         try:

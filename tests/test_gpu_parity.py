@@ -152,10 +152,13 @@ def test_persistent_rods(oracle, dtype, n, rc):
     ("f64", 100000, 0, 2, 0, None), ("f64", 100000, 16, 3, 10, 1), ("f64", 2 ** 20, 0, 0, 0, None),
     ("f64", 2 ** 20, 0, 0, 0, 1), ("f64", 2 ** 20, 0, 0, 0, 0), ("f64", 30720, 0, 2, 4, 0),
     ("f32", 16384 * 4, 0, 0, 0, 2), ("f32", 16384 * 4, 0, 1, 8, 0), ("f32", 2 ** 20, 128, 1, 0, 2), ("f32", 200000 - 200000 % 64, 32, 2, 20, None),
-    ("f32", 2 ** 20, 0, 0, 0, 1)])
+    ("f32", 2 ** 20, 0, 0, 0, 1),
+    ("f64", 2 ** 20, 0, 0, 0, 3), ("f64", 30720, 0, 1, 8, 3), ("f64", 100000, 16, 3, 10, 3), ("f32", 16384 * 4, 0, 0, 0, 3),
+    ("f32", 2 ** 20, 128, 1, 0, 3)])
 def test_persistent_whole_chip(oracle, dtype, n, rc, hl, rtb, sync):
     """Strategy C, path 2 (one rod spread over the chip by a cooperative launch, tiles meet every tb
-    levels): grid-wide barrier (default), neighbour flags (sync=0) and flag-in-data lines (sync=2), one
+    levels): grid-wide barrier (default), neighbour flags (sync=0), flag-in-data lines (sync=2) and
+    staggered flag-in-data lines (sync=3: published every tb/2 levels, consumed every other time), one
     and several halo lanes, many meetings, no
     meeting, ragged last tile, both starting phases, odd level counts, and several ge_run calls on
     one plan (the flag epoch carries over).  Must equal the per-level kernel bit for bit."""
