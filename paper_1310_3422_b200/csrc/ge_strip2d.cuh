@@ -89,63 +89,64 @@ __device__ __forceinline__ void solve2(T r1, T r2, T beta, T h1, T h3, T& n1, T&
     n2 = fma(h3, df, fma(-h1, s, r2));
 }
 
-// right-hand sides of the columns in slots 2m (right members b, d of the group to the left) and
-// 2m+1 (left members a, c) for the group rows (P1, Q0); P0 / Q1 are the rows below / above
+// Right-hand sides a row pair X = (X0, X1) contributes to the columns in slots 2m (right members b, d
+// of the group to the left) and 2m+1 (left members a, c).  The pair is the UPPER half of the group row
+// (j, j+1) = (previous pair's row 1, X0): Rd[m], Rc[m] (members d, c in row X0, X1 the row above) --
+// and, one iteration later, the LOWER half of the group row (X1, next pair's row 0): H[2m] = Rb[m],
+// H[2m+1] = Ra[m] (members b, a in row X1, X0 the row below).  Both halves read nothing but this pair,
+// so they are formed together when the pair passes (the y differences are shared) and only H -- one
+// value per column instead of the two rows -- waits in the stage's state slot for the next pair.
 template <typename T, int C>
-__device__ __forceinline__ void strip_rhs(const T (&P0)[C], const T (&P1)[C], const T (&Q0)[C], const T (&Q1)[C],
-                                          T r, T (&Ra)[C / 2], T (&Rb)[C / 2], T (&Rc)[C / 2], T (&Rd)[C / 2]) {
+__device__ __forceinline__ void strip_rhs_pair(const T (&X0)[C], const T (&X1)[C], T r, T (&H)[C],
+                                               T (&Rc)[C / 2], T (&Rd)[C / 2]) {
 #pragma unroll
     for (int m = 0; m < C / 2; ++m) {
-        const T exP = P1[2 * m + 1] - P1[2 * m];
-        const T exQ = Q0[2 * m + 1] - Q0[2 * m];
-        const T eyLb = P1[2 * m] - P0[2 * m], eyLa = P1[2 * m + 1] - P0[2 * m + 1];
-        const T eyHd = Q1[2 * m] - Q0[2 * m], eyHc = Q1[2 * m + 1] - Q0[2 * m + 1];
-        Rb[m] = fma(r, exP - eyLb, P1[2 * m]);          // right + below
-        Rd[m] = fma(r, exQ + eyHd, Q0[2 * m]);          // right + above
-        Ra[m] = fma(-r, exP + eyLa, P1[2 * m + 1]);     // left + below
-        Rc[m] = fma(r, eyHc - exQ, Q0[2 * m + 1]);      // left + above
+        const T ex1 = X1[2 * m + 1] - X1[2 * m];
+        const T ex0 = X0[2 * m + 1] - X0[2 * m];
+        const T eyb = X1[2 * m] - X0[2 * m], eya = X1[2 * m + 1] - X0[2 * m + 1];
+        H[2 * m] = fma(r, ex1 - eyb, X1[2 * m]);              // Rb: right + below
+        H[2 * m + 1] = fma(-r, ex1 + eya, X1[2 * m + 1]);     // Ra: left + below
+        Rd[m] = fma(r, ex0 + eyb, X0[2 * m]);                 // right + above
+        Rc[m] = fma(r, eya - ex0, X0[2 * m + 1]);             // left + above
     }
 }
 
-// R: unshifted rows -> rows shifted right by one column.  N0 / N1 are the new rows of P1 / Q0;
+// R: unshifted rows -> rows shifted right by one column.  H: lower-half right-hand sides left by the
+// previous pair, Rc / Rd: upper half from the current pair.  N0 / N1 are the new rows of the group row;
 // nx0[0..1]: new column 0 of those rows (lane is_lo only).
 template <typename T, int C, bool BC>
-__device__ __forceinline__ void strip_stage_R(const T (&P0)[C], const T (&P1)[C], const T (&Q0)[C],
-                                              const T (&Q1)[C], T (&N0)[C], T (&N1)[C], T (&nx0)[2],
-                                              const Strip2dCtx<T>& k) {
+__device__ __forceinline__ void strip_stage_R(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                              T (&N0)[C], T (&N1)[C], T (&nx0)[2], const Strip2dCtx<T>& k) {
     constexpr unsigned FULL = 0xffffffffu;
-    T Ra[C / 2], Rb[C / 2], Rc[C / 2], Rd[C / 2];
-    strip_rhs<T, C>(P0, P1, Q0, Q1, k.r, Ra, Rb, Rc, Rd);
-    const T RbN = __shfl_down_sync(FULL, Rb[0], 1);
+    const T RbN = __shfl_down_sync(FULL, H[0], 1);
     const T RdN = __shfl_down_sync(FULL, Rd[0], 1);
 #pragma unroll
     for (int m = 0; m < C / 2; ++m) {
-        const T rb = m + 1 < C / 2 ? Rb[m + 1] : RbN;
-        const T rd = m + 1 < C / 2 ? Rd[m + 1] : RdN;
+        const T ra = H[2 * m + 1];
+        const T rb = m + 1 < C / 2 ? H[2 * m + 2 < C ? 2 * m + 2 : 0] : RbN;
+        const T rd = m + 1 < C / 2 ? Rd[m + 1 < C / 2 ? m + 1 : 0] : RdN;
         T na, nb, nc, nd;
-        solve4(Ra[m], rb, Rc[m], rd, k.g2, k.g4, na, nb, nc, nd);
+        solve4(ra, rb, Rc[m], rd, k.g2, k.g4, na, nb, nc, nd);
         if constexpr (BC) {
             if (m == C / 2 - 1 && k.is_hi) {       // members b, d are the boundary column x = nx
-                solve2(Ra[m], Rc[m], k.xhi, k.h1, k.h3, na, nc);
+                solve2(ra, Rc[m], k.xhi, k.h1, k.h3, na, nc);
                 nb = k.xhi; nd = k.xhi;
             }
         }
         N0[2 * m] = na; N0[2 * m + 1] = nb;
         N1[2 * m] = nc; N1[2 * m + 1] = nd;
     }
-    if constexpr (BC) solve2(Rb[0], Rd[0], k.xlo, k.h1, k.h3, nx0[0], nx0[1]);   // group (x = -1, 0)
+    if constexpr (BC) solve2(H[0], Rd[0], k.xlo, k.h1, k.h3, nx0[0], nx0[1]);   // group (x = -1, 0)
 }
 
-// L: rows shifted right by one column -> unshifted rows.  pP / pQ: column 0 of the rows
-// P0, P1 / Q0, Q1 (lane is_lo only).
+// L: rows shifted right by one column -> unshifted rows.  pP / pQ: column 0 of the previous pair's /
+// the current pair's rows (lane is_lo only).
 template <typename T, int C, bool BC>
-__device__ __forceinline__ void strip_stage_L(const T (&P0)[C], const T (&P1)[C], const T (&Q0)[C],
-                                              const T (&Q1)[C], const T (&pP)[2], const T (&pQ)[2],
+__device__ __forceinline__ void strip_stage_L(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                              const T (&pP)[2], const T (&pQ)[2],
                                               T (&N0)[C], T (&N1)[C], const Strip2dCtx<T>& k) {
     constexpr unsigned FULL = 0xffffffffu;
-    T Ra[C / 2], Rb[C / 2], Rc[C / 2], Rd[C / 2];
-    strip_rhs<T, C>(P0, P1, Q0, Q1, k.r, Ra, Rb, Rc, Rd);
-    T ra = __shfl_up_sync(FULL, Ra[C / 2 - 1], 1);
+    T ra = __shfl_up_sync(FULL, H[C - 1], 1);
     T rc = __shfl_up_sync(FULL, Rc[C / 2 - 1], 1);
     if constexpr (BC) {
         if (k.is_lo) {     // members a, c are column 0; their left neighbour is the boundary column
@@ -154,11 +155,11 @@ __device__ __forceinline__ void strip_stage_L(const T (&P0)[C], const T (&P1)[C]
             rc = fma(k.r, (pQ[1] - c) - (c - k.xlo), c);
         }
     }
-    solve4(ra, Rb[0], rc, Rd[0], k.g2, k.g4, N0[0], N0[1], N1[0], N1[1]);
+    solve4(ra, H[0], rc, Rd[0], k.g2, k.g4, N0[0], N0[1], N1[0], N1[1]);
 #pragma unroll
     for (int m = 0; m + 1 < C / 2; ++m)
-        solve4(Ra[m], Rb[m + 1], Rc[m], Rd[m + 1], k.g2, k.g4, N0[2 * m + 2], N0[2 * m + 3], N1[2 * m + 2],
-               N1[2 * m + 3]);
+        solve4(H[2 * m + 1], H[2 * m + 2], Rc[m], Rd[m + 1], k.g2, k.g4, N0[2 * m + 2], N0[2 * m + 3],
+               N1[2 * m + 2], N1[2 * m + 3]);
 }
 
 // Generic stage for the few stage-iterations whose group rows (j, j+1) are not both interior
@@ -239,38 +240,35 @@ __device__ __noinline__ void strip_stage_slow(T* __restrict__ io, const Coef2<T>
     for (int s = 0; s < 2 * C + 2; ++s) io[s] = o[s];
 }
 
-// One stage of the pipeline: P = previous row pair of level l (with its column 0: xP), Q = current
-// one; writes the level-(l+1) pair into N (xN).  Odd stages are L, even stages R.
-// (`odd` is a constant after the stage loop is unrolled.)
+// One EDGE stage-iteration (group rows j, j+1 not both interior): P = previous row pair of level l (with
+// its column 0: xP), Q = current one, both raw; writes the level-(l+1) pair into N (xN).  Odd stages are
+// L, even stages R.
 template <typename T, int C, bool BC>
-__device__ __forceinline__ void strip_stage(const bool odd, const T (&P)[2][C], const T (&xP)[2],
-                                            const T (&Q)[2][C], const T (&xQ)[2], T (&N)[2][C], T (&xN)[2],
-                                            const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int j,
-                                            int ny) {
-    if ((unsigned)j < (unsigned)(ny - 1)) {          // group rows j, j+1 both interior: the fast stage
-        if (odd) strip_stage_L<T, C, BC>(P[0], P[1], Q[0], Q[1], xP, xQ, N[0], N[1], k);
-        else     strip_stage_R<T, C, BC>(P[0], P[1], Q[0], Q[1], N[0], N[1], xN, k);
-    } else {
-        T io[4 * C + 4];
+__device__ __forceinline__ void strip_stage_rows(const bool odd, const T (&P)[2][C], const T (&xP)[2],
+                                                 const T (&Q)[2][C], const T (&xQ)[2], T (&N)[2][C], T (&xN)[2],
+                                                 const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int j,
+                                                 int ny) {
+    T io[4 * C + 4];
 #pragma unroll
-        for (int s = 0; s < C; ++s) {
-            io[s] = P[0][s]; io[C + s] = P[1][s]; io[2 * C + s] = Q[0][s]; io[3 * C + s] = Q[1][s];
-        }
-        io[4 * C] = xP[0]; io[4 * C + 1] = xP[1]; io[4 * C + 2] = xQ[0]; io[4 * C + 3] = xQ[1];
-        const int yg = j == -1 ? 1 : (j + 1 == ny ? 2 : 0);
-        if (odd) strip_stage_slow<T, C, true>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
-        else     strip_stage_slow<T, C, false>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
-#pragma unroll
-        for (int s = 0; s < C; ++s) { N[0][s] = io[s]; N[1][s] = io[C + s]; }
-        if (!odd) { xN[0] = io[2 * C]; xN[1] = io[2 * C + 1]; }
+    for (int s = 0; s < C; ++s) {
+        io[s] = P[0][s]; io[C + s] = P[1][s]; io[2 * C + s] = Q[0][s]; io[3 * C + s] = Q[1][s];
     }
+    io[4 * C] = xP[0]; io[4 * C + 1] = xP[1]; io[4 * C + 2] = xQ[0]; io[4 * C + 3] = xQ[1];
+    const int yg = j == -1 ? 1 : (j + 1 == ny ? 2 : 0);
+    if (odd) strip_stage_slow<T, C, true>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
+    else     strip_stage_slow<T, C, false>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
+#pragma unroll
+    for (int s = 0; s < C; ++s) { N[0][s] = io[s]; N[1][s] = io[C + s]; }
+    if (!odd) { xN[0] = io[2 * C]; xN[1] = io[2 * C + 1]; }
 }
 
-// The pipeline state -- the previous row pair of every level 0 .. TB-1 -- lives in SHARED memory, in
-// lane-private slots (vector c of lane t at [(c*32 + t)*V], conflict-free, no synchronisation): stage l
-// loads its previous pair, computes, and stores the current pair in its place.  Registers hold only
-// the pair that flows through the stages and the row pairs in flight from HBM, so 20+ warps fit on
-// an SM and nothing rotates through register moves.
+// The pipeline state of every level 0 .. TB-1 lives in SHARED memory, in lane-private slots (vector c of
+// lane t at [(c*32 + t)*V], conflict-free, no synchronisation).  What a stage keeps between two iterations
+// is what the previous pair contributes to the next group row: its lower-half right-hand sides H (one value
+// per column, strip_rhs_pair) -- or, when the next group row touches a y edge and takes the generic path,
+// the raw pair (two rows; the same slot, the choice is warp-uniform and both sides derive it from j).
+// Registers hold only the pair that flows through the stages, so 12+ warps fit on an SM and nothing
+// rotates through register moves; shared-memory traffic per stage-iteration is one row in, one row out.
 template <typename T, int C>
 __device__ __forceinline__ void strip_lds(const T* __restrict__ sp, int lane, T (&v)[2][C]) {
     constexpr int V = VecOf<T>::V;
@@ -297,6 +295,31 @@ __device__ __forceinline__ void strip_sts(T* __restrict__ sp, int lane, const T 
             else { q.x = v[rr][c * V]; q.y = v[rr][c * V + 1]; }
             *reinterpret_cast<VT*>(sp + ((rr * (C / V) + c) * 32 + lane) * V) = q;
         }
+}
+
+// one row (the H values) in the first half of a state slot
+template <typename T, int C>
+__device__ __forceinline__ void strip_lds_half(const T* __restrict__ sp, int lane, T (&v)[C]) {
+    constexpr int V = VecOf<T>::V;
+    using VT = typename VecOf<T>::type;
+#pragma unroll
+    for (int c = 0; c < C / V; ++c) {
+        const VT q = *reinterpret_cast<const VT*>(sp + (c * 32 + lane) * V);
+        if constexpr (V == 4) { v[c * V] = q.x; v[c * V + 1] = q.y; v[c * V + 2] = q.z; v[c * V + 3] = q.w; }
+        else { v[c * V] = q.x; v[c * V + 1] = q.y; }
+    }
+}
+template <typename T, int C>
+__device__ __forceinline__ void strip_sts_half(T* __restrict__ sp, int lane, const T (&v)[C]) {
+    constexpr int V = VecOf<T>::V;
+    using VT = typename VecOf<T>::type;
+#pragma unroll
+    for (int c = 0; c < C / V; ++c) {
+        VT q;
+        if constexpr (V == 4) { q.x = v[c * V]; q.y = v[c * V + 1]; q.z = v[c * V + 2]; q.w = v[c * V + 3]; }
+        else { q.x = v[c * V]; q.y = v[c * V + 1]; }
+        *reinterpret_cast<VT*>(sp + (c * 32 + lane) * V) = q;
+    }
 }
 
 // Row pairs travel HBM -> shared memory with cp.async (16 bytes per lane, lane-private slots, so the
@@ -381,10 +404,25 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
         strip_lds<T, C>(ring + (it % kStripRing) * kPair, lane, cur);
 #pragma unroll
         for (int l = 0; l < TB; ++l) {
-            T P[2][C], N[2][C], nx0[2] = {T(0), T(0)};
-            strip_lds<T, C>(sp + l * kPair, lane, P);
-            strip_stage<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, y0 - 1 - l, ny);
-            strip_sts<T, C>(sp + l * kPair, lane, cur);
+            const int j = y0 - 1 - l;                                          // group rows j, j+1
+            const bool fast = (unsigned)j < (unsigned)(ny - 1);                // both interior
+            const bool next_fast = (unsigned)(j + 2) < (unsigned)(ny - 1);     // this stage, next iteration
+            T* slot = sp + l * kPair;
+            T N[2][C], nx0[2] = {T(0), T(0)};
+            T Hn[C], Rc[C / 2], Rd[C / 2];
+            strip_rhs_pair<T, C>(cur[0], cur[1], k.r, Hn, Rc, Rd);
+            if (fast) {
+                T H[C];
+                strip_lds_half<T, C>(slot, lane, H);
+                if ((l & 1) != 0) strip_stage_L<T, C, BC>(H, Rc, Rd, px[l], cx, N[0], N[1], k);
+                else              strip_stage_R<T, C, BC>(H, Rc, Rd, N[0], N[1], nx0, k);
+            } else {
+                T P[2][C];
+                strip_lds<T, C>(slot, lane, P);
+                strip_stage_rows<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, j, ny);
+            }
+            if (next_fast) strip_sts_half<T, C>(slot, lane, Hn);
+            else           strip_sts<T, C>(slot, lane, cur);
 #pragma unroll
             for (int s = 0; s < C; ++s) { cur[0][s] = N[0][s]; cur[1][s] = N[1][s]; }
             if constexpr (BC) { px[l][0] = cx[0]; px[l][1] = cx[1]; cx[0] = nx0[0]; cx[1] = nx0[1]; }
