@@ -322,8 +322,9 @@ __device__ __forceinline__ void strip_sts_half(T* __restrict__ sp, int lane, con
     }
 }
 
-// Row pairs travel HBM -> shared memory with cp.async (16 bytes per lane, lane-private slots, so the
-// issuing lane is the only reader and cp.async.wait_group is all the synchronisation needed) through a
+// Row pairs travel HBM -> shared memory with cp.async (16 bytes per lane into the lane-private slots; a
+// slot is read by its owner lane after cp.async.wait_group and a __syncwarp, since with C/V > 1 another
+// lane of the warp may have issued the copy) through a
 // ring of kStripRing pairs: a pair is requested kStripRing-1 iterations before it is used, no register
 // holds data in flight, and nothing has to be moved while a load is pending.
 constexpr int kStripRing = GE_STRIP_RING;
@@ -346,9 +347,14 @@ __device__ __forceinline__ void strip_request_pair(const T* __restrict__ uin, in
     for (int rr = 0; rr < 2; ++rr) {
         const int yy = y + rr;
         if ((unsigned)yy < (unsigned)ny) {
-            const T* __restrict__ row = uin + (int64_t)yy * nx + e0;
+            // the warp copies the row's 32*C values as C/V instructions of 32 CONSECUTIVE 16-byte chunks
+            // (full sectors on the global side); chunk q belongs to lane q / (C/V), vector q % (C/V)
+            const T* __restrict__ row = uin + (int64_t)yy * nx + (e0 - lane * C);
 #pragma unroll
-            for (int c = 0; c < C / V; ++c) cp_async16(dst + ((rr * (C / V) + c) * 32 + lane) * V, row + c * V);
+            for (int cc = 0; cc < C / V; ++cc) {
+                const int q = cc * 32 + lane;
+                cp_async16(dst + ((rr * (C / V) + q % (C / V)) * 32 + q / (C / V)) * V, row + q * V);
+            }
         } else {
             const T f = yy == -1 ? ylo : (yy == ny ? yhi : T(0));
             VT q;
@@ -356,6 +362,40 @@ __device__ __forceinline__ void strip_request_pair(const T* __restrict__ uin, in
 #pragma unroll
             for (int c = 0; c < C / V; ++c) *reinterpret_cast<VT*>(dst + ((rr * (C / V) + c) * 32 + lane) * V) = q;
         }
+    }
+}
+
+// The TB stages of one iteration: `cur` (raw pair of level 0, rows y0, y0+1; cx its column 0) flows through
+// and comes out as the level-TB pair.  PURE: every group row (j = y0-1-l) is interior now and at the next
+// iteration, so there is neither an edge test nor a raw slot; otherwise each stage decides (warp-uniform).
+template <typename T, int C, int TB, bool BC, bool PURE>
+__device__ __forceinline__ void strip_stages(T (&cur)[2][C], T (&cx)[2], T (&px)[TB][2], T* __restrict__ sp, int lane,
+                                             const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int y0, int ny) {
+    constexpr int kPair = 2 * 32 * C;
+#pragma unroll
+    for (int l = 0; l < TB; ++l) {
+        const int j = y0 - 1 - l;                                                  // group rows j, j+1
+        const bool fast = PURE || (unsigned)j < (unsigned)(ny - 1);                // both interior
+        const bool next_fast = PURE || (unsigned)(j + 2) < (unsigned)(ny - 1);     // this stage, next iteration
+        T* slot = sp + l * kPair;
+        T N[2][C], nx0[2] = {T(0), T(0)};
+        T Hn[C], Rc[C / 2], Rd[C / 2];
+        strip_rhs_pair<T, C>(cur[0], cur[1], k.r, Hn, Rc, Rd);
+        if (fast) {
+            T H[C];
+            strip_lds_half<T, C>(slot, lane, H);
+            if ((l & 1) != 0) strip_stage_L<T, C, BC>(H, Rc, Rd, px[l], cx, N[0], N[1], k);
+            else              strip_stage_R<T, C, BC>(H, Rc, Rd, N[0], N[1], nx0, k);
+        } else {
+            T P[2][C];
+            strip_lds<T, C>(slot, lane, P);
+            strip_stage_rows<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, j, ny);
+        }
+        if (next_fast) strip_sts_half<T, C>(slot, lane, Hn);
+        else           strip_sts<T, C>(slot, lane, cur);
+#pragma unroll
+        for (int s = 0; s < C; ++s) { cur[0][s] = N[0][s]; cur[1][s] = N[1][s]; }
+        if constexpr (BC) { px[l][0] = cx[0]; px[l][1] = cx[1]; cx[0] = nx0[0]; cx[1] = nx0[1]; }
     }
 }
 
@@ -396,37 +436,17 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
     for (int it = 0; it < iters; ++it) {
         const int y0 = Y0 + 2 * it;
         // request the pair of iteration it + kStripRing - 1 (its slot was read in iteration it - 1)
+        if constexpr (C / V > 1) __syncwarp();    // by its owner lanes, which may not be the lanes that refill it
         strip_request_pair<T, C>(uin, nx, ny, kk.ylo, kk.yhi, y0 + 2 * (kStripRing - 1), e0,
                                  ring + ((it + kStripRing - 1) % kStripRing) * kPair, lane);
         cp_async_commit();
-        cp_async_wait<kStripRing - 1>();          // the pair of this iteration has landed
+        cp_async_wait<kStripRing - 1>();          // the pair of this iteration has landed (this lane's copies)
+        if constexpr (C / V > 1) __syncwarp();    // ... and the other lanes' copies into this lane's slots
         T cur[2][C], cx[2] = {T(0), T(0)};
         strip_lds<T, C>(ring + (it % kStripRing) * kPair, lane, cur);
-#pragma unroll
-        for (int l = 0; l < TB; ++l) {
-            const int j = y0 - 1 - l;                                          // group rows j, j+1
-            const bool fast = (unsigned)j < (unsigned)(ny - 1);                // both interior
-            const bool next_fast = (unsigned)(j + 2) < (unsigned)(ny - 1);     // this stage, next iteration
-            T* slot = sp + l * kPair;
-            T N[2][C], nx0[2] = {T(0), T(0)};
-            T Hn[C], Rc[C / 2], Rd[C / 2];
-            strip_rhs_pair<T, C>(cur[0], cur[1], k.r, Hn, Rc, Rd);
-            if (fast) {
-                T H[C];
-                strip_lds_half<T, C>(slot, lane, H);
-                if ((l & 1) != 0) strip_stage_L<T, C, BC>(H, Rc, Rd, px[l], cx, N[0], N[1], k);
-                else              strip_stage_R<T, C, BC>(H, Rc, Rd, N[0], N[1], nx0, k);
-            } else {
-                T P[2][C];
-                strip_lds<T, C>(slot, lane, P);
-                strip_stage_rows<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, j, ny);
-            }
-            if (next_fast) strip_sts_half<T, C>(slot, lane, Hn);
-            else           strip_sts<T, C>(slot, lane, cur);
-#pragma unroll
-            for (int s = 0; s < C; ++s) { cur[0][s] = N[0][s]; cur[1][s] = N[1][s]; }
-            if constexpr (BC) { px[l][0] = cx[0]; px[l][1] = cx[1]; cx[0] = nx0[0]; cx[1] = nx0[1]; }
-        }
+        // every stage's group row interior now and at its next iteration: the pure pipeline, no edge tests
+        if (y0 - TB >= 0 && y0 + 1 < ny - 1) strip_stages<T, C, TB, BC, true>(cur, cx, px, sp, lane, k, coef, y0, ny);
+        else                                 strip_stages<T, C, TB, BC, false>(cur, cx, px, sp, lane, k, coef, y0, ny);
         // cur holds level-TB rows (y0 - TB, y0 - TB + 1), unshifted (TB is even)
         if (it >= TB) {
             const int yo = y0 - TB;
