@@ -329,7 +329,10 @@ int launch_temporal_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) 
 #ifndef GE_STRIP_C_F32
 #define GE_STRIP_C_F32 4
 #endif
-template <typename T> struct StripC { static constexpr int c = sizeof(T) == 8 ? 4 : GE_STRIP_C_F32; };
+#ifndef GE_STRIP_C_F64
+#define GE_STRIP_C_F64 2
+#endif
+template <typename T> struct StripC { static constexpr int c = sizeof(T) == 8 ? GE_STRIP_C_F64 : GE_STRIP_C_F32; };
 bool strip2d_ok(const ge_plan* p) {
     const int c = p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c;
     return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * c;

@@ -476,7 +476,7 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
 #define GE_STRIP_MINB_F32 3
 #endif
 #ifndef GE_STRIP_MINB_F64
-#define GE_STRIP_MINB_F64 3
+#define GE_STRIP_MINB_F64 4
 #endif
 template <typename T> struct StripMinBlocks { static constexpr int n = sizeof(T) == 8 ? GE_STRIP_MINB_F64 : GE_STRIP_MINB_F32; };
 

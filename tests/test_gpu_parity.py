@@ -263,9 +263,10 @@ def test_per_step_2d(oracle, dtype, nx, ny):
             assert rel_err(got, ref) <= (2e-14 if dtype == "f64" else 3e-6), (nx, ny, level0, steps)
 
 
-def _launches_2d(nx, tb, level0, steps):
-    """ge_run's 2-D schedule: the strip kernel (nx % 4 == 0, nx >= 128) starts at odd levels only."""
-    strips = nx % 4 == 0 and nx >= 128
+def _launches_2d(nx, tb, level0, steps, dtype):
+    """ge_run's 2-D schedule: the strip kernel (nx % 4 == 0, nx >= one strip: 128 columns in fp32, 64 in
+    fp64) starts at odd levels only."""
+    strips = nx % 4 == 0 and nx >= (128 if dtype == "f32" else 64)
     level, left, n = level0, steps, 0
     while left > 0:
         if strips and left > tb and level % 2 == 0:
@@ -286,7 +287,7 @@ def _launches_2d(nx, tb, level0, steps):
                                          (128, 16, 4, 2), (128, 130, 6, 5), (352, 77, 6, 64), (240, 64, 8, 3),
                                          (1000, 37, 4, 64), (2048, 20, 8, 64)])
 def test_temporal_2d(oracle, dtype, nx, ny, tb, hp):
-    """Strategy B in 2-D (warp strips streaming along y): the drift-free strip kernel (nx >= 128:
+    """Strategy B in 2-D (warp strips streaming along y): the drift-free strip kernel (nx >= 128 in fp32, 64 in fp64:
     aligned first/last strips, R/L stages, x-edge groups on lane 0 / 31, y-edge groups in the
     generic stage) and the drifting kernel for narrow grids; several strips and segments, ragged
     last strip/segment, odd ny, both starting phases, and a remainder of levels that falls back to
@@ -295,7 +296,7 @@ def test_temporal_2d(oracle, dtype, nx, ny, tb, hp):
     for level0, steps in ((0, tb), (1, tb), (0, 2 * tb + 3), (1, 3 * tb), (0, 4 * tb + 1)):
         got, info = run_gpu(cfg, steps, kernel="temporal", tb=tb, level0=level0, hp=hp)
         ref = run_oracle(oracle, cfg, steps, level0=level0)
-        assert info["kernel"] == "temporal" and info["launches"] == _launches_2d(nx, tb, level0, steps), info
+        assert info["kernel"] == "temporal" and info["launches"] == _launches_2d(nx, tb, level0, steps, dtype), info
         assert rel_err(got, ref) <= (1e-13 if dtype == "f64" else 1e-5), (nx, ny, level0, steps, info)
         same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
         np.testing.assert_array_equal(got, same, err_msg=str((nx, ny, level0, steps)))
