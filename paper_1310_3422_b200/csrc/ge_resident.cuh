@@ -587,6 +587,19 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
 #pragma unroll 1
     while (left >= 2) {
         if (usedl + 2 > a.tb) { meet(); usedl = 0; }
+        // two level pairs back to back where the halo allows it: the scheduler overlaps the tail of one
+        // pair with the head of the next (a lone warp drains its pipeline at every loop back-edge)
+        // (not for the largest tiles: their window alone takes half the register file)
+        if constexpr (C * sizeof(T) <= 256) {
+            if (left >= 4 && usedl + 4 <= a.tb) {
+                level_R<T, C, false>(v, x0, c, 0);
+                level_L<T, C, false>(v, x0, c, 0);
+                level_R<T, C, false>(v, x0, c, 0);
+                level_L<T, C, false>(v, x0, c, 0);
+                usedl += 4; left -= 4;
+                continue;
+            }
+        }
         level_R<T, C, false>(v, x0, c, 0);
         level_L<T, C, false>(v, x0, c, 0);
         usedl += 2; left -= 2;
