@@ -123,8 +123,8 @@ int ge_run(ge_plan *p, void *u, int64_t steps, ge_stream_t stream);
 
 /* End-to-end variant with HOST buffers: copies u_host (batch*nx or ny*nx elements, ideally pinned)
  * to a plan-owned device buffer, runs `steps` levels, copies the result back into u_host and
- * synchronises `stream` before returning.  One long rod (dim 1, batch 1, nx >= 2^25) is cut into chunks
- * of 2^24 nodes that carry 2*steps+8 extra nodes per side -- more than the dependency cone of `steps`
+ * synchronises `stream` before returning.  One long rod (dim 1, batch 1, nx >= 2^23) is cut into chunks
+ * of 2^22 nodes that carry 2*steps+8 extra nodes per side -- more than the dependency cone of `steps`
  * levels -- and are marched independently through a three-slot pipeline (upload, compute and download of
  * neighbouring chunks overlap; u_host should be pinned for that); the result is bit-identical.  Batched rods
  * (batch >= 64, >= 8 MiB) travel through the same pipeline in eight groups of rods. */

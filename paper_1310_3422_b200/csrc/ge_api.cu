@@ -769,7 +769,10 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
 // run -- and the chunks travel through a three-slot pipeline: while chunk c is computed, chunk c+1 is
 // on its way to the device and chunk c-1 on its way back.
 constexpr int kHostSlots = 3;
-constexpr int64_t kHostChunk = (int64_t)1 << 24;
+#ifndef GE_HOST_CHUNK_LOG2
+#define GE_HOST_CHUNK_LOG2 22
+#endif
+constexpr int64_t kHostChunk = (int64_t)1 << GE_HOST_CHUNK_LOG2;
 
 static int host_pipeline(ge_plan* p, void* u_host, int64_t steps, cudaStream_t user) {
     const size_t es = elem_size(p->dtype);
