@@ -432,18 +432,37 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
         cp_async_commit();
     }
 
+    // loop-carried bookkeeping instead of per-iteration multiplies and modulos: ring slots of the pair to
+    // request / to read, element offsets of the rows to request / to write (64-bit, may run outside the grid:
+    // only used under the row tests)
+    int rq = kStripRing - 1, rd = 0;
+    int64_t in_off = (int64_t)(Y0 + 2 * (kStripRing - 1)) * nx + e0;
+    int64_t out_off = (int64_t)(Y0 - TB) * nx + e0;
+    bool st_ok[C / V];
+#pragma unroll
+    for (int c = 0; c < C / V; ++c) st_ok[c] = e0 + c * V >= out_lo && e0 + c * V < out_hi;
 #pragma unroll 1
-    for (int it = 0; it < iters; ++it) {
+    for (int it = 0; it < iters; ++it, in_off += 2 * (int64_t)nx, out_off += 2 * (int64_t)nx) {
         const int y0 = Y0 + 2 * it;
         // request the pair of iteration it + kStripRing - 1 (its slot was read in iteration it - 1)
         if constexpr (C / V > 1) __syncwarp();    // by its owner lanes, which may not be the lanes that refill it
-        strip_request_pair<T, C>(uin, nx, ny, kk.ylo, kk.yhi, y0 + 2 * (kStripRing - 1), e0,
-                                 ring + ((it + kStripRing - 1) % kStripRing) * kPair, lane);
+        {
+            const int yq = y0 + 2 * (kStripRing - 1);
+            T* dst = ring + rq * kPair;
+            if (C == V && yq >= 0 && yq + 1 < ny) {        // both rows inside the grid (warp-uniform)
+                cp_async16(dst + lane * V, uin + in_off);
+                cp_async16(dst + (32 + lane) * V, uin + in_off + nx);
+            } else {
+                strip_request_pair<T, C>(uin, nx, ny, kk.ylo, kk.yhi, yq, e0, dst, lane);
+            }
+            rq = rq + 1 == kStripRing ? 0 : rq + 1;
+        }
         cp_async_commit();
         cp_async_wait<kStripRing - 1>();          // the pair of this iteration has landed (this lane's copies)
         if constexpr (C / V > 1) __syncwarp();    // ... and the other lanes' copies into this lane's slots
         T cur[2][C], cx[2] = {T(0), T(0)};
-        strip_lds<T, C>(ring + (it % kStripRing) * kPair, lane, cur);
+        strip_lds<T, C>(ring + rd * kPair, lane, cur);
+        rd = rd + 1 == kStripRing ? 0 : rd + 1;
         // every stage's group row interior now and at its next iteration: the pure pipeline, no edge tests
         if (y0 - TB >= 0 && y0 + 1 < ny - 1) strip_stages<T, C, TB, BC, true>(cur, cx, px, sp, lane, k, coef, y0, ny);
         else                                 strip_stages<T, C, TB, BC, false>(cur, cx, px, sp, lane, k, coef, y0, ny);
@@ -453,15 +472,14 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
 #pragma unroll
             for (int rr = 0; rr < 2; ++rr) {
                 if (yo + rr < ye) {
-                    T* __restrict__ row = uout + (int64_t)(yo + rr) * nx;
+                    T* __restrict__ row = uout + out_off + (rr ? nx : 0);
 #pragma unroll
                     for (int c = 0; c < C / V; ++c) {
-                        const int e = e0 + c * V;
-                        if (e >= out_lo && e < out_hi) {
+                        if (st_ok[c]) {
                             T t[V];
 #pragma unroll
                             for (int q = 0; q < V; ++q) t[q] = cur[rr][c * V + q];
-                            st_vec(row + e, t);
+                            st_vec(row + c * V, t);
                         }
                     }
                 }
