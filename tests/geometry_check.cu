@@ -77,12 +77,23 @@ int main() {
     for (int TB : {4, 6, 8}) for (int64_t nx : {128, 132, 232, 244, 256, 1000, 8192}) for (int64_t ny : {1, 7, 64, 1000}) for (int hp : {1, 5, 56, 64}) {
         check_strips_2d(4, 4, TB, nx, ny, hp);
         check_strips_2d(4, 2, TB, nx, ny, hp);
+        check_strips_2d(2, 2, TB, nx, ny, hp);           // the fp64 default: 64-column strips
     }
+    for (int TB : {4, 6, 8}) for (int64_t nx : {64, 68, 116, 120}) for (int64_t ny : {1, 7, 64}) for (int hp : {1, 5, 56})
+        check_strips_2d(2, 2, TB, nx, ny, hp);
     for (int k : {2, 3, 5, 16, 64, 1000}) for (int phase = 0; phase < 2; ++phase) for (int64_t nx : {1, 2, 3, 30, 62, 8206, 100000}) check_units(k, phase, nx);
     // meetings of the whole-chip kernel: never more levels between two meetings than tb
     for (int tb = 2; tb <= 64; tb += 2) for (int64_t steps : {0, 1, 2, 3, 63, 64, 65, 1000, 10001}) for (int ph = 0; ph < 2; ++ph) {
         const int64_t m = ge::grid_resident_meetings(steps, ph, tb);
         CHECK(m >= (steps > tb + 2 ? (steps - 2) / tb - 1 : 0) && m <= steps / 2 + 1, "meetings steps=%lld tb=%d m=%lld", (long long)steps, tb, (long long)m);
+    }
+    // staggered meetings: a tile publishes every tbh levels and refreshes its halo every second publication,
+    // so 2*tbh <= tb must hold; the host's count of publications (+ the final one) is the meeting loop at tbh
+    for (int tb = 8; tb <= 128; tb += 2) for (int64_t steps : {0, 1, 2, 3, 63, 64, 65, 1000, 10001}) for (int ph = 0; ph < 2; ++ph) {
+        const int tbh = tb / 2 - (tb / 2) % 2;
+        CHECK(tbh >= 2 && 2 * tbh <= tb, "stagger tb=%d tbh=%d", tb, tbh);
+        const int64_t h = ge::grid_resident_halves(steps, ph, tb);
+        CHECK(h == ge::grid_resident_meetings(steps, ph, tbh) + 1, "halves steps=%lld tb=%d h=%lld", (long long)steps, tb, (long long)h);
     }
     std::printf("%s (%d failures)\n", fails ? "GEOMETRY FAILED" : "GEOMETRY OK", fails);
     return fails ? 1 : 0;
