@@ -162,7 +162,7 @@ enum {
                                   default for rods of >= 4 tiles (needs nx >= 32 * value)                   */
     GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
                                   2-D: one of the compiled-in block lengths 4, 8)                            */
-    GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 64)       */
+    GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64) */
     GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
                                   long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
     GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */

@@ -619,7 +619,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     // the chip (1-D only), else the temporally blocked ones
     p->tb = 0;
     p->tc = default_tc(p->dtype, p->nx);
-    p->hp = 56;                    // measured on C5
+    p->hp = p->dtype == GE_F64 ? 56 : 67;   // measured on C5 (the rate depends on the segment count, and sharply)
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
