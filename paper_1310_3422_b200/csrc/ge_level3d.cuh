@@ -30,13 +30,13 @@ struct Coef3 {
 };
 
 #ifndef GE_L3D_BX
-#define GE_L3D_BX 32
+#define GE_L3D_BX 16
 #endif
 #ifndef GE_L3D_BY
 #define GE_L3D_BY 4
 #endif
 #ifndef GE_L3D_BZ
-#define GE_L3D_BZ 1
+#define GE_L3D_BZ 2
 #endif
 #ifndef GE_L3D_MINB
 #define GE_L3D_MINB 1
