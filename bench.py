@@ -15,6 +15,13 @@ collective; value = updates of all ranks / max-over-rank
 
 --impl reference times the ORACLE (oracle/ge_ref.c, plain fp64 C, one host core) on a bounded sample
 of the same workload; it is a deliberately slow baseline, not the target.
+
+Beside the contract's keys the default line carries: `alu_peaks` (FFMA / DFMA throughput measured in this
+run by libge's ge_fma_probe, the denominator of every "bound": "alu" roofline), `parity` (sampled
+dependency cones of a run from the config's initial state against the oracle), `cpu_baseline` with a
+one-thread and an all-cores leg on ONE sample (the same one --impl reference times), `secondary` (C5 f32,
+C5 f64, C2, C3 device-resident, so that the 2-D half of the north_star target is in the driver's record),
+and the PCIe ceiling beside `e2e`.  `--sweep sync` is the synchronisation study.
 """
 from __future__ import annotations
 
@@ -98,8 +105,49 @@ def oracle_time(cfg):
 
 
 def sample_desc(cfg, scale):
-    return "same recipe at 1/%d of the grid (%s), all %d levels, oracle/ge_ref.c -O2, 1 thread" % (
+    return "same recipe at 1/%d of the grid (%s), all %d levels, oracle/ge_ref.c -O2" % (
         round(1 / scale), workload_desc(cfg).split(": ")[1].split(",")[1].strip(), cfg["steps"])
+
+
+def oracle_time_allcores(cfg):
+    """Seconds of the all-cores timing driver (oracle/ge_ref_omp.c: the same literal formulas, the groups of
+    a level split across threads; pinned bit for bit to ge_ref.c by tests/test_oracle_omp.py), or None for
+    workloads it does not cover (k >= 2, 3-D)."""
+    from oracle import ge_oracle_omp as om
+    if cfg.get("k", 1) != 1 or cfg["dim"] == 3:
+        return None, 0
+    om.build()
+    u0 = cfg["u0"].astype(np.float64)
+    t0 = time.perf_counter()
+    if cfg["dim"] == 2:
+        om.run_2d(u0, cfg["r"][0], cfg["steps"], (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1]))
+    elif cfg["batch"] == 1:
+        om.run_1d(u0.reshape(-1), cfg["r"][0], cfg["steps"], cfg["bc_lo"][0], cfg["bc_hi"][0])
+    else:
+        om.run_batched_1d(u0, cfg["r"], cfg["steps"], cfg["bc_lo"], cfg["bc_hi"])
+    return time.perf_counter() - t0, om.threads()
+
+
+def cpu_baseline(cfg_name, scale, k=1, levels=0, reps=2):
+    """The oracle as it stands on this box's host cores, on ONE bounded sample of the workload: (a) one
+    thread (the parity oracle itself), (b) all cores (the OpenMP timing driver).  `value` is leg (a)."""
+    from oracle import ge_oracle
+    ge_oracle.build()
+    scfg = make_cfg(cfg_name, scale)
+    scfg["k"] = k
+    if levels:
+        scfg["steps"] = levels
+    ts = [oracle_time(scfg) for _ in range(reps)]
+    t1 = min(ts)
+    out = {"value": units(scfg) / t1 / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": sample_desc(scfg, scale) + ", best of %d" % reps, "seconds": t1, "seconds_each": ts}
+    ta, nthreads = oracle_time_allcores(scfg)
+    if ta is not None:
+        ta = min(ta, oracle_time_allcores(scfg)[0])
+        out["all_cores"] = {"value": units(scfg) / ta / 1e9, "unit": UNIT, "cores": nthreads,
+                            "host_cores": os.cpu_count(), "kind": "oracle formulas, OpenMP over the groups of a level (oracle/ge_ref_omp.c)",
+                            "sample": "the same sample", "seconds": ta}
+    return out
 
 
 def run_reference(args):
@@ -123,7 +171,7 @@ def run_reference(args):
         "data": "synthetic",
         "config": {"workload": full, "sample": sample_desc(cfg, scale)},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                         "sample": sample_desc(cfg, scale)},
+                         "sample": sample_desc(cfg, scale) + ", 1 thread, every step one run of the sample"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -221,6 +269,204 @@ def job_value(units_per_rank_step, steps, world, ms):
 
 
 # ------------------------------------------------------------------ our arm (CUDA) ------
+SYNC_IDS = {"flags": 0, "grid": 1, "lines": 2, "stagger": 3}
+
+
+def fma_peaks(dev, stream_obj):
+    """Sustained FFMA / DFMA throughput of this GPU, measured now with libge's probe kernel (8 independent
+    FMA chains per thread, 2048 threads per SM): the peak the "alu"-bound rooflines are divided by
+    (the lane counts are an assumption until measured)."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    sink = torch.zeros(16, dtype=torch.float64, device=dev)
+    out = {}
+    for dt, iters in (("f32", 1 << 17), ("f64", 1 << 16)):
+        libge.ge_fma_probe(dt, 1 << 12, sink.data_ptr(), stream_obj.cuda_stream)       # warm-up
+        best = 0.0
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream_obj)
+            flops = libge.ge_fma_probe(dt, iters, sink.data_ptr(), stream_obj.cuda_stream)
+            e1.record(stream_obj)
+            torch.cuda.synchronize(dev)
+            best = max(best, flops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        out[dt + "_tflops"] = best
+    clk = float(measured_peaks()[0].get("sm_max_mhz", 1965.0)) * 1e6
+    out["derived"] = {dt + "_tflops": 2.0 * LANES[dt] * SMS * clk / 1e12 for dt in ("f32", "f64")}
+    out["how"] = ("ge_fma_probe (csrc/ge_probe.cuh): 8 independent dependent-FMA chains per thread, 2048 threads per SM, "
+                  "best of 3 launches of ~10 ms, CUDA events; derived = 2 flop x lanes/SM (128 f32, 64 f64) x %d SMs x %.0f MHz" % (SMS, clk / 1e6))
+    return out
+
+
+def pcie_rates(dev, stream_obj, nbytes=1 << 29):
+    """Host<->device copy rates of this box (pinned memory, one direction at a time): the ceiling of `e2e`."""
+    import torch
+    h = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    out = {}
+    for name, fn in (("h2d_gbs", lambda: d.copy_(h, non_blocking=True)), ("d2h_gbs", lambda: h.copy_(d, non_blocking=True))):
+        fn()
+        torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream_obj)
+        fn()
+        e1.record(stream_obj)
+        torch.cuda.synchronize(dev)
+        out[name] = nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9
+    return out
+
+
+def _window_1d(oracle, u0, r, steps, lo, hi, start, width):
+    """Oracle values of elements [start, start+width) after `steps` levels from level 0, marched on the
+    dependency cone only (a two-point group reads u_{i-1}..u_{i+2}: at most 2 nodes per side
+    and level); the sub-rod starts at an even element so that its pair pattern is the global one, a cut end
+    gets an arbitrary boundary value whose influence cannot reach the window."""
+    n = u0.shape[0]
+    halo = 2 * steps + 4
+    a = max(0, start - halo)
+    a -= a % 2
+    b = min(n, start + width + halo)
+    out = oracle.run_1d(u0[a:b].astype(np.float64), r, steps, lo if a == 0 else 0.123, hi if b == n else -0.456)
+    return out[start - a:start - a + width]
+
+
+def _window_2d(oracle, u0, r, steps, bc, x0, y0, w):
+    ny, nx = u0.shape
+    halo = 2 * steps + 4
+    ax = max(0, x0 - halo); ax -= ax % 2
+    ay = max(0, y0 - halo); ay -= ay % 2
+    bx, by = min(nx, x0 + w + halo), min(ny, y0 + w + halo)
+    sbc = (bc[0] if ax == 0 else 0.1, bc[1] if bx == nx else -0.2, bc[2] if ay == 0 else 0.3, bc[3] if by == ny else -0.4)
+    out = oracle.run_2d(u0[ay:by, ax:bx].astype(np.float64), r, steps, sbc)
+    return out[y0 - ay:y0 - ay + w, x0 - ax:x0 - ax + w]
+
+
+def parity_check(cfg, plan, dev, stream, k=1, budget=4e8):
+    """A run from the config's initial state in the timed launch configuration, compared with the oracle on
+    sampled dependency cones (rods: whole sampled rods).  Where the cones of the full level count would cost
+    more than `budget` oracle updates each (C5: 1000 levels -> 4000^2 nodes per window) the run is repeated
+    with fewer levels -- the full-length comparison is tests/test_gpu_longrun.py's."""
+    import torch
+    from oracle import ge_oracle
+    if cfg["dim"] == 3 or k != 1:
+        return None
+    ge_oracle.build()
+    tol = 1e-12 if cfg["dtype"] == "f64" else 1e-5
+    levels = cfg["steps"]
+    if cfg["dim"] == 2:
+        while (24 + 4 * levels + 8) ** 2 * levels > budget and levels > 8:
+            levels //= 2
+    elif cfg["dim"] == 1 and cfg["batch"] == 1:
+        while (64 + 4 * levels + 8) * levels > budget and levels > 8:
+            levels //= 2
+    u = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
+    plan.level = 0
+    plan.run(u.data_ptr(), levels, stream)
+    torch.cuda.synchronize(dev)
+    got = u.cpu().numpy().astype(np.float64).reshape(cfg["u0"].shape)
+    del u
+    rng = np.random.default_rng(12345)
+    worst, what = 0.0, ""
+    if cfg["dim"] == 2:
+        ny, nx = cfg["u0"].shape
+        w = 24
+        bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1])
+        pts = [(0, 0), (nx - w, ny - w)] + [tuple(int(v) for v in rng.integers(0, min(nx, ny) - w, size=2)) for _ in range(2)]
+        for x0, y0 in pts:
+            x0 -= x0 % 2; y0 -= y0 % 2
+            ref = _window_2d(ge_oracle, cfg["u0"], cfg["r"][0], levels, bc, x0, y0, w)
+            worst = max(worst, float(np.abs(got[y0:y0 + w, x0:x0 + w] - ref).max()))
+        scale = float(np.abs(cfg["u0"]).max())
+        what = "%d windows of %dx%d nodes on their dependency cones" % (len(pts), w, w)
+    elif cfg["batch"] == 1:
+        n, w = cfg["nx"], 64
+        u0 = cfg["u0"].reshape(-1)
+        g = got.reshape(-1)
+        starts = [0, n - w] + [int(v) for v in rng.integers(0, n - w, size=2)] if n > 4 * w else [0]
+        for st in starts:
+            st -= st % 2
+            ww = min(w, n - st)
+            ref = _window_1d(ge_oracle, u0, cfg["r"][0], levels, cfg["bc_lo"][0], cfg["bc_hi"][0], st, ww)
+            worst = max(worst, float(np.abs(g[st:st + ww] - ref).max()))
+        scale = float(np.abs(u0).max())
+        what = "%d windows of %d nodes on their dependency cones" % (len(starts), w)
+    else:
+        rows = np.unique(np.concatenate([[0, cfg["batch"] - 1], rng.integers(0, cfg["batch"], size=2)]))
+        ref = ge_oracle.run_batched_1d(cfg["u0"][rows].astype(np.float64), cfg["r"][rows], levels,
+                                       cfg["bc_lo"][rows], cfg["bc_hi"][rows])
+        worst = float((np.abs(got[rows] - ref).max(axis=1) / np.abs(ref).max(axis=1)).max())
+        scale = 1.0
+        what = "%d whole rods" % len(rows)
+    err = worst / scale
+    return {"rel_err": err, "tolerance": tol, "ok": bool(err <= tol), "levels": levels, "sample": what,
+            "norm": "max|gpu - oracle| / max|u| (DESIGN.md reading R-A7)", "oracle": "oracle/ge_ref.c"}
+
+
+def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clocks_index=None, flush_l2=False,
+                  with_parity=True, k=1):
+    """W warm-up steps, then K timed steps of ge_run on a device-resident state; returns the measurement dict
+    and the plan (open) for the caller's further legs."""
+    import torch
+    import torch.distributed as dist
+    from paper_1310_3422_b200 import libge
+    stream = stream_obj.cuda_stream
+    levels = cfg["steps"]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    u = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
+    plan = libge.Plan(cfg, kernel=args_like.get("kernel", "auto"), tb=args_like.get("tb", 0), stream=stream, group_k=k)
+    for key, what in (("tc", libge.GE_TUNE_TEMPORAL_C), ("rc", libge.GE_TUNE_RESIDENT_C), ("hl", libge.GE_TUNE_HALO_LANES)):
+        if args_like.get(key):
+            plan.tune(what, args_like[key])
+    if args_like.get("sync"):
+        plan.tune(libge.GE_TUNE_SYNC_MODE, SYNC_IDS[args_like["sync"]])
+    if args_like.get("rtb"):
+        plan.tune(libge.GE_TUNE_TB, args_like["rtb"])
+    info0 = plan.info()
+    flush = torch.empty(1 << 28, dtype=torch.uint8, device=dev) if flush_l2 else None     # 256 MiB > 126 MB of L2
+    clocks = ClockSampler(clocks_index) if clocks_index is not None else None     # started early: nvidia-smi needs ~0.2 s
+    for _ in range(warmup):
+        plan.run(u.data_ptr(), levels, stream)
+    barrier()
+    l0, m0 = plan.info()["launches"], plan.info()["meetings"]
+    e0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    e1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    barrier()
+    if clocks:
+        clocks.begin()
+    for i in range(steps):
+        if flush is not None:
+            flush.zero_()
+        e0[i].record(stream_obj)
+        plan.run(u.data_ptr(), levels, stream)
+        e1[i].record(stream_obj)
+    barrier()
+    if clocks:
+        clocks.end()
+    per_step = [e0[i].elapsed_time(e1[i]) for i in range(steps)]
+    # consecutive steps without a flush: the whole bracket (first start to last end); with a flush between
+    # the steps: the sum of the steps' own intervals (the flush is not part of the workload)
+    total_ms = sum(per_step) if flush is not None else e0[0].elapsed_time(e1[-1])
+    launches = plan.info()["launches"] - l0
+    meetings = plan.info()["meetings"] - m0
+    total_ms_max = max_over_ranks(total_ms, world, dev)
+    finite = bool(torch.isfinite(u).all().item())
+    fault = plan.sync_fault() if info0["resident_path"] == 2 else 0
+    del u, flush
+    if clocks:
+        clocks.close()
+    info0["group_k"] = k
+    out = {"value": job_value(units(cfg), steps, world, total_ms_max), "ms_per_step": total_ms_max / steps,
+           "total_ms_this_rank": total_ms, "per_step": per_step, "launches": launches, "meetings": meetings,
+           "finite": finite and not fault, "info": info0, "clocks": clocks.summary() if clocks else None,
+           "l2": "flushed between timed steps (256 MiB write)" if flush_l2 else None}
+    return out, plan
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -239,13 +485,6 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
         dist.barrier()
     libge.load()
-
-    cfg = make_cfg(args.config)
-    if args.levels:
-        cfg["steps"] = args.levels
-    levels = cfg["steps"]
-    es = ESIZE[cfg["dtype"]]
-    nelem = cfg["nx"] * cfg["ny"] * cfg.get("nz", 1) * cfg["batch"]
     stream_obj = torch.cuda.current_stream(dev)
     stream = stream_obj.cuda_stream
 
@@ -254,126 +493,200 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    host0 = torch.from_numpy(cfg["u0"].reshape(-1))
-    u = host0.to(dev)
-    plan = libge.Plan(cfg, kernel=args.kernel, tb=args.tb, stream=stream, group_k=args.k)
-    if args.tc:
-        plan.tune(libge.GE_TUNE_TEMPORAL_C, args.tc)
-    if args.rc:
-        plan.tune(libge.GE_TUNE_RESIDENT_C, args.rc)
-    if args.hl:
-        plan.tune(libge.GE_TUNE_HALO_LANES, args.hl)
-    if args.sync:
-        plan.tune(libge.GE_TUNE_SYNC_MODE, {"flags": libge.GE_SYNC_FLAGS, "grid": libge.GE_SYNC_GRID, "lines": libge.GE_SYNC_LINES, "stagger": libge.GE_SYNC_STAGGER}[args.sync])
-    if args.rtb:
-        plan.tune(libge.GE_TUNE_TB, args.rtb)
-    info0 = plan.info()
+    peaks_alu = fma_peaks(dev, stream_obj)
+    tune = dict(kernel=args.kernel, tb=args.tb, tc=args.tc, rc=args.rc, hl=args.hl, sync=args.sync, rtb=args.rtb)
+
+    cfg = make_cfg(args.config)
+    if args.levels:
+        cfg["steps"] = args.levels
+    levels = cfg["steps"]
+    es = ESIZE[cfg["dtype"]]
+    nelem = cfg["nx"] * cfg["ny"] * cfg.get("nz", 1) * cfg["batch"]
+    fits_l2 = nelem * es <= 126e6
 
     # ---- device-resident timing: W warm-up steps, then exactly K timed steps ----
-    clocks = ClockSampler(local) if rank == 0 else None       # started early: nvidia-smi needs ~0.2 s to come up
-    for _ in range(args.warmup):
-        plan.run(u.data_ptr(), levels, stream)
-    barrier()
-    l0, m0 = plan.info()["launches"], plan.info()["meetings"]
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    barrier()
-    if clocks:
-        clocks.begin()
-    ev[0].record(stream_obj)
-    for i in range(args.steps):
-        plan.run(u.data_ptr(), levels, stream)
-        ev[i + 1].record(stream_obj)
-    barrier()
-    if clocks:
-        clocks.end()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    launches = plan.info()["launches"] - l0
-    meetings = plan.info()["meetings"] - m0
-    total_ms_max = max_over_ranks(total_ms, world, dev)
-    value = job_value(units(cfg), args.steps, world, total_ms_max)
-    finite = bool(torch.isfinite(u).all().item())
-
-    # ---- roofline of the dominant kernel: its average launch duration over the timed region ----
-    info0["group_k"] = args.k
-    roof = roofline(cfg, info0, total_ms, launches, args.steps)
-    fault = plan.sync_fault() if info0["resident_path"] == 2 else 0
+    m, plan = device_timing(cfg, tune, dev, stream_obj, args.steps, args.warmup, world=world,
+                            clocks_index=local if rank == 0 else None, flush_l2=fits_l2, k=args.k)
+    info0 = m["info"]
+    roof = roofline(cfg, info0, m["total_ms_this_rank"], m["launches"], args.steps, peaks_alu)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
     if not args.no_e2e:
-        hbuf = host0.clone().pin_memory()
+        hbuf = torch.from_numpy(cfg["u0"].reshape(-1)).clone().pin_memory()
         plan.level = 0
-        for _ in range(1):
+        for _ in range(args.warmup):
             plan.run_host(hbuf.data_ptr(), levels, stream)
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        ksteps = max(1, min(args.steps, 3))
         t0 = time.perf_counter()
         e0.record(stream_obj)
-        for _ in range(ksteps):
+        for _ in range(args.steps):
             plan.run_host(hbuf.data_ptr(), levels, stream)     # H2D + levels + D2H + stream sync
         e1.record(stream_obj)
         barrier()
         ms = e0.elapsed_time(e1)
         wall = (time.perf_counter() - t0) * 1e3
         tt = max_over_ranks(max(ms, wall), world, dev)
-        e2e = {"value": job_value(units(cfg), ksteps, world, tt), "unit": UNIT,
+        e2e = {"value": job_value(units(cfg), args.steps, world, tt), "unit": UNIT,
                "h2d_bytes_per_step": nelem * es, "d2h_bytes_per_step": nelem * es,
-               "steps": ksteps, "ms_per_step": tt / ksteps}
+               "steps": args.steps, "warmup": args.warmup, "ms_per_step": tt / args.steps}
         del hbuf
+        if rank == 0:
+            pc = pcie_rates(dev, stream_obj)
+            # uploads and downloads overlap (ge_run_host pipelines chunks): the slower direction is the floor
+            floor_ms = max(nelem * es / pc["h2d_gbs"], nelem * es / pc["d2h_gbs"]) / 1e6
+            e2e["pcie"] = dict(pc, ceiling_ms_per_step=floor_ms, frac_of_ceiling=floor_ms / (tt / args.steps),
+                               note="measured on this box with pinned 512 MiB copies, one direction at a time; "
+                                    "the step cannot be faster than its slower copy direction")
 
+    # ---- oracle legs on this box's host cores (rank 0, N = 1 only): parity of the timed configuration, CPU baseline ----
+    parity, cpu = None, None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        parity = parity_check(cfg, plan, dev, stream, k=args.k)
+        cpu = cpu_baseline(args.config, args.cpu_scale, k=args.k, levels=args.levels)
     info = plan.info()
     plan.close()
-    del u
-    if clocks:
-        clocks.close()
+
+    # ---- the other single-GPU configs, device-resident (rank 0, N = 1, default workload only) ----
+    secondary = None
+    if rank == 0 and world == 1 and args.config == "c4" and not args.no_secondary and args.kernel == "auto" and not args.levels:
+        secondary = {}
+        for name in ("c5_f32", "c5_f64", "c2", "c3"):
+            scfg = make_cfg(name)
+            sn = scfg["nx"] * scfg["ny"] * scfg["batch"] * ESIZE[scfg["dtype"]]
+            sm_, splan = device_timing(scfg, {}, dev, stream_obj, 3, 3, clocks_index=local, flush_l2=sn <= 126e6)
+            sroof = roofline(scfg, sm_["info"], sm_["total_ms_this_rank"], sm_["launches"], 3, peaks_alu)
+            spar = parity_check(scfg, splan, dev, stream) if not args.no_cpu else None
+            splan.close()
+            secondary[name] = {"workload": workload_desc(scfg), "value": sm_["value"], "unit": UNIT, "steps": 3, "warmup": 3,
+                               "ms_per_step": sm_["ms_per_step"], "ms_per_step_each": sm_["per_step"],
+                               "kernel": sroof["kernel"], "gpu_launches": sm_["launches"], "finite": sm_["finite"],
+                               "effective_gbs": sm_["value"] * 2 * ESIZE[scfg["dtype"]], "l2": sm_["l2"],
+                               "roofline": {kk: sroof.get(kk) for kk in ("bound", "achieved", "peak", "unit", "frac", "issue_frac", "peak_source", "ms_per_launch", "levels_per_launch")},
+                               "parity": spar, "clocks": sm_["clocks"]}
+            del scfg
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- oracle timed beside it on this box's host cores (rank 0, N = 1 only) ----
-    cpu = None
-    if world == 1 and not args.no_cpu:
-        from oracle import ge_oracle
-        ge_oracle.build()
-        scale = args.cpu_scale
-        scfg = make_cfg(args.config, scale)
-        scfg["k"] = args.k
-        if args.levels:
-            scfg["steps"] = args.levels
-        t = oracle_time(scfg)
-        cpu = {"value": units(scfg) / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": sample_desc(scfg, scale), "seconds": t}
-
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": m["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
         "config": {"workload": workload_desc(cfg), "levels_per_step": levels, "kernel": info["kernel"],
                    "group_k": args.k, "tb": info["resident_tb"] if info["resident_path"] == 2 else (0 if info["resident_path"] else info["tb"]),
                    "resident": {"path": info["resident_path"], "c": info["resident_c"],
                                 "warps": info["resident_warps"], "capacity": info["resident_capacity"],
-                                "meetings_per_step": meetings // max(1, args.steps),
+                                "meetings_per_step": m["meetings"] // max(1, args.steps),
                                 "sync": args.sync or "grid"} if info["resident_path"] else None,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "state %.0f MiB %s L2 (126 MB)" % (nelem * es / 2 ** 20,
-                                                              "larger than" if nelem * es > 126e6 else "fits in"),
+                   "l2": "state %.0f MiB %s L2 (126 MB)%s" % (nelem * es / 2 ** 20, "fits in" if fits_l2 else "larger than",
+                                                             "; " + m["l2"] if m["l2"] else "; no flush needed"),
+                   "state": "consecutive: step i starts from the end state of step i-1 (the cost of a level does not depend on the data); parity is checked on a separate run from u0",
                    "r": float(cfg["r"][0]) if cfg["batch"] == 1 else "per rod U[0.5,8]"},
-        "effective_gbs": value * 2 * es,            # what one-round-trip-per-level would have had to move
-        "ms_per_step_each": per_step,
-        "finite": finite and not fault,
-        "gpu_launches": launches,
+        "effective_gbs": m["value"] * 2 * es,            # what one-round-trip-per-level would have had to move
+        "ms_per_step_each": m["per_step"],
+        "finite": m["finite"],
+        "parity": parity,
+        "gpu_launches": m["launches"],
         "roofline": roof,
+        "alu_peaks": peaks_alu,
         "e2e": e2e,
         "cpu_baseline": cpu,
-        "clocks": clocks.summary() if clocks else None,
+        "clocks": m["clocks"],
+        "secondary": secondary,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_sweep(args):
+    """Synchronisation study on B200: the paper asks where the barriers of its threaded
+    loop must go (Fig 3) and sweeps the number of virtual blocks (Fig 4).
+    The analogue here, on one long rod that fits on the chip (BASELINE.json configs[1], C2): launch per level
+    (strategy A) / per tb levels (B) / one cooperative launch (C) with its kinds of meeting; tile size (values
+    per lane C), halo lanes and meeting interval of strategy C.  One line per setting; every setting runs the
+    same seeded input and must reproduce the first one bit for bit.  `--md FILE` also writes a markdown table."""
+    import torch
+    from paper_1310_3422_b200 import build as gebuild, inputs, libge
+    gebuild.build()
+    libge.load()
+    dev = torch.device("cuda:0")
+    n, levels, reps = args.sweep_n, args.levels or 10000, max(3, args.steps if args.steps != 20 else 5)
+    cfg = inputs.make_c2(n=n, steps=levels)
+    stream_obj = torch.cuda.current_stream(dev)
+    stream = stream_obj.cuda_stream
+    u0 = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
+    sync_names = {libge.GE_SYNC_FLAGS: "flag + fence", libge.GE_SYNC_GRID: "grid barrier",
+                  libge.GE_SYNC_LINES: "flag-in-data", libge.GE_SYNC_STAGGER: "staggered flag-in-data"}
+    settings = [("A: launch per level", dict(kernel="per_step"), {}),
+                ("B: warp-per-tile, tb 16", dict(kernel="temporal", tb=16), {libge.GE_TUNE_TEMPORAL_C: 16}),
+                ("B: TMA-staged, tb 20", dict(kernel="temporal", tb=20), {})]
+    for c in (16, 32, 64):
+        for hl in (1, 2, 3):
+            for sync in (libge.GE_SYNC_FLAGS, libge.GE_SYNC_GRID, libge.GE_SYNC_LINES):
+                settings.append(("C: C=%d, halo %d, %s" % (c, hl, sync_names[sync]), dict(kernel="persistent"),
+                                 {libge.GE_TUNE_RESIDENT_C: c, libge.GE_TUNE_HALO_LANES: hl,
+                                  libge.GE_TUNE_SYNC_MODE: sync}))
+    for tb in (8, 16, 32):
+        for sync in (libge.GE_SYNC_FLAGS, libge.GE_SYNC_GRID, libge.GE_SYNC_LINES):
+            settings.append(("C: C=32, halo 2, %s, tb %d" % (sync_names[sync], tb), dict(kernel="persistent"),
+                             {libge.GE_TUNE_RESIDENT_C: 32, libge.GE_TUNE_HALO_LANES: 2,
+                              libge.GE_TUNE_SYNC_MODE: sync, libge.GE_TUNE_TB: tb}))
+    for c, hl in ((32, 2), (32, 1), (64, 2)):
+        settings.append(("C: C=%d, halo %d, %s" % (c, hl, sync_names[libge.GE_SYNC_STAGGER]), dict(kernel="persistent"),
+                         {libge.GE_TUNE_RESIDENT_C: c, libge.GE_TUNE_HALO_LANES: hl,
+                          libge.GE_TUNE_SYNC_MODE: libge.GE_SYNC_STAGGER}))
+    rows, first = [], None
+    for name, kw, tune in settings:
+        try:
+            plan = libge.Plan(cfg, stream=stream, **kw)
+            for what, value in tune.items():
+                plan.tune(what, value)
+        except libge.GeError as e:
+            print("%-44s skipped (%s)" % (name, e))
+            continue
+        u = u0.clone()
+        plan.run(u.data_ptr(), levels, stream)          # warm-up, and the result to compare
+        torch.cuda.synchronize(dev)
+        res = u.cpu().numpy()
+        if first is None:
+            first = res
+        same = bool(np.array_equal(res, first))
+        ts = []
+        m0 = plan.info()["meetings"]
+        for _ in range(reps):
+            plan.level = 0
+            u.copy_(u0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream_obj)
+            plan.run(u.data_ptr(), levels, stream)
+            e1.record(stream_obj)
+            torch.cuda.synchronize(dev)
+            ts.append(e0.elapsed_time(e1))
+        info = plan.info()
+        meetings = (info["meetings"] - m0) // reps
+        fault = plan.sync_fault() if info["resident_path"] == 2 else 0
+        plan.close()
+        ms = statistics.median(ts)
+        glups = n * levels / ms / 1e6
+        rows.append((name, info["kernel"], info["resident_tb"] or info["tb"], meetings, info["resident_warps"], ms,
+                     glups, same and not fault))
+        print("%-44s %-10s tb %3d meetings %5d tiles %5d  %8.3f ms  %8.1f GLUPS  %s" % (
+            name, info["kernel"], rows[-1][2], meetings, info["resident_warps"], ms, glups,
+            "bit-identical" if rows[-1][-1] else "MISMATCH"), flush=True)
+    if args.md:
+        with open(args.md, "w") as f:
+            f.write("| setting | kernel | tb | meetings per run | tiles | ms per run | GLUPS | bit-identical |\n|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s | %s | %d | %d | %d | %.3f | %.1f | %s |\n" % (r[0], r[1], r[2], r[3], r[4], r[5], r[6],
+                                                                       "yes" if r[7] else "NO"))
+    if not all(r[-1] for r in rows):
+        raise SystemExit(1)
 
 
 def run_src(args):
@@ -454,7 +767,7 @@ def traffic_of(kernel_key):
         return json.load(f).get(kernel_key, {}).get("dram_bytes_per_launch")
 
 
-def roofline(cfg, info, total_ms, launches, steps):
+def roofline(cfg, info, total_ms, launches, steps, alu=None):
     """The step is `launches/steps` launches of ONE kernel; its average duration is the CUDA-event
     time of the timed region divided by the launches in it.  Per-level kernel: HBM-bound, achieved =
     algorithmic bytes (2*sizeof(T) per update) per second against the measured copy
@@ -482,7 +795,8 @@ def roofline(cfg, info, total_ms, launches, steps):
     key = "%s/%s" % (cfg["name"], name)
     eff = 2.0 * es * upd / (ms * 1e-3) / 1e9
     out = {"kernel": name, "levels_per_launch": lv, "launches_timed": launches, "ms_per_launch": ms,
-           "traffic": traffic_of(key), "peak_source": src,
+           "traffic": traffic_of(key), "traffic_source": "profiles/traffic.json: dram bytes read + written per launch from a separate `ncu --set full` capture of this kernel on this workload (not measured in this run)",
+           "peak_source": src,
            "algorithmic_bytes_per_launch": 2.0 * es * upd, "effective_gbs": eff,
            "effective_frac_of_hbm": eff / peaks["hbm_gbs"]}
     if kernel == "per_step" or lv <= 1.0:
@@ -490,10 +804,15 @@ def roofline(cfg, info, total_ms, launches, steps):
                     "frac": eff / peaks["hbm_gbs"]})
     else:
         clk = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-        peak = 2.0 * LANES[cfg["dtype"]] * SMS * clk / 1e12
+        derived = 2.0 * LANES[cfg["dtype"]] * SMS * clk / 1e12
+        measured = (alu or {}).get(cfg["dtype"] + "_tflops")
+        peak = measured or derived
         ach = FLOPS[cfg["dim"]] * upd / (ms * 1e-3) / 1e12
+        # issue terms: FP instructions of the factored form per second against the probe's FMA instructions per second
         out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                    "issue_frac": INSTR[cfg["dim"]] * upd / (ms * 1e-3) / (LANES[cfg["dtype"]] * SMS * clk),
+                    "issue_frac": INSTR[cfg["dim"]] * upd / (ms * 1e-3) / (peak * 1e12 / 2.0),
+                    "peak_source": "measured (in-run FMA microbenchmark, ge_fma_probe)" if measured else "derived",
+                    "peak_derived": derived,
                     "peak_derivation": "2 flop x %d %s lanes/SM x %d SMs x %.0f MHz" % (
                         LANES[cfg["dtype"]], cfg["dtype"], SMS, clk / 1e6)})
     return out
@@ -516,14 +835,20 @@ def main():
     ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines", "stagger"], help="whole-chip persistent kernel: meeting kind")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
     ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
+    ap.add_argument("--sweep", default="", choices=["", "sync"], help="sync: the synchronisation study on the C2-shaped rod (NEXT-2)")
+    ap.add_argument("--sweep-n", type=int, default=2 ** 20, help="--sweep: nodes of the rod")
+    ap.add_argument("--md", default="", help="--sweep: also write a markdown table to this file")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--cpu-scale", type=float, default=1 / 32, help="grid fraction of the cpu_baseline sample")
-    ap.add_argument("--ref-scale", type=float, default=1 / 256, help="grid fraction of the --impl reference sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle legs (parity, cpu_baseline)")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the C5 / C2 / C3 block of the default line")
+    ap.add_argument("--cpu-scale", type=float, default=1 / 128, help="grid fraction of the cpu_baseline sample")
+    ap.add_argument("--ref-scale", type=float, default=1 / 128, help="grid fraction of the --impl reference sample (the same sample)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         sys.stderr.write("bench.py: warning: fewer than 3 warm-up steps; the number is not reportable\n")
-    if args.src:
+    if args.sweep:
+        run_sweep(args)
+    elif args.src:
         run_src(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -161,7 +161,7 @@ enum {
                                   warp-per-tile kernel; 18, 22, 26 (f64) / 36, 44, 52 (f32): TMA-staged persistent kernel, 22 / 52 the
                                   default for rods of >= 4 tiles (needs nx >= 32 * value)                   */
     GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
-                                  2-D: one of the compiled-in block lengths 4, 8)                            */
+                                  2-D: one of the compiled-in block lengths 4, 6, 8; 6 needs the strip kernel)                            */
     GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64) */
     GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
                                   long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
@@ -173,6 +173,15 @@ enum {
                                   taking opposite turns (needs tb >= 8); default 1, the fastest measured            */
 };
 int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
+
+/* Measurement helper, not part of the path ("64 fp64 lanes -- assumption, measure with an FMA
+ * microbenchmark"): enqueues ONE launch of a kernel in which each of 2048 threads per SM runs 8 independent
+ * chains of `iters` dependent fused multiply-adds of `dtype` (ge_dtype), and stores in *flops the
+ * floating-point operations of that launch (an FMA counts 2).  The caller times the launch with events on
+ * `stream`; flops / seconds is the sustained FFMA / DFMA rate of the chip at the clock it holds.
+ * sink: device pointer to at least 8 writable bytes (never written in practice).  GE_EINVAL for a bad
+ * dtype, iters < 1 or a null pointer. */
+int ge_fma_probe(int32_t dtype, int64_t iters, void *sink, double *flops, ge_stream_t stream);
 
 /* Frees the plan's device buffers (stream-ordered on the stream last used) and the plan. */
 int ge_plan_destroy(ge_plan *p);

@@ -22,7 +22,7 @@ NVCC_FLAGS = [
     "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",            # every fma in the kernels is written out; no implicit contraction
     "-Xcompiler", "-fPIC", "-shared",
-    "-cudart", "static",
+    "-cudart", "static", "-ldl",
 ]
 
 

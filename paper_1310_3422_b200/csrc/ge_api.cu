@@ -4,6 +4,7 @@
 #include "../../include/ge.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>     // header-only NVTX v3: ranges around ge_run / ge_run_host
 
 #include <cmath>
 #include <cstdio>
@@ -21,6 +22,7 @@
 #include "ge_level_k.cuh"
 #include "ge_level_src.cuh"
 #include "ge_level3d.cuh"
+#include "ge_probe.cuh"
 
 namespace {
 
@@ -37,6 +39,12 @@ thread_local cudaError_t g_last_cuda = cudaSuccess;
     } while (0)
 
 inline size_t elem_size(int dtype) { return dtype == GE_F64 ? 8 : 4; }
+
+// NVTX range for the lifetime of the object (a no-op unless a profiler has injected itself)
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 }  // namespace
 
@@ -523,6 +531,7 @@ int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
 
 // Decide the strategy-C path at plan creation / after a tuning call.
 int resident_configure(ge_plan* p, int want_c) {
+    if (p->group_k != 1) return GE_EUNSUPPORTED;       // two-point groups only (callers check; never silently k = 1)
     p->res_path = 0;
     if (p->dim != 1) return GE_OK;
     const int* cs = resident_c_list(p->dtype);
@@ -691,6 +700,7 @@ int ge_step_3d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
 
 int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     if (!p || !u || steps < 0) return GE_EINVAL;
+    NvtxRange nvtx("ge_run");
     const size_t es = elem_size(p->dtype);
     if ((uintptr_t)u % es) return GE_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -897,6 +907,7 @@ static int host_pipeline_rods(ge_plan* p, void* u_host, int64_t steps, cudaStrea
 
 int ge_run_host(ge_plan* p, void* u_host, int64_t steps, ge_stream_t stream) {
     if (!p || !u_host || steps < 0) return GE_EINVAL;
+    NvtxRange nvtx("ge_run_host");
     cudaStream_t s = (cudaStream_t)stream;
     const size_t bytes = (size_t)p->count * elem_size(p->dtype);
     if (p->dim == 1 && p->batch == 1 && p->group_k == 1 && steps > 0 && p->nx >= 2 * kHostChunk &&
@@ -941,13 +952,19 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
         case GE_INFO_KERNEL: *value = p->kernel; return GE_OK;
         case GE_INFO_TB: *value = p->tb; return GE_OK;
         case GE_INFO_LAUNCHES: *value = p->launches; return GE_OK;
-        case GE_INFO_TILE_VALID:
-            *value = p->kernel != GE_KERNEL_TEMPORAL ? 0
-                     : p->dim == 1 ? ge::temporal1d_geom(p->tc, p->dtype == GE_F64 ? 2 : 4, p->tb, 1).valid
-                                   : ge::temporal2d_geom(p->tc, p->dtype == GE_F64 ? 2 : 4, p->tb, 0, p->nx, p->ny, p->hp).valid;
+        case GE_INFO_TILE_VALID: {
+            const int V = p->dtype == GE_F64 ? 2 : 4;
+            if (p->kernel != GE_KERNEL_TEMPORAL) *value = 0;
+            else if (p->dim == 1) *value = ge::temporal1d_geom(p->tc, V, p->tb, 1).valid;
+            else if (strip2d_ok(p))   // the kernel that runs: strips of 32*C columns, halo stale columns per side
+                *value = ge::strip2d_geom(p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c, V, p->tb, p->nx, p->ny, p->hp).valid;
+            else *value = ge::temporal2d_geom(p->tc, V, p->tb, 0, p->nx, p->ny, p->hp).valid;
             return GE_OK;
+        }
         case GE_INFO_TILE_LOADED:
-            *value = p->kernel == GE_KERNEL_TEMPORAL ? 32 * p->tc : 0;
+            if (p->kernel != GE_KERNEL_TEMPORAL) *value = 0;
+            else if (p->dim == 2 && strip2d_ok(p)) *value = 32 * (p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c);
+            else *value = 32 * p->tc;
             return GE_OK;
         case GE_INFO_TEMPORAL_C: *value = p->kernel == GE_KERNEL_TEMPORAL && p->dim == 1 ? p->tc : 0; return GE_OK;
         case GE_INFO_RESIDENT_PATH: *value = p->kernel == GE_KERNEL_PERSISTENT ? p->res_path : 0; return GE_OK;
@@ -991,6 +1008,8 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_RESIDENT_C: {
             // path 1: values per lane (warps follow); path 2: values per lane of a tile
             if (p->kernel != GE_KERNEL_PERSISTENT || value < 2 || value > 128) return GE_EINVAL;
+            // the register-resident kernels are the k = 1 scheme; a k >= 2 plan stays on its shared-memory path
+            if (p->group_k >= 2 || p->res_path == 3) return GE_EUNSUPPORTED;
             const int32_t path0 = p->res_path, c0 = p->res_c, w0 = p->res_w;
             p->res_tb = 0;                                     // back to the largest the new halo allows
             int rc = resident_configure(p, (int)value);
@@ -1040,6 +1059,17 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             return GE_OK;
         default: return GE_EINVAL;
     }
+}
+
+int ge_fma_probe(int32_t dtype, int64_t iters, void* sink, double* flops, ge_stream_t stream) {
+    if ((dtype != GE_F32 && dtype != GE_F64) || iters < 1 || !sink || !flops) return GE_EINVAL;
+    int dev = 0, sms = 0;
+    GE_CUDA(cudaGetDevice(&dev));
+    GE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const cudaError_t e = dtype == GE_F64 ? ge::fma_probe_launch<double>((double*)sink, iters, sms, flops, (cudaStream_t)stream)
+                                          : ge::fma_probe_launch<float>((float*)sink, iters, sms, flops, (cudaStream_t)stream);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    return GE_OK;
 }
 
 int ge_plan_destroy(ge_plan* p) {

@@ -1,0 +1,50 @@
+// ge_probe.cuh -- measurement helper, not on the hot path: sustained FFMA / DFMA throughput of the chip.
+//
+// SURVEY.md 8(d) bounds the temporally blocked and resident kernels by the plain fp32 / fp64 pipes and
+// flags the lane counts (128 fp32, 64 fp64 per SM) as an assumption "to be measured with an FMA
+// microbenchmark".  This is that microbenchmark: every thread runs CHAINS independent dependent-FMA
+// chains (x <- x*a + b), 2048 threads per SM, so latency is covered many times over and the only limit
+// left is the issue rate of the pipe at the clock the GPU actually holds.  bench.py times it with CUDA
+// events and uses the result as `roofline.peak` of the "alu"-bound kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ge {
+
+constexpr int kProbeChains = 8;
+constexpr int kProbeThreads = 256;
+constexpr int kProbeBlocksPerSm = 8;      // 2048 threads per SM
+
+template <typename T>
+__global__ void __launch_bounds__(kProbeThreads, kProbeBlocksPerSm)
+ge_fma_probe_kernel(T* __restrict__ sink, T a, T b, int64_t iters) {
+    T x[kProbeChains];
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) x[c] = T(threadIdx.x + c) * a;
+#pragma unroll 1
+    for (int64_t i = 0; i < iters; i += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int c = 0; c < kProbeChains; ++c) x[c] = fma(x[c], a, b);
+    }
+    T s = T(0);
+#pragma unroll
+    for (int c = 0; c < kProbeChains; ++c) s += x[c];
+    // a is chosen < 1 by the host, so the chains converge to b/(1-a): the store below never happens,
+    // but the compiler cannot know
+    if (s == T(-1)) sink[0] = s;
+}
+
+// Enqueues one launch; returns the flops it performs (an FMA counts 2).
+template <typename T>
+inline cudaError_t fma_probe_launch(T* sink, int64_t iters, int sm_count, double* flops, cudaStream_t s) {
+    iters = (iters + 3) / 4 * 4;
+    const int blocks = sm_count * kProbeBlocksPerSm;
+    ge_fma_probe_kernel<T><<<blocks, kProbeThreads, 0, s>>>(sink, T(0.999), T(0.001), iters);
+    *flops = 2.0 * kProbeChains * (double)iters * (double)blocks * kProbeThreads;
+    return cudaGetLastError();
+}
+
+}  // namespace ge

@@ -70,8 +70,6 @@ def rel_err(got, ref):
     """max-abs error relative to max|oracle| (reading R-A7); per rod for batched input."""
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
-    if ref.ndim == 2 and got.shape == ref.shape and ref.shape[0] > 1 and False:
-        pass
     return float(np.abs(got - ref).max() / max(np.abs(ref).max(), 1e-300))
 
 

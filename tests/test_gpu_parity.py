@@ -234,6 +234,26 @@ def test_general_k_resident_needs_the_rod_to_fit():
     assert info["kernel"] == "per_step"
 
 
+def test_general_k_plan_rejects_the_two_point_resident_tuning(oracle):
+    """GE_TUNE_RESIDENT_C configures the register-resident kernels, which are the k = 1 scheme: a k >= 2 plan
+    on its shared-memory resident path must refuse it (and keep computing the k = 16 scheme)."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    cfg = inputs.random_rods(2, 8192 - 2, "f64", seed=3)
+    u = torch.from_numpy(cfg["u0"]).to("cuda:0")
+    with libge.Plan(cfg, group_k=16, kernel="persistent") as plan:
+        assert plan.info()["resident_path"] == 3
+        for c in (8, 16, 32, 64):
+            with pytest.raises(libge.GeError) as ei:
+                plan.tune(libge.GE_TUNE_RESIDENT_C, c)
+            assert ei.value.status == libge.GE_EUNSUPPORTED
+        assert plan.info()["resident_path"] == 3
+        plan.run(u.data_ptr(), 30)
+        torch.cuda.synchronize()
+    ref = run_oracle(oracle, cfg, 30, k=16)
+    assert rel_err_rows(u.cpu().numpy(), ref, cfg) <= TOL["f64"]
+
+
 def test_general_k_matches_the_closed_form(oracle):
     """k = 16 on N = 254 (the paper's SDC width 32): the end state follows e^{-pi^2 t} sin(pi x) to the
     oracle's own error (tests/golden P6: 5.35e-5 at t ~ 0.1, r = 1)."""
