@@ -213,6 +213,12 @@ class ClockSampler:
         for ln in self.proc.stdout:
             self.rows.append((time.monotonic(), ln.strip()))
 
+    def wait_ready(self, timeout=2.0):
+        """nvidia-smi needs a few hundred ms to deliver its first row; short timed regions would see none"""
+        t = time.monotonic()
+        while self.proc and not self.rows and time.monotonic() - t < timeout:
+            time.sleep(0.02)
+
     def begin(self):
         self.t0 = time.monotonic()
 
@@ -422,6 +428,12 @@ def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clock
     for key, what in (("tc", libge.GE_TUNE_TEMPORAL_C), ("rc", libge.GE_TUNE_RESIDENT_C), ("hl", libge.GE_TUNE_HALO_LANES)):
         if args_like.get(key):
             plan.tune(what, args_like[key])
+    if args_like.get("hp"):
+        plan.tune(libge.GE_TUNE_SEG_PAIRS, args_like["hp"])
+    if args_like.get("coop") is not None and args_like.get("coop") >= 0:
+        plan.tune(libge.GE_TUNE_STRIP_COOP, args_like["coop"])
+    if args_like.get("form3d") is not None and args_like.get("form3d") >= 0:
+        plan.tune(libge.GE_TUNE_FORM_3D, args_like["form3d"])
     if args_like.get("sync"):
         plan.tune(libge.GE_TUNE_SYNC_MODE, SYNC_IDS[args_like["sync"]])
     if args_like.get("rtb"):
@@ -437,6 +449,7 @@ def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clock
     e1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
     barrier()
     if clocks:
+        clocks.wait_ready()
         clocks.begin()
     for i in range(steps):
         if flush is not None:
@@ -494,7 +507,8 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     peaks_alu = fma_peaks(dev, stream_obj)
-    tune = dict(kernel=args.kernel, tb=args.tb, tc=args.tc, rc=args.rc, hl=args.hl, sync=args.sync, rtb=args.rtb)
+    tune = dict(kernel=args.kernel, tb=args.tb, tc=args.tc, rc=args.rc, hl=args.hl, sync=args.sync, rtb=args.rtb,
+                hp=args.hp, coop=args.coop, form3d=args.form3d)
 
     cfg = make_cfg(args.config)
     if args.levels:
@@ -833,6 +847,9 @@ def main():
     ap.add_argument("--hl", type=int, default=0, help="whole-chip persistent kernel: halo lanes per side")
     ap.add_argument("--rtb", type=int, default=0, help="whole-chip persistent kernel: levels between meetings")
     ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines", "stagger"], help="whole-chip persistent kernel: meeting kind")
+    ap.add_argument("--hp", type=int, default=0, help="2-D strip kernel: output row pairs per segment")
+    ap.add_argument("--coop", type=int, default=-1, help="2-D strip kernel: warps sharing one strip (0, 4, 8; -1 = plan default)")
+    ap.add_argument("--form3d", type=int, default=-1, help="3-D: 1 streaming + shell kernels, 0 a thread per group (-1 = plan default)")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
     ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
     ap.add_argument("--sweep", default="", choices=["", "sync"], help="sync: the synchronisation study on the C2-shaped rod (NEXT-2)")

@@ -166,6 +166,12 @@ enum {
     GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
                                   long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
     GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */
+    GE_TUNE_STRIP_COOP = 6,    /* 2-D strip kernel: warps of a CTA that share ONE strip and exchange their edge columns
+                                  every level through shared memory and named barriers instead of each recomputing
+                                  tb stale columns per side (0 = a warp per strip; 4, 8; needs tb = 6 and
+                                  nx >= value * 32 * columns per lane)                                              */
+    GE_TUNE_FORM_3D = 7,       /* 3-D per-level kernels: 1 = streaming kernel for the deep groups + shell kernel for the
+                                  outermost layer of groups (default, two launches per level), 0 = a thread per group    */
     GE_TUNE_SYNC_MODE = 5      /* path 2, how the tiles meet: 0 = neighbour flags (data, release fence, flag per
                                   tile, acquire), 1 = grid-wide barrier (cooperative groups), 2 = neighbour
                                   flag-in-data lines (no fence, no separate flag), 3 = the same lines published

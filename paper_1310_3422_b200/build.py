@@ -21,17 +21,22 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",            # every fma in the kernels is written out; no implicit contraction
-    "-Xcompiler", "-fPIC", "-shared",
-    "-cudart", "static", "-ldl",
+    "-Xcompiler", "-fPIC",
 ]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-ldl"]
+OBJ = os.path.join(_HERE, "lib", "obj")
 
 
 def _sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
+def _headers():
+    return glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(INCLUDE, "*.h"))
+
+
 def _deps():
-    return _sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(INCLUDE, "*.h"))
+    return _sources() + _headers()
 
 
 def needs_build() -> bool:
@@ -42,19 +47,45 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Every .cu of csrc/ is a translation unit of its own (the kernel families compile in parallel); objects are
+    cached under lib/obj and recompiled when the source, any header or the flags changed."""
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    tmp = LIB + ".tmp.%d" % os.getpid()
     extra = os.environ.get("GE_NVCC_EXTRA", "").split()        # e.g. -DGE_STRIP_MINB_F32=4 for tuning sweeps
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + _sources()
-    proc = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    if verbose or proc.returncode != 0:
-        sys.stderr.write(proc.stdout)
+    os.makedirs(OBJ, exist_ok=True)
+    hdr_time = max(os.path.getmtime(f) for f in _headers())
+    flags_tag = " ".join(NVCC_FLAGS + extra)
+    jobs, objs = [], []
+    for src in _sources():
+        obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+        tag = obj + ".flags"
+        objs.append(obj)
+        fresh = (not force and os.path.exists(obj) and os.path.exists(tag) and open(tag).read() == flags_tag
+                 and os.path.getmtime(obj) > max(hdr_time, os.path.getmtime(src)))
+        if fresh:
+            continue
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-c", "-o", obj, src]
+        jobs.append((src, tag, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    failed = False
+    for src, tag, proc in jobs:
+        out, _ = proc.communicate()
+        if verbose or proc.returncode != 0:
+            sys.stderr.write(out)
+        if proc.returncode != 0:
+            failed = True
+        else:
+            with open(tag, "w") as f:
+                f.write(flags_tag)
+    if failed:
+        raise RuntimeError("nvcc failed building libge.so")
+    tmp = LIB + ".tmp.%d" % os.getpid()
+    proc = subprocess.run([nvcc] + LINK_FLAGS + ["-o", tmp] + objs, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if proc.returncode != 0:
+        sys.stderr.write(proc.stdout)
         if os.path.exists(tmp):
             os.remove(tmp)
-        raise RuntimeError("nvcc failed building libge.so (exit %d)" % proc.returncode)
+        raise RuntimeError("nvcc failed linking libge.so (exit %d)" % proc.returncode)
     os.replace(tmp, LIB)
     return LIB
 

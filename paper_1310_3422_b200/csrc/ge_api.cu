@@ -18,10 +18,9 @@
 #include "ge_temporal2d.cuh"
 #include "ge_resident.cuh"
 #include "ge_stream.cuh"
-#include "ge_strip2d.cuh"
+#include "ge_dispatch.h"
 #include "ge_level_k.cuh"
 #include "ge_level_src.cuh"
-#include "ge_level3d.cuh"
 #include "ge_probe.cuh"
 
 namespace {
@@ -80,7 +79,9 @@ struct ge_plan {
     HostSlot* slots;          // kHostSlots entries (lazy)
     ge_desc host_desc;        // shape of this plan for the sub-plans (r, boundary values below)
     double host_r, host_lo, host_hi;
-    int32_t strip_attr_tb;    // block length whose strip-kernel function attributes are set on this device (0: none)
+    int32_t strip_attr_tb;    // strip-kernel instantiation (tb*16 + coop) whose function attributes are set on this device (0: none)
+    int32_t form3d;           // 3-D per-level form: 1 streaming + shell kernels (default), 0 a thread per group
+    int32_t strip_coop;       // warps that share one strip of the 2-D strip kernel (0: a warp per strip)
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
     bool rodk_attr;           // ... and of its shared-memory-resident form
 };
@@ -241,11 +242,12 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
         rc = p->dtype == GE_F64 ? launch_level_k<double>(p, uin, uout, phase, s)
                                 : launch_level_k<float>(p, uin, uout, phase, s);
     else if (p->dim == 3) {
-        cudaError_t e = p->dtype == GE_F64
-            ? ge::level3d_launch<double>((const double*)uin, (double*)uout, p->nx, p->ny, p->nz, (const ge::Coef3<double>*)p->coef, phase, s)
-            : ge::level3d_launch<float>((const float*)uin, (float*)uout, p->nx, p->ny, p->nz, (const ge::Coef3<float>*)p->coef, phase, s);
+        // the streaming form (deep groups) + shell, unless the grid is too small to have deep groups worth a launch
+        const int form = p->form3d && p->nx >= 8 && p->ny >= 8 && p->nz >= 8 ? 1 : 0;
+        int n = 0;
+        const cudaError_t e = ge::level3d_dispatch(p->dtype, form, uin, uout, p->nx, p->ny, p->nz, p->coef, phase, p->sm_count, s, &n);
         if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
-        p->launches += 1;
+        p->launches += n;
         rc = GE_OK;
     }
     else if (p->dim == 1) rc = p->dtype == GE_F64 ? launch_level_1d<double>(p, uin, uout, phase, s)
@@ -333,33 +335,23 @@ int launch_temporal_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) 
     p->level += p->tb;
     return GE_OK;
 }
-// ---- strategy B launch (2-D, drift-free strips): plan->tb levels from the current PHASE-1 level ----
-#ifndef GE_STRIP_C_F32
-#define GE_STRIP_C_F32 4
-#endif
-#ifndef GE_STRIP_C_F64
-#define GE_STRIP_C_F64 2
-#endif
-template <typename T> struct StripC { static constexpr int c = sizeof(T) == 8 ? GE_STRIP_C_F64 : GE_STRIP_C_F32; };
+// ---- strategy B launch (2-D, drift-free strips; ge_strip2d.cu): plan->tb levels from the current PHASE-1 level ----
 bool strip2d_ok(const ge_plan* p) {
-    const int c = p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c;
-    return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * c;
+    return p->dim == 2 && p->nx % 4 == 0 && p->nx >= 32 * ge::strip2d_columns_per_lane(p->dtype);
+}
+// COOP warps of a CTA share one strip (GE_TUNE_STRIP_COOP): the grid must hold at least one such strip
+bool strip2d_coop_ok(const ge_plan* p, int64_t coop) {
+    return coop == 0 || (strip2d_ok(p) && ge::strip2d_coop_compiled(p->dtype, p->tb, (int)coop) &&
+                         p->nx >= coop * 32 * ge::strip2d_columns_per_lane(p->dtype));
 }
 
-template <typename T>
 int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
-    auto* in = (const T*)uin;
-    auto* out = (T*)uout;
-    auto* c = (const ge::Coef2<T>*)p->coef;
-    cudaError_t e;
-    bool configured = p->strip_attr_tb == p->tb;
-    switch (p->tb) {
-        case 4: e = ge::strip2d_launch<T, StripC<T>::c, 4>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
-        case 6: e = ge::strip2d_launch<T, StripC<T>::c, 6>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
-        case 8: e = ge::strip2d_launch<T, StripC<T>::c, 8>(in, out, p->nx, p->ny, c, p->hp, configured, s); break;
-        default: return GE_EINVAL;
-    }
-    if (configured) p->strip_attr_tb = p->tb;
+    if (!ge::strip2d_tb_compiled(p->tb)) return GE_EINVAL;
+    const int coop = strip2d_coop_ok(p, p->strip_coop) ? p->strip_coop : 0;
+    const int key = p->tb * 16 + coop;
+    bool configured = p->strip_attr_tb == key;
+    const cudaError_t e = ge::strip2d_dispatch(p->dtype, p->tb, coop, uin, uout, p->nx, p->ny, p->coef, p->hp, configured, s);
+    if (configured) p->strip_attr_tb = key;
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     p->launches += 1;
     p->level += p->tb;
@@ -629,6 +621,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->tb = 0;
     p->tc = default_tc(p->dtype, p->nx);
     p->hp = p->dtype == GE_F64 ? 56 : 67;   // measured on C5 (the rate depends on the segment count, and sharply)
+    p->form3d = 1;
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
@@ -731,8 +724,7 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                 rc = launch_level(p, cur, oth, s);
                 left -= 1;
             } else if (strips && left >= p->tb && (p->level & 1) == 1) {
-                rc = p->dtype == GE_F64 ? launch_strip_2d<double>(p, cur, oth, s)
-                                        : launch_strip_2d<float>(p, cur, oth, s);
+                rc = launch_strip_2d(p, cur, oth, s);
                 left -= p->tb;
             } else if (!strips && left >= p->tb) {
                 rc = p->dtype == GE_F64 ? launch_temporal_2d<double>(p, cur, oth, s)
@@ -952,20 +944,18 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
         case GE_INFO_KERNEL: *value = p->kernel; return GE_OK;
         case GE_INFO_TB: *value = p->tb; return GE_OK;
         case GE_INFO_LAUNCHES: *value = p->launches; return GE_OK;
-        case GE_INFO_TILE_VALID: {
+        case GE_INFO_TILE_VALID:
+        case GE_INFO_TILE_LOADED: {
             const int V = p->dtype == GE_F64 ? 2 : 4;
-            if (p->kernel != GE_KERNEL_TEMPORAL) *value = 0;
-            else if (p->dim == 1) *value = ge::temporal1d_geom(p->tc, V, p->tb, 1).valid;
-            else if (strip2d_ok(p))   // the kernel that runs: strips of 32*C columns, halo stale columns per side
-                *value = ge::strip2d_geom(p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c, V, p->tb, p->nx, p->ny, p->hp).valid;
-            else *value = ge::temporal2d_geom(p->tc, V, p->tb, 0, p->nx, p->ny, p->hp).valid;
+            int valid = 0, loaded = 0;
+            if (p->kernel != GE_KERNEL_TEMPORAL) { }
+            else if (p->dim == 1) { valid = ge::temporal1d_geom(p->tc, V, p->tb, 1).valid; loaded = 32 * p->tc; }
+            else if (strip2d_ok(p))   // the kernel that runs: strips of (coop*)32*C columns, halo stale columns per side
+                ge::strip2d_tile(p->dtype, p->tb, strip2d_coop_ok(p, p->strip_coop) ? p->strip_coop : 0, p->nx, p->ny, p->hp, &valid, &loaded);
+            else { valid = ge::temporal2d_geom(p->tc, V, p->tb, 0, p->nx, p->ny, p->hp).valid; loaded = 32 * p->tc; }
+            *value = what == GE_INFO_TILE_VALID ? valid : loaded;
             return GE_OK;
         }
-        case GE_INFO_TILE_LOADED:
-            if (p->kernel != GE_KERNEL_TEMPORAL) *value = 0;
-            else if (p->dim == 2 && strip2d_ok(p)) *value = 32 * (p->dtype == GE_F64 ? StripC<double>::c : StripC<float>::c);
-            else *value = 32 * p->tc;
-            return GE_OK;
         case GE_INFO_TEMPORAL_C: *value = p->kernel == GE_KERNEL_TEMPORAL && p->dim == 1 ? p->tc : 0; return GE_OK;
         case GE_INFO_RESIDENT_PATH: *value = p->kernel == GE_KERNEL_PERSISTENT ? p->res_path : 0; return GE_OK;
         case GE_INFO_RESIDENT_C: *value = p->res_path ? p->res_c : 0; return GE_OK;
@@ -995,6 +985,14 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_SEG_PAIRS:
             if (value < 1 || value > (1 << 20) || p->dim != 2) return GE_EINVAL;
             p->hp = (int32_t)value;
+            return GE_OK;
+        case GE_TUNE_FORM_3D:
+            if (p->dim != 3 || (value != 0 && value != 1)) return GE_EINVAL;
+            p->form3d = (int32_t)value;
+            return GE_OK;
+        case GE_TUNE_STRIP_COOP:
+            if (p->dim != 2 || p->kernel != GE_KERNEL_TEMPORAL || (value != 0 && !strip2d_coop_ok(p, value))) return GE_EINVAL;
+            p->strip_coop = (int32_t)value;
             return GE_OK;
         case GE_TUNE_TEMPORAL_C: {
             if (p->dim != 1) return GE_EINVAL;

@@ -42,6 +42,15 @@ struct Coef2 {
     T pad[7];
 };
 
+// 3-D coefficients (one set per plan; ge_level3d.cuh).
+template <typename T>
+struct Coef3 {
+    T r;
+    T c1, c2, c3;          // 2r/(1+2r)/8, 4r/(1+4r)/8, 6r/(1+6r)/8
+    T lo[3], hi[3];        // face values: x, y, z
+    T pad[6];
+};
+
 template <typename T> struct VecOf;
 template <> struct VecOf<float>  { using type = float4;  static constexpr int V = 4; };
 template <> struct VecOf<double> { using type = double2; static constexpr int V = 2; };

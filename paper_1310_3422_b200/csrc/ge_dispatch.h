@@ -1,0 +1,25 @@
+// ge_dispatch.h -- non-template entry points of the kernel families that live in their own translation
+// units (so that the families compile in parallel); called by ge_api.cu only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ge {
+
+// 2-D strip kernels (ge_strip2d.cu).  dtype: 0 = f32, 1 = f64 (ge_dtype).  coop: 0 = a warp per strip
+// (ge2d_strip_kernel), 4 / 8 = that many warps of a CTA share one strip (ge2d_strip_coop_kernel).
+// `configured`: the caller's per-plan flag for the function attributes of the instantiation last used.
+cudaError_t strip2d_dispatch(int dtype, int tb, int coop, const void* uin, void* uout, int64_t nx, int64_t ny,
+                             const void* coef, int hp, bool& configured, cudaStream_t s);
+int strip2d_columns_per_lane(int dtype);                       // C of the instantiations for that dtype
+bool strip2d_tb_compiled(int tb);                              // 4, 6, 8
+bool strip2d_coop_compiled(int dtype, int tb, int coop);
+// valid output columns per strip and columns a strip loads, for ge_plan_info
+void strip2d_tile(int dtype, int tb, int coop, int64_t nx, int64_t ny, int hp, int* valid, int* loaded);
+
+// 3-D per-level kernels (ge_stream3d.cu).  form 0: a thread per group (ge3d_level_kernel); form 1: the streaming
+// kernel for the deep groups + the shell kernel for the outermost layer (two launches).
+cudaError_t level3d_dispatch(int dtype, int form, const void* uin, void* uout, int64_t nx, int64_t ny, int64_t nz,
+                             const void* coef, int phase, int sm_count, cudaStream_t s, int* launches);
+
+}  // namespace ge

@@ -21,14 +21,6 @@
 
 namespace ge {
 
-template <typename T>
-struct Coef3 {
-    T r;
-    T c1, c2, c3;          // 2r/(1+2r)/8, 4r/(1+4r)/8, 6r/(1+6r)/8
-    T lo[3], hi[3];        // face values: x, y, z
-    T pad[6];
-};
-
 #ifndef GE_L3D_BX
 #define GE_L3D_BX 16
 #endif

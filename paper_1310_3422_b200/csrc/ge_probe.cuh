@@ -13,6 +13,7 @@
 namespace ge {
 
 constexpr int kProbeChains = 8;
+constexpr int kProbeUnroll = 32;
 constexpr int kProbeThreads = 256;
 constexpr int kProbeBlocksPerSm = 8;      // 2048 threads per SM
 
@@ -22,10 +23,11 @@ ge_fma_probe_kernel(T* __restrict__ sink, T a, T b, int64_t iters) {
     T x[kProbeChains];
 #pragma unroll
     for (int c = 0; c < kProbeChains; ++c) x[c] = T(threadIdx.x + c) * a;
+    // 32 x 8 = 256 FMAs per trip: the counter, compare and branch are 1 % of the issue slots
 #pragma unroll 1
-    for (int64_t i = 0; i < iters; i += 4) {
+    for (int64_t i = 0; i < iters; i += kProbeUnroll) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int u = 0; u < kProbeUnroll; ++u)
 #pragma unroll
             for (int c = 0; c < kProbeChains; ++c) x[c] = fma(x[c], a, b);
     }
@@ -40,7 +42,7 @@ ge_fma_probe_kernel(T* __restrict__ sink, T a, T b, int64_t iters) {
 // Enqueues one launch; returns the flops it performs (an FMA counts 2).
 template <typename T>
 inline cudaError_t fma_probe_launch(T* sink, int64_t iters, int sm_count, double* flops, cudaStream_t s) {
-    iters = (iters + 3) / 4 * 4;
+    iters = (iters + kProbeUnroll - 1) / kProbeUnroll * kProbeUnroll;
     const int blocks = sm_count * kProbeBlocksPerSm;
     ge_fma_probe_kernel<T><<<blocks, kProbeThreads, 0, s>>>(sink, T(0.999), T(0.001), iters);
     *flops = 2.0 * kProbeChains * (double)iters * (double)blocks * kProbeThreads;

@@ -69,7 +69,61 @@ template <typename T>
 struct Strip2dCtx {
     T r, g2, g4, h1, h3, xlo, xhi;
     bool is_lo, is_hi;     // this lane holds column 0 in slot 0 / column nx-1 in slot C-1 (unshifted)
+    // cooperative strips (COOP > 1 warps share one strip; see strip_neighbour)
+    int warp;              // warp of the strip, 0 .. COOP-1
+    int gl;                // lane of the strip, warp*32 + lane
+    T* xch;                // shared memory: exchange lines of the strip
+    T* xslow;              // shared memory: [COOP*32 lanes][4 values] for the y-edge path
 };
+
+// ---- cooperative strips ----------------------------------------------------------------------------
+// COOP adjacent warps of a CTA own ONE strip of COOP*32*C columns and march through the same row pairs in
+// step.  A stage needs from the neighbouring LANE two right-hand sides (R stages: of the lane to the right,
+// L stages: to the left).  Inside a warp that is a pair of shuffles; with COOP > 1 every lane publishes its
+// two values in a shared-memory line of the strip and reads its neighbour's, so that the last (first) lane
+// of a warp gets them from the next (previous) WARP instead of recomputing TB stale columns: only the two
+// ends of the CTA's strip carry a redundant halo.  Ordering between two adjacent warps is a pair of named
+// barriers (bar.arrive by the producer, bar.sync by the consumer, 64 threads): barrier 1+w orders "warp w+1
+// published, warp w may read" (R stages), barrier COOP+w "warp w published, warp w+1 may read" (L stages).
+// A producer never waits; since R and L stages alternate, a warp can run at most one stage ahead of its
+// neighbour, which is also why one line per stage type (and iteration parity, for slack) is enough: the
+// producer of an R line rewrites it two stages later, after an L stage that needed the consumer's arrive,
+// which follows the consumer's read in program order.
+__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// elements of the exchange area of one strip: [2 stage types][2 iteration parities] lines of [COOP*32 lanes]
+// [2 values], then the line of the y-edge path [COOP*32 lanes][4 values]
+template <int COOP> struct StripXch {
+    static constexpr int lines = COOP > 1 ? 4 * COOP * 32 * 2 : 0;
+    static constexpr int elems = COOP > 1 ? lines + COOP * 32 * 4 : 0;
+};
+
+// RIGHT: the values (a, b) of lane gl+1, else of lane gl-1.  The lanes at the two ends of the strip get
+// their own values back (stale columns of the CTA's halo, as lane 31 / lane 0 of a lone warp do).
+template <typename T, int COOP, bool RIGHT>
+__device__ __forceinline__ void strip_neighbour(T a, T b, T& na, T& nb, const Strip2dCtx<T>& k, int par) {
+    constexpr unsigned FULL = 0xffffffffu;
+    if constexpr (COOP == 1) {
+        na = RIGHT ? __shfl_down_sync(FULL, a, 1) : __shfl_up_sync(FULL, a, 1);
+        nb = RIGHT ? __shfl_down_sync(FULL, b, 1) : __shfl_up_sync(FULL, b, 1);
+    } else {
+        T* line = k.xch + ((RIGHT ? 0 : 2) + par) * (COOP * 32 * 2);
+        if constexpr (sizeof(T) == 4) *reinterpret_cast<float2*>(line + 2 * k.gl) = make_float2(a, b);
+        else                          *reinterpret_cast<double2*>(line + 2 * k.gl) = make_double2(a, b);
+        if constexpr (RIGHT) {
+            if (k.warp > 0) bar_arrive(1 + k.warp - 1, 64);
+            if (k.warp < COOP - 1) bar_sync(1 + k.warp, 64); else __syncwarp();
+        } else {
+            if (k.warp < COOP - 1) bar_arrive(COOP + k.warp, 64);
+            if (k.warp > 0) bar_sync(COOP + k.warp - 1, 64); else __syncwarp();
+        }
+        int nl = RIGHT ? k.gl + 1 : k.gl - 1;
+        nl = nl < 0 ? 0 : (nl > COOP * 32 - 1 ? COOP * 32 - 1 : nl);
+        if constexpr (sizeof(T) == 4) { const float2 v = *reinterpret_cast<const float2*>(line + 2 * nl); na = v.x; nb = v.y; }
+        else                          { const double2 v = *reinterpret_cast<const double2*>(line + 2 * nl); na = v.x; nb = v.y; }
+    }
+}
 
 // the closed-form 4x4 solve, members a b / c d
 template <typename T>
@@ -115,11 +169,9 @@ __device__ __forceinline__ void strip_rhs_pair(const T (&X0)[C], const T (&X1)[C
 // previous pair, Rc / Rd: upper half from the current pair.  N0 / N1 are the new rows of the group row;
 // nx0[0..1]: new column 0 of those rows (lane is_lo only).
 template <typename T, int C, bool BC>
-__device__ __forceinline__ void strip_stage_R(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
-                                              T (&N0)[C], T (&N1)[C], T (&nx0)[2], const Strip2dCtx<T>& k) {
-    constexpr unsigned FULL = 0xffffffffu;
-    const T RbN = __shfl_down_sync(FULL, H[0], 1);
-    const T RdN = __shfl_down_sync(FULL, Rd[0], 1);
+__device__ __forceinline__ void strip_stage_R_given(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                                    T (&N0)[C], T (&N1)[C], T (&nx0)[2], const Strip2dCtx<T>& k,
+                                                    const T RbN, const T RdN) {
 #pragma unroll
     for (int m = 0; m < C / 2; ++m) {
         const T ra = H[2 * m + 1];
@@ -138,16 +190,20 @@ __device__ __forceinline__ void strip_stage_R(const T (&H)[C], const T (&Rc)[C /
     }
     if constexpr (BC) solve2(H[0], Rd[0], k.xlo, k.h1, k.h3, nx0[0], nx0[1]);   // group (x = -1, 0)
 }
+template <typename T, int C, bool BC, int COOP = 1>
+__device__ __forceinline__ void strip_stage_R(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                              T (&N0)[C], T (&N1)[C], T (&nx0)[2], const Strip2dCtx<T>& k, int par = 0) {
+    T RbN, RdN;
+    strip_neighbour<T, COOP, true>(H[0], Rd[0], RbN, RdN, k, par);
+    strip_stage_R_given<T, C, BC>(H, Rc, Rd, N0, N1, nx0, k, RbN, RdN);
+}
 
 // L: rows shifted right by one column -> unshifted rows.  pP / pQ: column 0 of the previous pair's /
 // the current pair's rows (lane is_lo only).
 template <typename T, int C, bool BC>
-__device__ __forceinline__ void strip_stage_L(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
-                                              const T (&pP)[2], const T (&pQ)[2],
-                                              T (&N0)[C], T (&N1)[C], const Strip2dCtx<T>& k) {
-    constexpr unsigned FULL = 0xffffffffu;
-    T ra = __shfl_up_sync(FULL, H[C - 1], 1);
-    T rc = __shfl_up_sync(FULL, Rc[C / 2 - 1], 1);
+__device__ __forceinline__ void strip_stage_L_given(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                                    const T (&pP)[2], const T (&pQ)[2],
+                                                    T (&N0)[C], T (&N1)[C], const Strip2dCtx<T>& k, T ra, T rc) {
     if constexpr (BC) {
         if (k.is_lo) {     // members a, c are column 0; their left neighbour is the boundary column
             const T a = pP[1], c = pQ[0];
@@ -160,6 +216,14 @@ __device__ __forceinline__ void strip_stage_L(const T (&H)[C], const T (&Rc)[C /
     for (int m = 0; m + 1 < C / 2; ++m)
         solve4(H[2 * m + 1], H[2 * m + 2], Rc[m], Rd[m + 1], k.g2, k.g4, N0[2 * m + 2], N0[2 * m + 3],
                N1[2 * m + 2], N1[2 * m + 3]);
+}
+template <typename T, int C, bool BC, int COOP = 1>
+__device__ __forceinline__ void strip_stage_L(const T (&H)[C], const T (&Rc)[C / 2], const T (&Rd)[C / 2],
+                                              const T (&pP)[2], const T (&pQ)[2],
+                                              T (&N0)[C], T (&N1)[C], const Strip2dCtx<T>& k, int par = 0) {
+    T ra, rc;
+    strip_neighbour<T, COOP, false>(H[C - 1], Rc[C / 2 - 1], ra, rc, k, par);
+    strip_stage_L_given<T, C, BC>(H, Rc, Rd, pP, pQ, N0, N1, k, ra, rc);
 }
 
 // Generic stage for the few stage-iterations whose group rows (j, j+1) are not both interior
@@ -210,9 +274,10 @@ __device__ __noinline__ void strip_stage_edge(const T* __restrict__ ext, T* __re
 // column-0 values (4: lane is_lo, shifted rows); builds the extended rows (two neighbour columns
 // per side, by shuffles), runs the generic stage and leaves N0, N1 (2*C values) and the new
 // column 0 of the two rows (2) at the start of io.  Called from a warp-uniform branch.
-template <typename T, int C, bool SHIFTED>
+template <typename T, int C, bool SHIFTED, int COOP = 1>
 __device__ __noinline__ void strip_stage_slow(T* __restrict__ io, const Coef2<T>* __restrict__ coef, int yg,
-                                              bool outside, bool is_lo, bool is_hi) {
+                                              bool outside, bool is_lo, bool is_hi, T* __restrict__ xch = nullptr,
+                                              int gl = 0) {
     constexpr unsigned FULL = 0xffffffffu;
     constexpr int E = C + 4;
     const T xlo = coef->xlo, xhi = coef->xhi;
@@ -222,8 +287,19 @@ __device__ __noinline__ void strip_stage_slow(T* __restrict__ io, const Coef2<T>
         const T* v = io + rr * C;
 #pragma unroll
         for (int s = 0; s < C; ++s) ext[rr * E + s + 2] = v[s];
-        T l2 = __shfl_up_sync(FULL, v[C - 2], 1), l1 = __shfl_up_sync(FULL, v[C - 1], 1);
-        T r0 = __shfl_down_sync(FULL, v[0], 1), r1 = __shfl_down_sync(FULL, v[1], 1);
+        T l2, l1, r0, r1;
+        if constexpr (COOP == 1) {
+            l2 = __shfl_up_sync(FULL, v[C - 2], 1); l1 = __shfl_up_sync(FULL, v[C - 1], 1);
+            r0 = __shfl_down_sync(FULL, v[0], 1); r1 = __shfl_down_sync(FULL, v[1], 1);
+        } else {
+            // the whole CTA (= the strip's COOP warps) is here: the edge test is the same for all of them
+            T* sl = xch;            // the strip's y-edge line
+            __syncthreads();
+            sl[4 * gl] = v[0]; sl[4 * gl + 1] = v[1]; sl[4 * gl + 2] = v[C - 2]; sl[4 * gl + 3] = v[C - 1];
+            __syncthreads();
+            const int nl = gl > 0 ? gl - 1 : 0, nr = gl < COOP * 32 - 1 ? gl + 1 : gl;
+            l2 = sl[4 * nl + 2]; l1 = sl[4 * nl + 3]; r0 = sl[4 * nr]; r1 = sl[4 * nr + 1];
+        }
         if (is_lo) {
             if (SHIFTED) { l1 = io[4 * C + rr]; l2 = xlo; } else { l1 = xlo; l2 = T(0); }
         }
@@ -243,7 +319,7 @@ __device__ __noinline__ void strip_stage_slow(T* __restrict__ io, const Coef2<T>
 // One EDGE stage-iteration (group rows j, j+1 not both interior): P = previous row pair of level l (with
 // its column 0: xP), Q = current one, both raw; writes the level-(l+1) pair into N (xN).  Odd stages are
 // L, even stages R.
-template <typename T, int C, bool BC>
+template <typename T, int C, bool BC, int COOP = 1>
 __device__ __forceinline__ void strip_stage_rows(const bool odd, const T (&P)[2][C], const T (&xP)[2],
                                                  const T (&Q)[2][C], const T (&xQ)[2], T (&N)[2][C], T (&xN)[2],
                                                  const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int j,
@@ -255,8 +331,8 @@ __device__ __forceinline__ void strip_stage_rows(const bool odd, const T (&P)[2]
     }
     io[4 * C] = xP[0]; io[4 * C + 1] = xP[1]; io[4 * C + 2] = xQ[0]; io[4 * C + 3] = xQ[1];
     const int yg = j == -1 ? 1 : (j + 1 == ny ? 2 : 0);
-    if (odd) strip_stage_slow<T, C, true>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
-    else     strip_stage_slow<T, C, false>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi);
+    if (odd) strip_stage_slow<T, C, true, COOP>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi, k.xslow, k.gl);
+    else     strip_stage_slow<T, C, false, COOP>(io, coef, yg, yg == 0, BC && k.is_lo, BC && k.is_hi, k.xslow, k.gl);
 #pragma unroll
     for (int s = 0; s < C; ++s) { N[0][s] = io[s]; N[1][s] = io[C + s]; }
     if (!odd) { xN[0] = io[2 * C]; xN[1] = io[2 * C + 1]; }
@@ -368,9 +444,10 @@ __device__ __forceinline__ void strip_request_pair(const T* __restrict__ uin, in
 // The TB stages of one iteration: `cur` (raw pair of level 0, rows y0, y0+1; cx its column 0) flows through
 // and comes out as the level-TB pair.  PURE: every group row (j = y0-1-l) is interior now and at the next
 // iteration, so there is neither an edge test nor a raw slot; otherwise each stage decides (warp-uniform).
-template <typename T, int C, int TB, bool BC, bool PURE>
+template <typename T, int C, int TB, bool BC, bool PURE, int COOP = 1>
 __device__ __forceinline__ void strip_stages(T (&cur)[2][C], T (&cx)[2], T (&px)[TB][2], T* __restrict__ sp, int lane,
-                                             const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int y0, int ny) {
+                                             const Strip2dCtx<T>& k, const Coef2<T>* __restrict__ coef, int y0, int ny,
+                                             int par = 0) {
     constexpr int kPair = 2 * 32 * C;
 #pragma unroll
     for (int l = 0; l < TB; ++l) {
@@ -384,12 +461,12 @@ __device__ __forceinline__ void strip_stages(T (&cur)[2][C], T (&cx)[2], T (&px)
         if (fast) {
             T H[C];
             strip_lds_half<T, C>(slot, lane, H);
-            if ((l & 1) != 0) strip_stage_L<T, C, BC>(H, Rc, Rd, px[l], cx, N[0], N[1], k);
-            else              strip_stage_R<T, C, BC>(H, Rc, Rd, N[0], N[1], nx0, k);
+            if ((l & 1) != 0) strip_stage_L<T, C, BC, COOP>(H, Rc, Rd, px[l], cx, N[0], N[1], k, par);
+            else              strip_stage_R<T, C, BC, COOP>(H, Rc, Rd, N[0], N[1], nx0, k, par);
         } else {
             T P[2][C];
             strip_lds<T, C>(slot, lane, P);
-            strip_stage_rows<T, C, BC>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, j, ny);
+            strip_stage_rows<T, C, BC, COOP>((l & 1) != 0, P, px[l], cur, cx, N, nx0, k, coef, j, ny);
         }
         if (next_fast) strip_sts_half<T, C>(slot, lane, Hn);
         else           strip_sts<T, C>(slot, lane, cur);
@@ -399,20 +476,22 @@ __device__ __forceinline__ void strip_stages(T (&cur)[2][C], T (&cx)[2], T (&px)
     }
 }
 
-template <typename T, int C, int TB, bool BC>
+template <typename T, int C, int TB, bool BC, int COOP = 1>
 __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny,
                                           const Coef2<T>* __restrict__ coef, T* __restrict__ sp, int a0,
                                           int out_lo, int out_hi, bool first, bool last, int ys, int ye,
-                                          int lane) {
+                                          int lane, int warp = 0, T* __restrict__ xch = nullptr) {
     constexpr int V = VecOf<T>::V;
     constexpr int kPair = 2 * 32 * C;             // elements of one row pair of the strip
     static_assert(TB % 2 == 0 && C % 2 == 0 && C % V == 0, "TB even; C holds whole groups and vectors");
     const Coef2<T> kk = *coef;
     Strip2dCtx<T> k;
     k.r = kk.r; k.g2 = kk.g2; k.g4 = kk.g4; k.h1 = kk.h1; k.h3 = kk.h3; k.xlo = kk.xlo; k.xhi = kk.xhi;
-    k.is_lo = BC && first && lane == 0; k.is_hi = BC && last && lane == 31;
-    const int e0 = a0 + lane * C;
+    k.warp = warp; k.gl = warp * 32 + lane; k.xch = xch; k.xslow = xch + StripXch<COOP>::lines;
+    k.is_lo = BC && first && k.gl == 0; k.is_hi = BC && last && k.gl == COOP * 32 - 1;
+    const int e0 = a0 + k.gl * C;
     const int Y0 = ys - TB;                       // first row pair that enters the pipeline
+    constexpr int kLag = TB;                      // rows between the pair that enters and the pair that leaves
     const int iters = (ye - ys + 1) / 2 + TB;
 
     {
@@ -437,7 +516,7 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
     // only used under the row tests)
     int rq = kStripRing - 1, rd = 0;
     int64_t in_off = (int64_t)(Y0 + 2 * (kStripRing - 1)) * nx + e0;
-    int64_t out_off = (int64_t)(Y0 - TB) * nx + e0;
+    int64_t out_off = (int64_t)(Y0 - kLag) * nx + e0;
     bool st_ok[C / V];
 #pragma unroll
     for (int c = 0; c < C / V; ++c) st_ok[c] = e0 + c * V >= out_lo && e0 + c * V < out_hi;
@@ -464,11 +543,11 @@ __device__ __forceinline__ void strip_run(const T* __restrict__ uin, T* __restri
         strip_lds<T, C>(ring + rd * kPair, lane, cur);
         rd = rd + 1 == kStripRing ? 0 : rd + 1;
         // every stage's group row interior now and at its next iteration: the pure pipeline, no edge tests
-        if (y0 - TB >= 0 && y0 + 1 < ny - 1) strip_stages<T, C, TB, BC, true>(cur, cx, px, sp, lane, k, coef, y0, ny);
-        else                                 strip_stages<T, C, TB, BC, false>(cur, cx, px, sp, lane, k, coef, y0, ny);
-        // cur holds level-TB rows (y0 - TB, y0 - TB + 1), unshifted (TB is even)
-        if (it >= TB) {
-            const int yo = y0 - TB;
+        if (y0 - TB >= 0 && y0 + 1 < ny - 1) strip_stages<T, C, TB, BC, true, COOP>(cur, cx, px, sp, lane, k, coef, y0, ny, it & 1);
+        else                                 strip_stages<T, C, TB, BC, false, COOP>(cur, cx, px, sp, lane, k, coef, y0, ny, it & 1);
+        // cur holds level-TB rows (y0 - kLag, y0 - kLag + 1), unshifted (TB is even)
+        if (it >= kLag) {
+            const int yo = y0 - kLag;
 #pragma unroll
             for (int rr = 0; rr < 2; ++rr) {
                 if (yo + rr < ye) {
@@ -535,6 +614,56 @@ inline cudaError_t strip2d_launch(const T* uin, T* uout, int64_t nx, int64_t ny,
         configured = true;
     }
     ge2d_strip_kernel<T, C, TB><<<grid, kStripWarps * 32, smem, s>>>(uin, uout, (int)nx, (int)ny, coef, g);
+    return cudaGetLastError();
+}
+
+// ---- cooperative form: the CTA's COOP warps own ONE strip of COOP*32*C columns (strip_neighbour) ----
+inline Strip2dGeom strip2d_coop_geom(int C, int V, int TB, int COOP, int64_t nx, int64_t ny, int hp) {
+    Strip2dGeom g;
+    const int64_t w = (int64_t)COOP * 32 * C;
+    g.halo = (TB + V - 1) / V * V;
+    g.valid = (int)(w - 2 * g.halo);
+    g.nreg = 1 + (int)((nx + g.halo - w) / g.valid);
+    g.nstrips = g.nreg + 1;
+    g.hp = hp;
+    g.segs = (int)((ny + 2 * (int64_t)hp - 1) / (2 * (int64_t)hp));
+    return g;
+}
+
+template <typename T, int C, int TB, int COOP>
+__global__ void __launch_bounds__(COOP * 32, 16 / COOP)     // 16 resident warps per SM, as for the plain kernel
+ge2d_strip_coop_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny,
+                       const Coef2<T>* __restrict__ coef, const Strip2dGeom g) {
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int strip = blockIdx.x;
+    const bool first = strip == 0, last = strip == g.nreg;
+    const int a0 = first ? 0 : (last ? nx - COOP * 32 * C : strip * g.valid - g.halo);
+    const int out_lo = strip * g.valid;
+    const int out_hi = last ? nx : out_lo + g.valid;
+    const int ys = 2 * g.hp * (int)blockIdx.y;
+    const int ye = ys + 2 * g.hp < ny ? ys + 2 * g.hp : ny;
+    extern __shared__ __align__(16) unsigned char strip_smem[];
+    T* xch = reinterpret_cast<T*>(strip_smem);
+    T* sp = xch + StripXch<COOP>::elems + (size_t)warp * (TB + kStripRing) * 2 * 32 * C;   // state + ring of this warp
+    if (first || last) strip_run<T, C, TB, true, COOP>(uin, uout, nx, ny, coef, sp, a0, out_lo, out_hi, first, last, ys, ye, lane, warp, xch);
+    else               strip_run<T, C, TB, false, COOP>(uin, uout, nx, ny, coef, sp, a0, out_lo, out_hi, false, false, ys, ye, lane, warp, xch);
+}
+
+// Host launcher of the cooperative form; requires nx >= COOP*32*C on top of strip2d_launch's conditions.
+template <typename T, int C, int TB, int COOP>
+inline cudaError_t strip2d_coop_launch(const T* uin, T* uout, int64_t nx, int64_t ny, const Coef2<T>* coef, int hp,
+                                       bool& configured, cudaStream_t s) {
+    const Strip2dGeom g = strip2d_coop_geom(C, VecOf<T>::V, TB, COOP, nx, ny, hp);
+    dim3 grid((unsigned)g.nstrips, (unsigned)g.segs);
+    constexpr size_t smem = ((size_t)COOP * (TB + kStripRing) * 2 * 32 * C + StripXch<COOP>::elems) * sizeof(T);
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(ge2d_strip_coop_kernel<T, C, TB, COOP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(ge2d_strip_coop_kernel<T, C, TB, COOP>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    ge2d_strip_coop_kernel<T, C, TB, COOP><<<grid, COOP * 32, smem, s>>>(uin, uout, (int)nx, (int)ny, coef, g);
     return cudaGetLastError();
 }
 

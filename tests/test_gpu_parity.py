@@ -322,6 +322,26 @@ def test_temporal_2d(oracle, dtype, nx, ny, tb, hp):
         np.testing.assert_array_equal(got, same, err_msg=str((nx, ny, level0, steps)))
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("coop", [2, 4, 8])
+@pytest.mark.parametrize("nx,ny,hp", [(1024, 64, 8), (1032, 77, 5), (2048, 40, 64), (2600, 130, 11), (4096 + 8, 33, 3)])
+def test_temporal_2d_cooperative_strips(oracle, dtype, coop, nx, ny, hp):
+    """The cooperative form of the strip kernel (GE_TUNE_STRIP_COOP: 4 or 8 warps of a CTA share one strip and
+    pass their edge right-hand sides through shared memory behind pairwise named barriers): one strip and
+    several, ragged last strip, segments shorter than the pipeline, x- and y-edge groups (the CTA-wide slow
+    path), both starting phases.  Must equal the per-level kernel bit for bit and match the oracle."""
+    cfg = inputs.random_grid(nx, ny, dtype, seed=nx + 3 * ny, r=1.7)
+    tb = 6
+    for level0, steps in ((1, tb), (0, 2 * tb + 3), (1, 5 * tb)):
+        got, info = run_gpu(cfg, steps, kernel="temporal", tb=tb, level0=level0, hp=hp, coop=coop)
+        assert info["kernel"] == "temporal" and info["launches"] == _launches_2d(nx, tb, level0, steps, dtype), info
+        assert info["tile_loaded"] == coop * (128 if dtype == "f32" else 64)
+        ref = run_oracle(oracle, cfg, steps, level0=level0)
+        assert rel_err(got, ref) <= (1e-13 if dtype == "f64" else 1e-5), (nx, ny, level0, steps, info)
+        same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+        np.testing.assert_array_equal(got, same, err_msg=str((nx, ny, coop, level0, steps)))
+
+
 def test_step_2d_entry_point(oracle):
     cfg = inputs.random_grid(96, 40, "f64", seed=8)
     a, _ = run_gpu(cfg, 4, via="step")
