@@ -473,6 +473,7 @@ def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clock
     if clocks:
         clocks.close()
     info0["group_k"] = k
+    info0["form3d"] = 0 if args_like.get("form3d") == 0 else 1
     out = {"value": job_value(units(cfg), steps, world, total_ms_max), "ms_per_step": total_ms_max / steps,
            "total_ms_this_rank": total_ms, "per_step": per_step, "launches": launches, "meetings": meetings,
            "finite": finite and not fault, "info": info0, "clocks": clocks.summary() if clocks else None,
@@ -795,11 +796,15 @@ def roofline(cfg, info, total_ms, launches, steps, alu=None):
     lv = cfg["steps"] * steps / max(launches, 1)            # levels per launch (average)
     upd = nelem * lv                                        # updates per launch
     names = {"per_step": "ge%dd_level_kernel", "temporal": "ge%dd_temporal_kernel"}
-    if info.get("group_k", 1) >= 2:
+    gk = info.get("group_k", 1)
+    if gk >= 2:
         names["per_step"] = "ge%dd_level_k_kernel"
+        names["temporal"] = "ge%dd_temporal_k_kernel"
+    if cfg["dim"] == 3:
+        names["per_step"] = "ge%dd_stream_kernel+shell" if info.get("form3d", 1) else "ge%dd_level_kernel"
     if kernel == "persistent":
         name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
-    elif kernel == "temporal" and info.get("temporal_c") in (18, 22, 26, 36, 44, 52):
+    elif kernel == "temporal" and gk == 1 and info.get("temporal_c") in (18, 22, 26, 36, 44, 52):
         name = "ge1d_stream_kernel"                      # the TMA-staged form of strategy B
     elif kernel == "temporal" and cfg["dim"] == 2 and cfg["nx"] % 4 == 0 and cfg["nx"] >= 128:
         name = "ge2d_strip_kernel"                       # the drift-free form of strategy B in 2-D
@@ -821,10 +826,13 @@ def roofline(cfg, info, total_ms, launches, steps, alu=None):
         derived = 2.0 * LANES[cfg["dtype"]] * SMS * clk / 1e12
         measured = (alu or {}).get(cfg["dtype"] + "_tflops")
         peak = measured or derived
-        ach = FLOPS[cfg["dim"]] * upd / (ms * 1e-3) / 1e12
+        # k >= 2: a Saul'yev node is (new - old) + (old' - old), fma: 3 instructions, 4 flops; pairs as for k = 1
+        flops = FLOPS[cfg["dim"]] if gk == 1 else (4.0 * (gk - 1) + 5.0) / gk
+        instr = INSTR[cfg["dim"]] if gk == 1 else (3.0 * (gk - 1) + 3.0) / gk
+        ach = flops * upd / (ms * 1e-3) / 1e12
         # issue terms: FP instructions of the factored form per second against the probe's FMA instructions per second
         out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                    "issue_frac": INSTR[cfg["dim"]] * upd / (ms * 1e-3) / (peak * 1e12 / 2.0),
+                    "issue_frac": instr * upd / (ms * 1e-3) / (peak * 1e12 / 2.0),
                     "peak_source": "measured (in-run FMA microbenchmark, ge_fma_probe)" if measured else "derived",
                     "peak_derived": derived,
                     "peak_derivation": "2 flop x %d %s lanes/SM x %d SMs x %.0f MHz" % (

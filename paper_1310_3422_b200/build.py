@@ -49,10 +49,12 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Every .cu of csrc/ is a translation unit of its own (the kernel families compile in parallel); objects are
     cached under lib/obj and recompiled when the source, any header or the flags changed."""
-    if not force and not needs_build():
-        return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     extra = os.environ.get("GE_NVCC_EXTRA", "").split()        # e.g. -DGE_STRIP_MINB_F32=4 for tuning sweeps
+    libtag = LIB + ".flags"
+    same_flags = os.path.exists(libtag) and open(libtag).read() == " ".join(NVCC_FLAGS + extra)
+    if not force and same_flags and not needs_build():
+        return LIB
     os.makedirs(OBJ, exist_ok=True)
     hdr_time = max(os.path.getmtime(f) for f in _headers())
     flags_tag = " ".join(NVCC_FLAGS + extra)
@@ -87,6 +89,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             os.remove(tmp)
         raise RuntimeError("nvcc failed linking libge.so (exit %d)" % proc.returncode)
     os.replace(tmp, LIB)
+    with open(libtag, "w") as f:
+        f.write(flags_tag)
     return LIB
 
 

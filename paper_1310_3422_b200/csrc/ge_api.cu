@@ -80,10 +80,13 @@ struct ge_plan {
     ge_desc host_desc;        // shape of this plan for the sub-plans (r, boundary values below)
     double host_r, host_lo, host_hi;
     int32_t strip_attr_tb;    // strip-kernel instantiation (tb*16 + coop) whose function attributes are set on this device (0: none)
+    cudaStream_t aux3d;       // 3-D: side stream of the shell kernel, with its fork / join events (lazy)
+    cudaEvent_t ev3d[2];
     int32_t form3d;           // 3-D per-level form: 1 streaming + shell kernels (default), 0 a thread per group
     int32_t strip_coop;       // warps that share one strip of the 2-D strip kernel (0: a warp per strip)
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
     bool rodk_attr;           // ... and of its shared-memory-resident form
+    bool temporalk_attr;      // ... and of its temporally blocked form
 };
 
 namespace {
@@ -210,6 +213,34 @@ int launch_level_k(ge_plan* p, const void* uin, void* uout, int phase, cudaStrea
     return GE_OK;
 }
 
+// strategy B for k >= 2: `levels` <= tb levels per launch on tiles of the rod (ge1d_temporal_k_kernel)
+#ifndef GE_TK_SMEM_KB
+#define GE_TK_SMEM_KB 64
+#endif
+constexpr size_t kTemporalKSmemBudget = GE_TK_SMEM_KB * 1024;
+bool temporal_k_ok(const ge_plan* p, int tb) {
+    return p->dim == 1 && p->group_k >= 2 && tb >= 1 &&
+           ge::temporal_k_geom(p->group_k, tb, p->nx, elem_size(p->dtype), kTemporalKSmemBudget).valid > 0;
+}
+template <typename T>
+int launch_temporal_k(ge_plan* p, const void* uin, void* uout, int levels, cudaStream_t s) {
+    const ge::TemporalKGeom g = ge::temporal_k_geom(p->group_k, p->tb, p->nx, sizeof(T), kTemporalKSmemBudget);
+    if (g.valid <= 0 || levels < 1 || levels > p->tb) return GE_EINVAL;
+    if (!p->temporalk_attr) {
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_temporal_k_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(kTemporalKSmemBudget + 1024)));
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_temporal_k_kernel<T>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        p->temporalk_attr = true;
+    }
+    dim3 grid((unsigned)g.tiles, (unsigned)(p->batch < 65535 ? p->batch : 65535));
+    ge::ge1d_temporal_k_kernel<T><<<grid, g.threads, g.smem, s>>>((const T*)uin, (T*)uout, p->nx, p->batch,
+                                                                  (const ge::Coef1<T>*)p->coef, g, (int)(p->level & 1), levels);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    p->level += levels;
+    return GE_OK;
+}
+
 // strategy C for k >= 2: the rod resident in shared memory, one launch for the whole run (res_path 3)
 constexpr size_t kRodKSmemMax = 200 * 1024;
 bool rod_k_fits(const ge_plan* p) {
@@ -245,7 +276,17 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
         // the streaming form (deep groups) + shell, unless the grid is too small to have deep groups worth a launch
         const int form = p->form3d && p->nx >= 8 && p->ny >= 8 && p->nz >= 8 ? 1 : 0;
         int n = 0;
-        const cudaError_t e = ge::level3d_dispatch(p->dtype, form, uin, uout, p->nx, p->ny, p->nz, p->coef, phase, p->sm_count, s, &n);
+        if (form == 1 && !p->aux3d) {        // side stream of the shell kernel (lazy; a failure just keeps everything on s)
+            if (cudaStreamCreateWithFlags(&p->aux3d, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&p->ev3d[0], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&p->ev3d[1], cudaEventDisableTiming) != cudaSuccess) {
+                cudaGetLastError();
+                if (p->aux3d) cudaStreamDestroy(p->aux3d);
+                p->aux3d = nullptr; p->ev3d[0] = p->ev3d[1] = nullptr;
+            }
+        }
+        const cudaError_t e = ge::level3d_dispatch(p->dtype, form, uin, uout, p->nx, p->ny, p->nz, p->coef, phase, p->sm_count, s, &n,
+                                                   p->aux3d, p->ev3d[0], p->ev3d[1]);
         if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
         p->launches += n;
         rc = GE_OK;
@@ -627,8 +668,11 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     int kernel = d->kernel;
     if (d->group_k >= 2) {                                  // k >= 2 (ge_level_k.cuh): strategy A, or C when the rod fits in shared memory
         const bool want_c = kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT;
+        const bool want_b = kernel != GE_KERNEL_PER_STEP;
+        const int tbk = d->tb > 0 ? d->tb : 8;
         kernel = GE_KERNEL_PER_STEP;
         if (want_c && rod_k_fits(p)) { kernel = GE_KERNEL_PERSISTENT; p->res_path = 3; }
+        else if (want_b && temporal_k_ok(p, tbk)) { kernel = GE_KERNEL_TEMPORAL; p->tb = tbk; }
     }
     if (d->dim == 3) kernel = GE_KERNEL_PER_STEP;          // 3-D: strategy A only (ge_level3d.cuh)
     if (d->group_k == 1 && (kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT)) {
@@ -640,7 +684,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->kernel = kernel;
     const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
     // measured on C4: the TMA-staged kernel is fp64-bound from tb ~ 12 on, best near 20
-    if (temporal_like && d->dim == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (is_stream_tc(p->dtype, p->tc) ? 20 : 16));
+    if (temporal_like && d->dim == 1 && d->group_k == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (is_stream_tc(p->dtype, p->tc) ? 20 : 16));
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
@@ -715,9 +759,16 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                                       : launch_rod_resident<float>(p, u, steps, s);
         return launch_grid_resident(p, u, steps, s);
     }
-    const bool temporal = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && temporal_ok(p, u);
+    const bool temporal = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && p->group_k == 1 && temporal_ok(p, u);
+    const bool temporal_k = p->kernel == GE_KERNEL_TEMPORAL && p->group_k >= 2;
     while (left > 0 && rc == GE_OK) {
-        if (temporal && p->dim == 2) {
+        if (temporal_k) {
+            // equal-sized blocks of at most tb levels (any starting phase)
+            const int64_t nl = (left + p->tb - 1) / p->tb;
+            const int lv = (int)((left + nl - 1) / nl);
+            rc = p->dtype == GE_F64 ? launch_temporal_k<double>(p, cur, oth, lv, s) : launch_temporal_k<float>(p, cur, oth, lv, s);
+            left -= lv;
+        } else if (temporal && p->dim == 2) {
             const bool strips = strip2d_ok(p);
             if (strips && left > p->tb && (p->level & 1) == 0) {
                 // the strip kernel starts at a phase-1 level: one per-level launch first
@@ -949,6 +1000,10 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
             const int V = p->dtype == GE_F64 ? 2 : 4;
             int valid = 0, loaded = 0;
             if (p->kernel != GE_KERNEL_TEMPORAL) { }
+            else if (p->dim == 1 && p->group_k >= 2) {
+                const ge::TemporalKGeom g = ge::temporal_k_geom(p->group_k, p->tb, p->nx, elem_size(p->dtype), kTemporalKSmemBudget);
+                valid = g.valid; loaded = g.window;
+            }
             else if (p->dim == 1) { valid = ge::temporal1d_geom(p->tc, V, p->tb, 1).valid; loaded = 32 * p->tc; }
             else if (strip2d_ok(p))   // the kernel that runs: strips of (coop*)32*C columns, halo stale columns per side
                 ge::strip2d_tile(p->dtype, p->tb, strip2d_coop_ok(p, p->strip_coop) ? p->strip_coop : 0, p->nx, p->ny, p->hp, &valid, &loaded);
@@ -956,7 +1011,7 @@ int ge_plan_info(const ge_plan* p, int32_t what, int64_t* value) {
             *value = what == GE_INFO_TILE_VALID ? valid : loaded;
             return GE_OK;
         }
-        case GE_INFO_TEMPORAL_C: *value = p->kernel == GE_KERNEL_TEMPORAL && p->dim == 1 ? p->tc : 0; return GE_OK;
+        case GE_INFO_TEMPORAL_C: *value = p->kernel == GE_KERNEL_TEMPORAL && p->dim == 1 && p->group_k == 1 ? p->tc : 0; return GE_OK;
         case GE_INFO_RESIDENT_PATH: *value = p->kernel == GE_KERNEL_PERSISTENT ? p->res_path : 0; return GE_OK;
         case GE_INFO_RESIDENT_C: *value = p->res_path ? p->res_c : 0; return GE_OK;
         case GE_INFO_RESIDENT_WARPS:
@@ -995,7 +1050,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             p->strip_coop = (int32_t)value;
             return GE_OK;
         case GE_TUNE_TEMPORAL_C: {
-            if (p->dim != 1) return GE_EINVAL;
+            if (p->dim != 1 || p->group_k != 1) return GE_EINVAL;
             const int c0 = p->dtype == GE_F64 ? 8 : 16;
             if (is_stream_tc(p->dtype, value)) { if (p->nx < 32 * value) return GE_EINVAL; p->stream_ctas = 0; }
             else if (value != c0 && value != 2 * c0 && value != 4 * c0) return GE_EINVAL;
@@ -1048,6 +1103,11 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
                 return GE_OK;
             }
             if (p->kernel != GE_KERNEL_TEMPORAL) return GE_EINVAL;
+            if (p->group_k >= 2) {
+                if (!temporal_k_ok(p, (int)(value > 4096 ? 4096 : value))) return GE_EINVAL;
+                p->tb = (int32_t)value;
+                return GE_OK;
+            }
             if (p->dim == 2) {
                 if (!temporal2d_tb_ok(p, value)) return GE_EINVAL;
                 p->tb = (int32_t)value;
@@ -1079,6 +1139,9 @@ int ge_plan_destroy(ge_plan* p) {
     cudaFree(p->hostpath);
     cudaFree(p->res_xbuf);
     cudaFree(p->res_flags);
+    if (p->aux3d) { cudaStreamSynchronize(p->aux3d); cudaStreamDestroy(p->aux3d); }
+    if (p->ev3d[0]) cudaEventDestroy(p->ev3d[0]);
+    if (p->ev3d[1]) cudaEventDestroy(p->ev3d[1]);
     if (p->slots) {
         for (int i = 0; i < kHostSlots; ++i) {
             for (int kd = 0; kd < 4; ++kd) if (p->slots[i].sub[kd]) ge_plan_destroy(p->slots[i].sub[kd]);

@@ -18,8 +18,10 @@ bool strip2d_coop_compiled(int dtype, int tb, int coop);
 void strip2d_tile(int dtype, int tb, int coop, int64_t nx, int64_t ny, int hp, int* valid, int* loaded);
 
 // 3-D per-level kernels (ge_stream3d.cu).  form 0: a thread per group (ge3d_level_kernel); form 1: the streaming
-// kernel for the deep groups + the shell kernel for the outermost layer (two launches).
+// kernel for the deep groups + the shell kernel for the outermost layer (two launches; the shell on the stream
+// `aux` between the events ev_in / ev_out when all three are given).
 cudaError_t level3d_dispatch(int dtype, int form, const void* uin, void* uout, int64_t nx, int64_t ny, int64_t nz,
-                             const void* coef, int phase, int sm_count, cudaStream_t s, int* launches);
+                             const void* coef, int phase, int sm_count, cudaStream_t s, int* launches,
+                             cudaStream_t aux = nullptr, cudaEvent_t ev_in = nullptr, cudaEvent_t ev_out = nullptr);
 
 }  // namespace ge

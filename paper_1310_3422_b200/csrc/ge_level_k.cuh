@@ -265,3 +265,179 @@ ge1d_rod_k_resident_kernel(T* u, int64_t nx, int64_t batch, const Coef1<T>* __re
 }
 
 }  // namespace ge
+
+// ------------------------------------------------------------------------------------------------
+// Strategy B for k >= 2: `levels` <= tb levels per HBM round trip on a long rod (the
+// paper's own k = 16, on rods that do not fit one CTA).  A CTA owns a tile of `valid` nodes,
+// loads them with `halo` more per side into shared memory (the skewed layout of the resident kernel) and
+// marches the window through the levels exactly as ge1d_rod_k_resident_kernel marches a rod -- one thread
+// per unit of 2k nodes, two CTA barriers per level -- treating whatever lies beyond a cut end as unknown.
+// What a cut end spoils: a node of an A sweep is only as good as its unit's left wall pair, a node of a B
+// sweep as good as everything from its left neighbour to the right wall pair (neighbours share
+// nothing but wall nodes), so the first good node moves inward by at most k+1 nodes per level (the A half
+// of the unit the front is in; the unit grid then shifts by k); a unit cut by the window's end is not marched
+// at all, which costs one more unit once: halo = tb (k+1) + 2k + 2 nodes.  A window end that IS the rod's end
+// holds the Dirichlet node and is exact.  Same expressions as the per-level kernel on the
+// same operands: bit-identical.
+namespace ge {
+
+struct TemporalKGeom {
+    int k, tb;
+    int halo;              // nodes per cut side
+    int valid;             // nodes a tile delivers
+    int window;            // valid + 2 halo
+    int threads;           // >= units of a window in either phase (+1 for a straddling unit), multiple of 32
+    int64_t tiles;
+    size_t smem;
+};
+inline TemporalKGeom temporal_k_geom(int k, int tb, int64_t nx, size_t elem, size_t smem_budget) {
+    TemporalKGeom g;
+    g.k = k; g.tb = tb;
+    g.halo = tb * (k + 1) + 2 * k + 2;
+    int64_t window = (int64_t)(smem_budget / elem) * 32 / 33 - 8;       // skew: one extra word per 32
+    if (window > 1020 * 2 * (int64_t)k) window = 1020 * 2 * (int64_t)k; // <= 1024 threads (units + 2, rounded to warps)
+    int64_t valid = window - 2 * g.halo;
+    if (valid > nx) valid = nx;
+    valid -= valid % 2;
+    if (valid < 2 * (int64_t)k || valid < g.halo) { g.valid = 0; g.window = 0; g.threads = 0; g.tiles = 0; g.smem = 0; return g; }
+    g.valid = (int)valid;
+    g.window = g.valid + 2 * g.halo;
+    const int units = g.window / (2 * k) + 2;
+    g.threads = (units + 31) / 32 * 32;
+    g.tiles = (nx + g.valid - 1) / g.valid;
+    const int64_t words = (int64_t)g.window + 4 + (g.window + 4) / 32 + 1;
+    g.smem = (size_t)words * elem;
+    if (g.threads > 1024) { g.valid = 0; g.tiles = 0; }
+    return g;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(1024)
+ge1d_temporal_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
+                       const Coef1<T>* __restrict__ coef, const TemporalKGeom g, int phase0, int levels) {
+    extern __shared__ __align__(16) unsigned char tk_smem[];
+    T* sm = reinterpret_cast<T*>(tk_smem);
+    const int k = g.k, two_k = 2 * g.k;
+    const int64_t N = nx;
+    const int t = threadIdx.x;
+    // nodes of this tile: valid [v0, v1), window [w0, w1) clipped to the rod with its Dirichlet nodes 0 and N+1
+    const int64_t v0 = 1 + (int64_t)blockIdx.x * g.valid;
+    const int64_t v1 = v0 + g.valid < N + 1 ? v0 + g.valid : N + 1;
+    const int64_t w0 = v0 - g.halo > 0 ? v0 - g.halo : 0;
+    const int64_t w1 = v1 + g.halo < N + 2 ? v1 + g.halo : N + 2;
+    const int len = (int)(w1 - w0);
+    auto at = [&](int j) -> T& { return sm[j + (j >> 5)]; };                         // window element j = node w0 + j
+    auto rd = [&](int j) -> T { return (j >= 0 && j < len) ? sm[j + (j >> 5)] : T(0); };
+    for (int64_t rod = blockIdx.y; rod < batch; rod += gridDim.y) {
+        const Coef1<T> c = coef[rod];
+        const T* __restrict__ in = uin + rod * nx;
+        T* __restrict__ out = uout + rod * nx;
+        // one cp.async per node: all of a thread's copies are in flight together (a plain load-store loop pays
+        // one HBM latency per trip: 30 trips ~ 30 us against ~1 us of levels)
+        for (int j = t; j < len; j += blockDim.x) {
+            const int64_t i = w0 + j;
+            if (i >= 1 && i <= N) {
+                const uint32_t d32 = (uint32_t)__cvta_generic_to_shared(&at(j));
+                if constexpr (sizeof(T) == 8)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d32), "l"(in + (i - 1)) : "memory");
+                else
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d32), "l"(in + (i - 1)) : "memory");
+            } else {
+                at(j) = i == 0 ? c.lo : c.hi;
+            }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncthreads();
+        // this thread's unit in either phase (window coordinates of its node with c = 0), hoisted out of the level
+        // loop; a unit is marched when it lies inside the window together with the two old values either side of
+        // it, or when it touches an end of the ROD (then the index-tested path below handles what is missing).
+        // A unit cut by an end of the WINDOW is left alone: its nodes are halo that is stale anyway.
+        int s_ph[2]; bool run_ph[2], fast_ph[2];
+#pragma unroll
+        for (int ph = 0; ph < 2; ++ph) {
+            const int64_t off = ph ? -(int64_t)k : 0;
+            const int64_t sg = off + ((w0 - off) / two_k + t) * two_k;     // w0 - off >= 0
+            const int64_t eg = sg + two_k - 1;
+            const int s = (int)(sg - w0);
+            s_ph[ph] = s;
+            const bool inside = s >= 2 && s + two_k + 1 < len;             // nodes s-2 .. e+2 in the window
+            fast_ph[ph] = inside && sg >= 2 && eg + 1 <= N;                // ... and all of them interior nodes
+            const bool rod_end = (sg < 2 && w0 == 0) || (eg + 1 > N && w1 == N + 2);
+            run_ph[ph] = sg <= N && s < len && (inside || rod_end);
+        }
+#pragma unroll 1
+        for (int lev = 0; lev < levels; ++lev) {
+            const int phase = (phase0 + lev) & 1;
+            const int s = phase ? s_ph[1] : s_ph[0], e = s + two_k - 1;     // window coordinates
+            const int64_t sg = w0 + s;                                     // node with c = 0 of this thread's unit
+            const bool mine = phase ? run_ph[1] : run_ph[0], fast = phase ? fast_ph[1] : fast_ph[0];
+            T om2 = T(0), om1 = T(0), op0 = T(0), op1 = T(0), o0 = T(0), o1 = T(0), oe1 = T(0), oe = T(0);
+            if (fast) {
+                om2 = at(s - 2); om1 = at(s - 1); o0 = at(s); o1 = at(s + 1);
+                oe1 = at(e - 1); oe = at(e); op0 = at(e + 1); op1 = at(e + 2);
+            } else if (mine) {
+                om2 = rd(s - 2); om1 = rd(s - 1); o0 = rd(s); o1 = rd(s + 1);
+                oe1 = rd(e - 1); oe = rd(e); op0 = rd(e + 1); op1 = rd(e + 2);
+            }
+            __syncthreads();                                           // everybody has its old wall values
+            if (fast) {
+                // no index tests; the address of a node written is the address it was read at one step earlier
+                T prev, next, dump;
+                pair_update(om2, om1, o0, o1, c.r, c.g, dump, prev);
+                pair_update(oe1, oe, op0, op1, c.r, c.g, next, dump);
+                at(s) = prev; at(e) = next;
+                T a_old = o1, b_old = oe1;
+                int wa = s + 1 + ((s + 1) >> 5), wb = e - 1 + ((e - 1) >> 5);
+#pragma unroll 4
+                for (int m = 1; m < k; ++m) {
+                    const int ra = s + m + 1 + ((s + m + 1) >> 5), rb = e - m - 1 + ((e - m - 1) >> 5);
+                    const T a_nxt = sm[ra];
+                    const T b_nxt = sm[rb];
+                    prev = fma(c.e, (prev - a_old) + (a_nxt - a_old), a_old);
+                    sm[wa] = prev;
+                    next = fma(c.e, (next - b_old) + (b_nxt - b_old), b_old);
+                    sm[wb] = next;
+                    a_old = a_nxt; b_old = b_nxt;
+                    wa = ra; wb = rb;
+                }
+            } else if (mine) {
+                const int64_t eg = sg + two_k - 1;
+                T prev = c.lo, next = c.hi;
+                if (sg >= 1) {
+                    T lo_, hi_;
+                    pair_update_bc(om2, om1, o0, o1, c, sg - 1 == 0, false, lo_, hi_);
+                    prev = hi_;
+                    if (s >= 0 && s < len) at(s) = prev;
+                }
+                if (eg >= 1 && eg <= N) {
+                    T lo_, hi_;
+                    pair_update_bc(oe1, oe, op0, op1, c, false, eg + 1 == N + 1, lo_, hi_);
+                    next = lo_;
+                    if (e >= 0 && e < len) at(e) = next;
+                }
+                T a_old = o1, b_old = oe1;
+#pragma unroll 1
+                for (int m = 1; m < k; ++m) {
+                    const int ja = s + m, jb = e - m;
+                    const int64_t ia = sg + m, ib = eg - m;
+                    const T a_nxt = rd(ja + 1);
+                    const T b_nxt = rd(jb - 1);
+                    if (ia >= 1 && ia <= N) {
+                        prev = fma(c.e, (prev - a_old) + (a_nxt - a_old), a_old);
+                        if (ja >= 0 && ja < len) at(ja) = prev;
+                    }
+                    if (ib >= 1 && ib <= N) {
+                        next = fma(c.e, (next - b_old) + (b_nxt - b_old), b_old);
+                        if (jb >= 0 && jb < len) at(jb) = next;
+                    }
+                    a_old = a_nxt; b_old = b_nxt;
+                }
+            }
+            __syncthreads();
+        }
+        for (int64_t i = v0 + t; i < v1; i += blockDim.x) out[i - 1] = at((int)(i - w0));
+        __syncthreads();                                               // the window is reused by the next rod
+    }
+}
+
+}  // namespace ge

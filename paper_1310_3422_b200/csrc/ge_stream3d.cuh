@@ -14,7 +14,8 @@
 //     which the warp above / below loads as its own: L1 / L2 hits), 4 vector stores;
 //   * the x neighbours (columns x-1, x+2) are the adjacent lanes' values: 8 shuffles; lanes 0 and 31 fetch
 //     theirs with one predicated scalar load each per row;
-//   * loads of the pair after next are in flight while a pair is computed (fp32; fp64 keeps one pair ahead);
+//   * the next pair is loaded while a pair is computed (a second pair ahead, a cp.async ring in shared memory
+//     and L2 prefetches were measured and bring nothing: DESIGN.md section 7);
 //   * no boundary logic at all: only "deep" groups (the group and its 24 out-of-group neighbours interior,
 //     ge_level3d.cuh) are stored; addresses of anything else are clamped into the grid and the results
 //     dropped.  The outermost layer of groups -- first and last group index of every axis -- is left to
@@ -26,19 +27,13 @@
 namespace ge {
 
 #ifndef GE_S3D_WY
-#define GE_S3D_WY 4
+#define GE_S3D_WY 8
 #endif
 #ifndef GE_S3D_MINB
-#define GE_S3D_MINB 1
+#define GE_S3D_MINB 2
 #endif
 #ifndef GE_S3D_UNROLL
 #define GE_S3D_UNROLL 1
-#endif
-#ifndef GE_S3D_AHEAD2_F32
-#define GE_S3D_AHEAD2_F32 1
-#endif
-#ifndef GE_S3D_AHEAD2_F64
-#define GE_S3D_AHEAD2_F64 0
 #endif
 constexpr int kS3Unroll = GE_S3D_UNROLL;
 constexpr int kS3Wy = GE_S3D_WY;          // warps of a CTA, stacked in y (their halo rows are each other's own rows)
@@ -81,49 +76,46 @@ __device__ __forceinline__ void s3_load_pair(const T* __restrict__ uin, int64_t 
     }
 }
 
-template <typename T, int PH, bool VEC, bool AHEAD2>
+// Group indices start at 1 in every axis: index 0 and the last one are the shell's.
+template <typename T, int PH, bool VEC>
 __global__ void __launch_bounds__(32 * kS3Wy, GE_S3D_MINB)
 ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
                    const Coef3<T>* __restrict__ coef, int kseg) {
     constexpr unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x;
-    const int x0 = 2 * ((int)blockIdx.x * 32 + lane) - PH;            // anchor element of the lane's group column
-    const int y0 = 2 * ((int)blockIdx.y * kS3Wy + (int)threadIdx.y) - PH;
-    if (!(y0 >= 1 && y0 + 2 < ny)) return;                           // the whole warp: its group row is shell
-    const bool deep_x = x0 >= 1 && x0 + 2 < nx;
-    const int ngz = (nz + PH) / 2 + 1;                               // group plane pairs: anchors -PH, 2-PH, ... <= nz-1
-    const int k0 = (int)blockIdx.z * kseg;
-    const int k1 = k0 + kseg < ngz ? k0 + kseg : ngz;
+    const int x0 = 2 * (1 + (int)blockIdx.x * 32 + lane) - PH;       // anchor element of the lane's group column
+    const int y0 = 2 * (1 + (int)blockIdx.y * kS3Wy + (int)threadIdx.y) - PH;
+    if (!(y0 + 2 < ny)) return;                                      // the whole warp: its group row is shell or beyond
+    const bool deep_x = x0 + 2 < nx;
+    const int klast = (nz - 1 + PH) / 2;                             // last group plane pair (shell)
+    const int k0 = 1 + (int)blockIdx.z * kseg;
+    const int k1 = k0 + kseg < klast ? k0 + kseg : klast;            // deep pairs: 1 .. klast-1
     if (k0 >= k1) return;
     const T r = coef->r, c1 = coef->c1, c2 = coef->c2, c3 = coef->c3;
     const int64_t sy = nx, sz = (int64_t)nx * ny;
-    // clamped addressing (only groups that are not deep ever see a clamped address; they are not stored)
+    // clamped addressing (only groups that are not deep ever see a clamped address; they are not stored):
     // columns x0, x0+1 clamped one by one, so that a lane next to a clamped one still gets its true neighbour
     // column through the shuffles (vector form: x0 and nx are even, the pair is clamped as a whole to nx-2)
-    const int xa = VEC ? (x0 > nx - 2 ? nx - 2 : x0) : (x0 < 0 ? 0 : (x0 > nx - 1 ? nx - 1 : x0));
-    const int xb = x0 + 1 < 0 ? 0 : (x0 + 1 > nx - 1 ? nx - 1 : x0 + 1);
+    const int xa = VEC ? (x0 > nx - 2 ? nx - 2 : x0) : (x0 > nx - 1 ? nx - 1 : x0);
+    const int xb = x0 + 1 > nx - 1 ? nx - 1 : x0 + 1;
     const int64_t ro[4] = {(int64_t)(y0 - 1) * sy, (int64_t)y0 * sy, (int64_t)(y0 + 1) * sy, (int64_t)(y0 + 2) * sy};
-    const int xl = x0 - 1 < 0 ? 0 : (x0 - 1 > nx - 1 ? nx - 1 : x0 - 1);       // lane 0's left / lane 31's right neighbour column
+    const int xl = x0 - 1;                                           // lane 0's left / lane 31's right neighbour column
     const int xr = x0 + 2 > nx - 1 ? nx - 1 : x0 + 2;
 
     T prevU[2][2];                    // rows y, y+1 of the plane below the current pair
-    S3Pair<T> cur, nxt, nn;
+    S3Pair<T> cur, nxt;
     {
-        int zz = 2 * k0 - PH - 1;
-        zz = zz < 0 ? 0 : zz;
-        const T* __restrict__ b = uin + zz * sz;
+        const T* __restrict__ b = uin + (int64_t)(2 * k0 - PH - 1) * sz;
         ld2<T, VEC>(b + ro[1], xa, xb, prevU[0]);
         ld2<T, VEC>(b + ro[2], xa, xb, prevU[1]);
     }
     s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * k0 - PH, nz, cur);
     s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * (k0 + 1) - PH, nz, nxt);
 
-    // unrolled by the period of the register rotation (cur <- nxt <- nn): no moves
-    constexpr int kUnroll = kS3Unroll ? (AHEAD2 ? 3 : 2) : 1;
-#pragma unroll(kUnroll)
+    // unrolled by the period of the register rotation (cur <- nxt): no moves
+#pragma unroll(kS3Unroll ? 2 : 1)
     for (int k = k0; k < k1; ++k) {
         const int z0 = 2 * k - PH;
-        if constexpr (AHEAD2) s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 4, nz, nn);
         // x neighbours of the four rows of the pair: columns x0-1 (left) and x0+2 (right)
         T lf[2][2], rt[2][2];
 #pragma unroll
@@ -134,11 +126,11 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
                 rt[pl][rr] = __shfl_down_sync(FULL, cur.own[pl][rr][0], 1);
             }
         if (lane == 0 || lane == 31) {
-            int za = z0 < 0 ? 0 : (z0 > nz - 1 ? nz - 1 : z0), zb = z0 + 1 > nz - 1 ? nz - 1 : (z0 + 1 < 0 ? 0 : z0 + 1);
+            const T* __restrict__ pa = uin + (int64_t)z0 * sz + (lane == 0 ? xl : xr);
 #pragma unroll
             for (int rr = 0; rr < 2; ++rr) {
-                const T va = __ldg(uin + za * sz + ro[1 + rr] + (lane == 0 ? xl : xr));
-                const T vb = __ldg(uin + zb * sz + ro[1 + rr] + (lane == 0 ? xl : xr));
+                const T va = __ldg(pa + ro[1 + rr]);
+                const T vb = __ldg(pa + sz + ro[1 + rr]);
                 if (lane == 0) { lf[0][rr] = va; lf[1][rr] = vb; } else { rt[0][rr] = va; rt[1][rr] = vb; }
             }
         }
@@ -162,7 +154,7 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
         W[3] *= c2; W[5] *= c2; W[6] *= c2;
         W[7] *= c3;
         wht8(W);
-        if (deep_x && z0 >= 1 && z0 + 2 < nz) {
+        if (deep_x) {
             T* __restrict__ ob = uout + (int64_t)z0 * sz + ro[1] + x0;
 #pragma unroll
             for (int dz = 0; dz < 2; ++dz)
@@ -175,8 +167,7 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 #pragma unroll
         for (int rr = 0; rr < 2; ++rr) { prevU[rr][0] = cur.own[1][rr][0]; prevU[rr][1] = cur.own[1][rr][1]; }
         cur = nxt;
-        if constexpr (AHEAD2) nxt = nn;
-        else s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 4, nz, nxt);
+        s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 4, nz, nxt);
     }
 }
 
@@ -203,32 +194,56 @@ ge3d_shell_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
 
 // ge3d_stream_kernel + ge3d_shell_kernel; requires nx even, nx, ny, nz >= 4 and 2-element alignment of both buffers
 // for the vector form (otherwise the scalar form is used in phase 0 too)
+template <typename T, int PH, bool VEC>
+inline cudaError_t stream3d_launch_one(const T* uin, T* uout, int nx, int ny, int nz, const Coef3<T>* coef, int kseg,
+                                       dim3 grid, cudaStream_t s) {
+    ge3d_stream_kernel<T, PH, VEC><<<grid, dim3(32, kS3Wy), 0, s>>>(uin, uout, nx, ny, nz, coef, kseg);
+    return cudaGetLastError();
+}
+
+// aux / ev_in / ev_out (optional): the shell kernel runs on the stream `aux`, beside the streaming kernel -- both
+// read the old level and write disjoint parts of the new one; ev_in orders it after the work already on `s`,
+// ev_out makes `s` wait for it.
 template <typename T>
 inline cudaError_t stream3d_launch(const T* uin, T* uout, int64_t nx, int64_t ny, int64_t nz, const Coef3<T>* coef,
-                                   int phase, int sm_count, cudaStream_t s) {
-    auto groups = [&](int64_t n) { return (n + phase) / 2 + 1; };      // anchors -phase, 2-phase, ... <= n-1
-    const int64_t gx = groups(nx), gy = groups(ny), gz = groups(nz);
-    // z segments: enough CTAs for ~8 resident CTAs on every SM, at least 8 pairs per segment
-    const int64_t ctas_xy = ((gx + 31) / 32) * ((gy + kS3Wy - 1) / kS3Wy);
-    int64_t segs = (8 * (int64_t)sm_count + ctas_xy - 1) / ctas_xy;
-    if (segs > gz / 8) segs = gz / 8;
-    if (segs < 1) segs = 1;
-    const int kseg = (int)((gz + segs - 1) / segs);
-    dim3 block(32, kS3Wy), grid((unsigned)((gx + 31) / 32), (unsigned)((gy + kS3Wy - 1) / kS3Wy), (unsigned)((gz + kseg - 1) / kseg));
-    const bool vec = phase == 0 && nx % 2 == 0 && (((uintptr_t)uin | (uintptr_t)uout) % (2 * sizeof(T))) == 0;
-    constexpr bool A2 = sizeof(T) == 4 ? GE_S3D_AHEAD2_F32 : GE_S3D_AHEAD2_F64;
-    if (phase == 0) {
-        if (vec) ge3d_stream_kernel<T, 0, true, A2><<<grid, block, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg);
-        else     ge3d_stream_kernel<T, 0, false, A2><<<grid, block, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg);
-    } else       ge3d_stream_kernel<T, 1, false, A2><<<grid, block, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    // shell: per face a 2-D grid over the two other axes' group indices
-    const int64_t gmax = gx > gy ? (gx > gz ? gx : gz) : (gy > gz ? gy : gz);
+                                   int phase, int sm_count, cudaStream_t s, cudaStream_t aux = nullptr,
+                                   cudaEvent_t ev_in = nullptr, cudaEvent_t ev_out = nullptr) {
+    auto last = [&](int64_t n) { return (n - 1 + phase) / 2; };         // group index of the last anchor <= n-1
+    const int64_t gx = last(nx) - 1, gy = last(ny) - 1, gz = last(nz) - 1;   // deep groups: indices 1 .. last-1
+    auto groups = [&](int64_t n) { return last(n) + 1; };
+    const int64_t ax = groups(nx), ay = groups(ny), az = groups(nz);
+    const int64_t gmax = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
+    cudaError_t e = cudaSuccess;
+    // shell first (it is small and latency-bound: it starts on part of the chip, the streaming kernel fills the rest)
+    const bool side = aux && ev_in && ev_out;
+    cudaStream_t ss = side ? aux : s;
+    if (side) {
+        e = cudaEventRecord(ev_in, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux, ev_in, 0);
+        if (e != cudaSuccess) return e;
+    }
     dim3 sblock(32, 4), sgrid((unsigned)((gmax + 31) / 32), (unsigned)((gmax + 3) / 4), 6);
-    if (phase == 0) ge3d_shell_kernel<T, 0><<<sgrid, sblock, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
-    else            ge3d_shell_kernel<T, 1><<<sgrid, sblock, 0, s>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
-    return cudaGetLastError();
+    if (phase == 0) ge3d_shell_kernel<T, 0><<<sgrid, sblock, 0, ss>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
+    else            ge3d_shell_kernel<T, 1><<<sgrid, sblock, 0, ss>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (side) { e = cudaEventRecord(ev_out, aux); if (e != cudaSuccess) return e; }
+    if (gx > 0 && gy > 0 && gz > 0) {
+        // z segments: enough CTAs for ~8 resident CTAs on every SM, at least 8 pairs per segment
+        const int64_t ctas_xy = ((gx + 31) / 32) * ((gy + kS3Wy - 1) / kS3Wy);
+        int64_t segs = (8 * (int64_t)sm_count + ctas_xy - 1) / ctas_xy;
+        if (segs > gz / 8) segs = gz / 8;
+        if (segs < 1) segs = 1;
+        const int kseg = (int)((gz + segs - 1) / segs);
+        dim3 grid((unsigned)((gx + 31) / 32), (unsigned)((gy + kS3Wy - 1) / kS3Wy), (unsigned)((gz + kseg - 1) / kseg));
+        const bool vec = phase == 0 && nx % 2 == 0 && (((uintptr_t)uin | (uintptr_t)uout) % (2 * sizeof(T))) == 0;
+        if (phase == 0) e = vec ? stream3d_launch_one<T, 0, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s)
+                                : stream3d_launch_one<T, 0, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s);
+        else            e = stream3d_launch_one<T, 1, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s);
+        if (e != cudaSuccess) return e;
+    }
+    if (side) e = cudaStreamWaitEvent(s, ev_out, 0);
+    return e;
 }
 
 }  // namespace ge

@@ -225,13 +225,42 @@ def test_general_k_per_level(oracle, dtype, k, n):
         np.testing.assert_array_equal(res, got)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("k,n,tb", [(2, 40000, 8), (3, 50001, 8), (16, 100000, 8), (16, 2 ** 18 - 2, 16), (64, 200000, 4),
+                                    (5, 30011, 13), (16, 70000, 1)])
+def test_general_k_temporal(oracle, dtype, k, n, tb):
+    """Strategy B for k >= 2 (ge1d_temporal_k_kernel): tb levels per launch on tiles whose window carries
+    tb (k+1) + 2k + 2 nodes of halo per cut side; several tiles, ragged last tile, rod ends inside a window, both
+    starting phases, >= 200 levels, a level count that is not a multiple of tb.  Against the oracle and bit
+    for bit against the per-level kernel."""
+    cfg = inputs.random_rods(2, n, dtype, seed=13 * k + n % 1000)
+    for level0, steps in ((0, 1), (1, 2 * tb + 3), (0, 203)):
+        got, info = run_gpu(cfg, steps, level0=level0, k=k, kernel="temporal", tb=tb)
+        assert info["kernel"] == "temporal" and info["tb"] == tb, info
+        assert info["launches"] == -(-steps // tb), info
+        ref = run_oracle(oracle, cfg, steps, level0=level0, k=k)
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (k, n, level0, steps, info)
+        same, i2 = run_gpu(cfg, steps, level0=level0, k=k, kernel="per_step")
+        assert i2["launches"] == steps
+        np.testing.assert_array_equal(got, same, err_msg=str((k, n, level0, steps)))
+
+
+def test_general_k_auto_takes_the_blocked_kernel_on_long_rods():
+    cfg = inputs.random_rods(1, 2 ** 20 - 2, "f64", seed=4)
+    _, info = run_gpu(cfg, 24, k=16)
+    assert info["kernel"] == "temporal" and info["tb"] == 8 and info["launches"] == 3, info
+    assert info["tile_loaded"] - info["tile_valid"] == 2 * (8 * 17 + 2 * 16 + 2)
+
+
 def test_general_k_resident_needs_the_rod_to_fit():
     cfg = inputs.random_rods(1, 100000, "f64", seed=1)           # 800 KB: more than a CTA's shared memory
     _, info = run_gpu(cfg, 3, k=16)
-    assert info["kernel"] == "per_step" and info["resident_path"] == 0 and info["launches"] == 3
+    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 1
+    _, info = run_gpu(cfg, 3, k=16, kernel="per_step")
+    assert info["kernel"] == "per_step" and info["launches"] == 3
     cfg = inputs.random_rods(1, 40000, "f32", seed=1)            # fits, but 10 001 units > 1024 threads at k = 2
     _, info = run_gpu(cfg, 3, k=2)
-    assert info["kernel"] == "per_step"
+    assert info["kernel"] == "temporal"
 
 
 def test_general_k_plan_rejects_the_two_point_resident_tuning(oracle):
