@@ -22,6 +22,7 @@
 #include "ge_level_k.cuh"
 #include "ge_level_src.cuh"
 #include "ge_probe.cuh"
+#include "ge_tail.cuh"
 
 namespace {
 
@@ -401,6 +402,30 @@ int launch_strip_2d(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
 // block lengths: 4, 8 everywhere; 6 only where the strip kernel runs
 bool temporal2d_tb_ok(const ge_plan* p, int64_t tb) { return tb == 4 || tb == 8 || (tb == 6 && strip2d_ok(p)); }
 
+// A single rod whose length is not a multiple of the vector: the blocked kernel marches the prefix of
+// nx - nx % V nodes, ge1d_tail_kernel recomputes the end piece (ge_tail.cuh).  Returns the prefix length, or 0.
+int64_t temporal_prefix(const ge_plan* p, const void* u) {
+    const int V = p->dtype == GE_F64 ? 2 : 4;
+    if (p->dim != 1 || p->group_k != 1 || p->batch != 1 || p->nx % V == 0) return 0;
+    if (((uintptr_t)u % 16) || ((uintptr_t)p->scratch % 16)) return 0;
+    const int64_t np = p->nx - p->nx % V;
+    // the window of the end piece (4 tb + 4 + tail, tb may grow by 2 in ge_run's schedule) must fit, and the
+    // prefix must still be a rod the blocked kernels take
+    if (4 * ((int64_t)p->tb + 2) + 8 + V > ge::kTailMaxLen || np < 8 * ((int64_t)p->tb + 2) + 64) return 0;
+    return np;
+}
+template <typename T>
+int launch_tail(ge_plan* p, const void* uin, void* uout, int64_t np, int phase0, int levels, cudaStream_t s) {
+    int64_t w0 = np - 4 * (int64_t)levels - 4;
+    w0 -= w0 & 1;
+    const int64_t o0 = np - 2 * (int64_t)levels - 2;
+    ge::ge1d_tail_kernel<T><<<1, ge::kTailThreads, 0, s>>>((const T*)uin, (T*)uout, p->nx, (const ge::Coef1<T>*)p->coef,
+                                                            w0, o0, phase0, levels);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    return GE_OK;
+}
+
 bool temporal_ok(const ge_plan* p, const void* u) {
     if (p->dim == 2 && (p->nx >= (1 << 30) || p->ny >= (1 << 30))) return false;
     const int V = p->dtype == GE_F64 ? 2 : 4;
@@ -759,7 +784,9 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                                       : launch_rod_resident<float>(p, u, steps, s);
         return launch_grid_resident(p, u, steps, s);
     }
-    const bool temporal = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && p->group_k == 1 && temporal_ok(p, u);
+    const bool blocked = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && p->group_k == 1;
+    const int64_t prefix = blocked ? temporal_prefix(p, u) : 0;
+    const bool temporal = blocked && (prefix > 0 || temporal_ok(p, u));
     const bool temporal_k = p->kernel == GE_KERNEL_TEMPORAL && p->group_k >= 2;
     while (left > 0 && rc == GE_OK) {
         if (temporal_k) {
@@ -802,6 +829,18 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                 const int64_t nl = (left + p->tb - 1) / p->tb;
                 tbn = (int)((left + nl - 1) / nl);
             }
+            if (prefix) {
+                // the prefix as a rod of its own (tile geometry and kernel choice follow its length), then the end piece
+                const int64_t nx0 = p->nx;
+                const int ph0 = (int)(p->level & 1);
+                p->nx = prefix;
+                rc = p->dtype == GE_F64 ? launch_temporal_1d<double>(p, cur, oth, tbn, s)
+                                        : launch_temporal_1d<float>(p, cur, oth, tbn, s);
+                p->nx = nx0;
+                if (rc == GE_OK)
+                    rc = p->dtype == GE_F64 ? launch_tail<double>(p, cur, oth, prefix, ph0, tbn, s)
+                                            : launch_tail<float>(p, cur, oth, prefix, ph0, tbn, s);
+            } else
             rc = p->dtype == GE_F64 ? launch_temporal_1d<double>(p, cur, oth, tbn, s)
                                     : launch_temporal_1d<float>(p, cur, oth, tbn, s);
             left -= tbn;

@@ -104,11 +104,33 @@ def test_temporal_1d_bitwise_equals_per_step():
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_temporal_1d_odd_n_falls_back_to_per_step(oracle, dtype):
+def test_temporal_1d_odd_n_batched_falls_back_to_per_step(oracle, dtype):
+    """Batched rods of odd length start at alternating alignments: no vector kernel, one launch per level."""
     cfg = inputs.random_rods(2, 1001, dtype, seed=77)
     got, info = run_gpu(cfg, 33, kernel="temporal")
     assert info["launches"] == 33
     assert rel_err_rows(got, run_oracle(oracle, cfg, 33)) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("n", [1001, 1002, 4099, 2 ** 20 + 1, 2 ** 20 + 2, 2 ** 20 + 3])
+@pytest.mark.parametrize("kernel", ["temporal", "auto", "persistent"])
+def test_awkward_lengths_stay_on_the_blocked_kernels(oracle, dtype, n, kernel):
+    """A single rod whose length is odd (a first-class case of the scheme: the last node is alone in phase 0,
+    paired in phase 1) or not a multiple of the 16-byte vector: the blocked kernel marches the prefix, the
+    end-piece kernel (ge_tail.cuh) recomputes the last 2 tb + 2 + nx % V nodes from the true boundary -- no
+    silent fall to one launch per level.  Both starting phases, odd level counts; against the oracle and bit
+    for bit against the per-level kernel."""
+    cfg = inputs.random_rods(1, n, dtype, seed=n % 977)
+    v = 2 if dtype == "f64" else 4
+    for level0, steps in ((0, 1), (1, 40), (0, 101)):
+        got, info = run_gpu(cfg, steps, kernel=kernel, level0=level0)
+        ref = run_oracle(oracle, cfg, steps, level0=level0)
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (n, level0, steps, info)
+        if n % v and steps >= 40 and info["resident_path"] == 0:
+            assert info["launches"] < steps, info            # blocked launches + one end piece each
+        same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+        np.testing.assert_array_equal(got, same, err_msg=str((dtype, n, kernel, level0, steps, info)))
 
 
 def test_run_is_deterministic():
@@ -179,7 +201,7 @@ def test_persistent_whole_chip(oracle, dtype, n, rc, hl, rtb, sync):
 
 
 def test_persistent_falls_back_when_the_shape_does_not_fit(oracle):
-    # odd N: no resident kernel, no vector kernel either -> per-level launches
+    # odd N, batched: no resident kernel, no vector kernel either -> per-level launches
     cfg = inputs.random_rods(2, 1001, "f64", seed=5)
     got, info = run_gpu(cfg, 20, kernel="persistent")
     assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 20
