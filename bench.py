@@ -696,10 +696,10 @@ def run_sweep(args):
             "bit-identical" if rows[-1][-1] else "MISMATCH"), flush=True)
     if args.md:
         with open(args.md, "w") as f:
-            f.write("| setting | kernel | tb | meetings per run | tiles | ms per run | GLUPS | bit-identical |\n|---|---|---|---|---|---|---|---|\n")
+            f.write("| setting | kernel | tb | meetings per run | tiles (warps) | tiles per SM | ms per run | GLUPS | bit-identical |\n|---|---|---|---|---|---|---|---|---|\n")
             for r in rows:
-                f.write("| %s | %s | %d | %d | %d | %.3f | %.1f | %s |\n" % (r[0], r[1], r[2], r[3], r[4], r[5], r[6],
-                                                                       "yes" if r[7] else "NO"))
+                f.write("| %s | %s | %d | %d | %d | %.2f | %.3f | %.1f | %s |\n" % (r[0], r[1], r[2], r[3], r[4], r[4] / float(SMS), r[5], r[6],
+                                                                             "yes" if r[7] else "NO"))
     if not all(r[-1] for r in rows):
         raise SystemExit(1)
 

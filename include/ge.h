@@ -116,6 +116,18 @@ int ge_step_3d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f, const double *bc4,
                    ge_stream_t stream);
 
+/* `steps` >= 0 levels of ge_step_1d_src in place (same restrictions: one rod, group_k == 1; one launch per level,
+ * ping-pong with the plan's scratch level, result in u, level += steps):
+ *   tau_f:          device pointer or NULL.  f_level_stride == 0: one stationary source of nx elements used at
+ *                   every level; f_level_stride >= nx: level n of the run reads tau_f + n * f_level_stride
+ *                   (`steps` rows);
+ *   bc_lo_t, bc_hi_t: HOST arrays of steps + 1 entries: the values of nodes 0 and N+1 at the run's levels
+ *                   0 .. steps (entry n is the old-level value of step n and the new-level value of step n-1).
+ * GE_EINVAL for batch > 1, dim != 1, a non-finite boundary value or 0 < f_level_stride < nx; GE_EUNSUPPORTED
+ * for group_k >= 2.  Nothing is enqueued on an argument error. */
+int ge_run_src(ge_plan *p, void *u, int64_t steps, const void *tau_f, int64_t f_level_stride,
+               const double *bc_lo_t, const double *bc_hi_t, ge_stream_t stream);
+
 /* `steps` >= 0 levels in place: on completion of the enqueued work u holds level (level0+steps) and
  * the plan's level counter has advanced by `steps`.  The plan's scratch level is used for
  * ping-ponging; the strategy is the plan's (AUTO/PER_STEP/TEMPORAL/PERSISTENT).  steps == 0 is a no-op. */

@@ -752,6 +752,28 @@ int ge_step_1d_src(ge_plan* p, const void* u_in, void* u_out, const void* tau_f,
     return GE_OK;
 }
 
+int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_level_stride, const double* bc_lo_t,
+               const double* bc_hi_t, ge_stream_t stream) {
+    if (!p || !u || steps < 0 || !bc_lo_t || !bc_hi_t || f_level_stride < 0 || p->dim != 1 || p->batch != 1) return GE_EINVAL;
+    if (p->group_k != 1) return GE_EUNSUPPORTED;
+    if (tau_f && f_level_stride != 0 && f_level_stride < p->nx) return GE_EINVAL;
+    for (int64_t n = 0; n <= steps; ++n)
+        if (!std::isfinite(bc_lo_t[n]) || !std::isfinite(bc_hi_t[n])) return GE_EINVAL;
+    NvtxRange nvtx("ge_run_src");
+    const size_t es = elem_size(p->dtype);
+    void* cur = u;
+    void* oth = p->scratch;
+    for (int64_t n = 0; n < steps; ++n) {
+        const double bc4[4] = {bc_lo_t[n], bc_lo_t[n + 1], bc_hi_t[n], bc_hi_t[n + 1]};
+        const void* f = tau_f ? (const char*)tau_f + (size_t)(n * f_level_stride) * es : nullptr;
+        const int rc = ge_step_1d_src(p, cur, oth, f, bc4, stream);
+        if (rc != GE_OK) return rc;
+        void* t = cur; cur = oth; oth = t;
+    }
+    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * es, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return GE_OK;
+}
+
 int ge_step_2d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
     return step_common(p, 2, u_in, u_out, (cudaStream_t)stream);
 }

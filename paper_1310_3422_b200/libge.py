@@ -33,7 +33,7 @@ _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
 _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 
 # every symbol include/ge.h declares
-EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
+EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_run_src", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
            "ge_fma_probe", "ge_strerror", "ge_version")
 
@@ -80,6 +80,7 @@ def load() -> ctypes.CDLL:
     lib.ge_step_3d.argtypes = [vp, vp, vp, vp]
     lib.ge_step_1d_src.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run.argtypes = [vp, vp, i64, vp]
+    lib.ge_run_src.argtypes = [vp, vp, i64, vp, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run_host.argtypes = [vp, vp, i64, vp]
     lib.ge_plan_get_level.argtypes = [vp, ctypes.POINTER(i64)]
     lib.ge_plan_set_level.argtypes = [vp, i64]
@@ -160,6 +161,15 @@ def ge_run(plan: int, u: int, steps: int, stream: int = 0):
     _check(load().ge_run(plan, u, steps, stream), "ge_run")
 
 
+def ge_run_src(plan: int, u: int, steps: int, tau_f: int, f_level_stride: int, bc_lo_t: Sequence[float],
+               bc_hi_t: Sequence[float], stream: int = 0):
+    """bc_lo_t / bc_hi_t: steps + 1 boundary values (levels 0 .. steps of the run); tau_f = device pointer or 0."""
+    lo, hi = _darr(bc_lo_t), _darr(bc_hi_t)
+    if len(lo) != steps + 1 or len(hi) != steps + 1:
+        raise GeError(GE_EINVAL, "ge_run_src (boundary arrays need steps + 1 values)")
+    _check(load().ge_run_src(plan, u, steps, tau_f or None, f_level_stride, lo, hi, stream), "ge_run_src")
+
+
 def ge_run_host(plan: int, u_host: int, steps: int, stream: int = 0):
     _check(load().ge_run_host(plan, u_host, steps, stream), "ge_run_host")
 
@@ -225,6 +235,9 @@ class Plan:
 
     def run(self, u: int, steps: int, stream: int = 0):
         ge_run(self.handle, u, steps, stream)
+
+    def run_src(self, u: int, steps: int, tau_f: int, f_level_stride: int, bc_lo_t, bc_hi_t, stream: int = 0):
+        ge_run_src(self.handle, u, steps, tau_f, f_level_stride, bc_lo_t, bc_hi_t, stream)
 
     def run_host(self, u_host: int, steps: int, stream: int = 0):
         ge_run_host(self.handle, u_host, steps, stream)

@@ -98,3 +98,48 @@ def test_step_src_argument_errors():
             plan.step_src(u.data_ptr(), u.data_ptr() + 8 * 64, 0, (0, float("nan"), 0, 0))
         with pytest.raises(libge.GeError):
             plan.step_src(u.data_ptr(), u.data_ptr(), 0, (0, 0, 0, 0))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("n,steps,level0,per_level", [(1000, 7, 0, True), (4099, 12, 1, True), (65536, 9, 0, False), (3, 5, 1, False)])
+def test_run_src_matches_the_oracle_marched_level_by_level(oracle, dtype, n, steps, level0, per_level):
+    """ge_run_src: the whole run behind one call -- a source array per level (or one stationary source) on the
+    device, boundary values as host arrays of steps + 1 entries, odd and even level counts (the result lands in u
+    either way), both starting phases."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    dt = _NP[dtype]
+    cfg = inputs.random_rods(1, n, dtype, seed=n + steps)
+    rng = np.random.default_rng(n)
+    srcs = rng.uniform(-0.1, 0.1, (steps if per_level else 1, n)).astype(dt)
+    walk = rng.uniform(-1, 1, (steps + 1, 2)).astype(dt).astype(np.float64)
+    dev = torch.device("cuda:0")
+    u = torch.from_numpy(cfg["u0"].reshape(-1).copy()).to(dev)
+    d_src = torch.from_numpy(srcs).to(dev)
+    s = torch.cuda.current_stream(dev).cuda_stream
+    with libge.Plan(cfg, stream=s) as plan:
+        plan.level = level0
+        plan.run_src(u.data_ptr(), steps, d_src.data_ptr(), n if per_level else 0, walk[:, 0], walk[:, 1], s)
+        torch.cuda.synchronize(dev)
+        assert plan.level == level0 + steps and plan.info()["launches"] == steps
+    ref = cfg["u0"].reshape(-1).astype(np.float64)
+    for i in range(steps):
+        ref = oracle.level_1d_src(ref, float(cfg["r"][0]), (level0 + i) % 2, (walk[i, 0], walk[i, 1]),
+                                  (walk[i + 1, 0], walk[i + 1, 1]), srcs[i if per_level else 0].astype(np.float64))
+    scale = max(np.abs(ref).max(), np.abs(walk).max())
+    assert np.abs(u.cpu().numpy().astype(np.float64) - ref).max() / scale <= TOL[dtype]
+
+
+def test_run_src_argument_errors():
+    import torch
+    from paper_1310_3422_b200 import libge
+    u = torch.zeros(256, dtype=torch.float64, device="cuda:0")
+    with libge.Plan(inputs.random_rods(1, 64, "f64")) as plan:
+        with pytest.raises(libge.GeError):
+            plan.run_src(u.data_ptr(), 2, 0, 0, (0, 0), (0, 0, 0))               # boundary arrays too short
+        with pytest.raises(libge.GeError):
+            plan.run_src(u.data_ptr(), 2, u.data_ptr() + 8 * 64, 10, (0, 0, 0), (0, 0, 0))   # 0 < stride < nx
+        with pytest.raises(libge.GeError):
+            plan.run_src(u.data_ptr(), 1, 0, 0, (0, float("inf")), (0, 0))
+        plan.run_src(u.data_ptr(), 0, 0, 0, (0.0,), (0.0,))
+        assert plan.level == 0
