@@ -432,6 +432,8 @@ def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clock
         plan.tune(libge.GE_TUNE_SEG_PAIRS, args_like["hp"])
     if args_like.get("coop") is not None and args_like.get("coop") >= 0:
         plan.tune(libge.GE_TUNE_STRIP_COOP, args_like["coop"])
+    if args_like.get("kform") is not None and args_like.get("kform") >= 0 and k >= 2:
+        plan.tune(libge.GE_TUNE_K_FORM, args_like["kform"])
     if args_like.get("form3d") is not None and args_like.get("form3d") >= 0:
         plan.tune(libge.GE_TUNE_FORM_3D, args_like["form3d"])
     if args_like.get("sync"):
@@ -509,7 +511,7 @@ def run_ours(args):
 
     peaks_alu = fma_peaks(dev, stream_obj)
     tune = dict(kernel=args.kernel, tb=args.tb, tc=args.tc, rc=args.rc, hl=args.hl, sync=args.sync, rtb=args.rtb,
-                hp=args.hp, coop=args.coop, form3d=args.form3d)
+                hp=args.hp, coop=args.coop, form3d=args.form3d, kform=args.kform)
 
     cfg = make_cfg(args.config)
     if args.levels:
@@ -857,6 +859,7 @@ def main():
     ap.add_argument("--sync", default="", choices=["", "flags", "grid", "lines", "stagger"], help="whole-chip persistent kernel: meeting kind")
     ap.add_argument("--hp", type=int, default=0, help="2-D strip kernel: output row pairs per segment")
     ap.add_argument("--coop", type=int, default=-1, help="2-D strip kernel: warps sharing one strip (0, 4, 8; -1 = plan default)")
+    ap.add_argument("--kform", type=int, default=-1, help="k >= 2 blocked kernel: 1 register-resident units, 0 shared-memory windows (-1 = plan default)")
     ap.add_argument("--form3d", type=int, default=-1, help="3-D: 1 streaming + shell kernels, 0 a thread per group (-1 = plan default)")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
     ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")

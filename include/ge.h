@@ -184,6 +184,9 @@ enum {
                                   nx >= value * 32 * columns per lane)                                              */
     GE_TUNE_FORM_3D = 7,       /* 3-D per-level kernels: 1 = streaming kernel for the deep groups + shell kernel for the
                                   outermost layer of groups (default, two launches per level), 0 = a thread per group    */
+    GE_TUNE_K_FORM = 8,        /* group_k >= 2, TEMPORAL: 1 = units of 2k nodes held in registers for tb levels + the two ends of the
+                                  rod recomputed by the shared-memory kernel (default where compiled: k = 2, 4, 8, 16, fp32 also 32),
+                                  0 = windows in shared memory throughout                                                  */
     GE_TUNE_SYNC_MODE = 5      /* path 2, how the tiles meet: 0 = neighbour flags (data, release fence, flag per
                                   tile, acquire), 1 = grid-wide barrier (cooperative groups), 2 = neighbour
                                   flag-in-data lines (no fence, no separate flag), 3 = the same lines published

@@ -83,6 +83,7 @@ struct ge_plan {
     int32_t strip_attr_tb;    // strip-kernel instantiation (tb*16 + coop) whose function attributes are set on this device (0: none)
     cudaStream_t aux3d;       // 3-D: side stream of the shell kernel, with its fork / join events (lazy)
     cudaEvent_t ev3d[2];
+    int32_t kform;            // k >= 2 blocked kernel: 1 register-resident units + end windows (default), 0 shared-memory windows
     int32_t form3d;           // 3-D per-level form: 1 streaming + shell kernels (default), 0 a thread per group
     int32_t strip_coop;       // warps that share one strip of the 2-D strip kernel (0: a warp per strip)
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
@@ -223,8 +224,40 @@ bool temporal_k_ok(const ge_plan* p, int tb) {
     return p->dim == 1 && p->group_k >= 2 && tb >= 1 &&
            ge::temporal_k_geom(p->group_k, tb, p->nx, elem_size(p->dtype), kTemporalKSmemBudget).valid > 0;
 }
+// the register-resident form (ge_unit_k.cuh) + the shared-memory kernel on the two ends of the rod
+int64_t unit_k_end_len(const ge_plan* p) { return (int64_t)p->tb * (p->group_k + 1) + 4 * p->group_k + 8; }
+bool unit_k_ok(const ge_plan* p, const void* u) {
+    const int V = p->dtype == GE_F64 ? 2 : 4;
+    if (p->dim != 1 || !ge::unit_k_compiled(p->dtype, p->group_k) || !p->kform) return false;
+    if (((uintptr_t)u % 16) || ((uintptr_t)p->scratch % 16) || (p->batch > 1 && p->nx % V)) return false;
+    if (p->batch > 65535 || p->nx < 4 * unit_k_end_len(p)) return false;
+    return ge::unit_k_valid_lanes(p->group_k, p->tb) >= 64 &&
+           ge::temporal_k_ends_geom(p->group_k, p->tb, unit_k_end_len(p), elem_size(p->dtype)).valid > 0;
+}
+template <typename T>
+int launch_unit_k(ge_plan* p, const void* uin, void* uout, int levels, cudaStream_t s) {
+    const int phase = (int)(p->level & 1);
+    cudaError_t e = ge::unit_k_dispatch(p->dtype, p->group_k, uin, uout, p->nx, p->batch, p->coef, p->tb, phase, levels, s);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    const ge::TemporalKGeom g = ge::temporal_k_ends_geom(p->group_k, p->tb, unit_k_end_len(p), sizeof(T));
+    if (!p->temporalk_attr) {
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_temporal_k_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(kTemporalKSmemBudget + 1024)));
+        GE_CUDA(cudaFuncSetAttribute(ge::ge1d_temporal_k_kernel<T>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        p->temporalk_attr = true;
+    }
+    dim3 grid(2, (unsigned)(p->batch < 65535 ? p->batch : 65535));
+    ge::ge1d_temporal_k_kernel<T><<<grid, g.threads, g.smem, s>>>((const T*)uin, (T*)uout, p->nx, p->batch,
+                                                                  (const ge::Coef1<T>*)p->coef, g, phase, levels);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 2;
+    p->level += levels;
+    return GE_OK;
+}
+
 template <typename T>
 int launch_temporal_k(ge_plan* p, const void* uin, void* uout, int levels, cudaStream_t s) {
+    if (unit_k_ok(p, uin) && unit_k_ok(p, uout)) return launch_unit_k<T>(p, uin, uout, levels, s);
     const ge::TemporalKGeom g = ge::temporal_k_geom(p->group_k, p->tb, p->nx, sizeof(T), kTemporalKSmemBudget);
     if (g.valid <= 0 || levels < 1 || levels > p->tb) return GE_EINVAL;
     if (!p->temporalk_attr) {
@@ -688,13 +721,14 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->tc = default_tc(p->dtype, p->nx);
     p->hp = p->dtype == GE_F64 ? 56 : 67;   // measured on C5 (the rate depends on the segment count, and sharply)
     p->form3d = 1;
+    p->kform = 1;
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
     if (d->group_k >= 2) {                                  // k >= 2 (ge_level_k.cuh): strategy A, or C when the rod fits in shared memory
         const bool want_c = kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT;
         const bool want_b = kernel != GE_KERNEL_PER_STEP;
-        const int tbk = d->tb > 0 ? d->tb : 8;
+        const int tbk = d->tb > 0 ? d->tb : 16;    // measured on the C4-shaped rod
         kernel = GE_KERNEL_PER_STEP;
         if (want_c && rod_k_fits(p)) { kernel = GE_KERNEL_PERSISTENT; p->res_path = 3; }
         else if (want_b && temporal_k_ok(p, tbk)) { kernel = GE_KERNEL_TEMPORAL; p->tb = tbk; }
@@ -1101,6 +1135,10 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_SEG_PAIRS:
             if (value < 1 || value > (1 << 20) || p->dim != 2) return GE_EINVAL;
             p->hp = (int32_t)value;
+            return GE_OK;
+        case GE_TUNE_K_FORM:
+            if (p->group_k < 2 || (value != 0 && value != 1)) return GE_EINVAL;
+            p->kform = (int32_t)value;
             return GE_OK;
         case GE_TUNE_FORM_3D:
             if (p->dim != 3 || (value != 0 && value != 1)) return GE_EINVAL;

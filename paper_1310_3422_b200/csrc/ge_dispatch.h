@@ -17,6 +17,13 @@ bool strip2d_coop_compiled(int dtype, int tb, int coop);
 // valid output columns per strip and columns a strip loads, for ge_plan_info
 void strip2d_tile(int dtype, int tb, int coop, int64_t nx, int64_t ny, int hp, int* valid, int* loaded);
 
+// Register-resident blocked kernel for sub-domain length k >= 2 (ge_unit_k.cu): `levels` <= tb levels from a level of
+// phase `phase`; the two ends of the rod are NOT valid afterwards (the caller recomputes them).
+bool unit_k_compiled(int dtype, int k);
+int unit_k_valid_lanes(int k, int tb);            // units a tile of 256 lanes delivers (<= 0: tb too large)
+cudaError_t unit_k_dispatch(int dtype, int k, const void* uin, void* uout, int64_t nx, int64_t batch, const void* coef,
+                            int tb, int phase, int levels, cudaStream_t s);
+
 // 3-D per-level kernels (ge_stream3d.cu).  form 0: a thread per group (ge3d_level_kernel); form 1: the streaming
 // kernel for the deep groups + the shell kernel for the outermost layer (two launches; the shell on the stream
 // `aux` between the events ev_in / ev_out when all three are given).

@@ -289,10 +289,11 @@ struct TemporalKGeom {
     int threads;           // >= units of a window in either phase (+1 for a straddling unit), multiple of 32
     int64_t tiles;
     size_t smem;
+    int64_t end_len;       // > 0: two CTAs per rod that recompute its first / last end_len nodes only (ge_unit_k.cuh)
 };
 inline TemporalKGeom temporal_k_geom(int k, int tb, int64_t nx, size_t elem, size_t smem_budget) {
     TemporalKGeom g;
-    g.k = k; g.tb = tb;
+    g.k = k; g.tb = tb; g.end_len = 0;
     g.halo = tb * (k + 1) + 2 * k + 2;
     int64_t window = (int64_t)(smem_budget / elem) * 32 / 33 - 8;       // skew: one extra word per 32
     if (window > 1020 * 2 * (int64_t)k) window = 1020 * 2 * (int64_t)k; // <= 1024 threads (units + 2, rounded to warps)
@@ -310,6 +311,19 @@ inline TemporalKGeom temporal_k_geom(int k, int tb, int64_t nx, size_t elem, siz
     if (g.threads > 1024) { g.valid = 0; g.tiles = 0; }
     return g;
 }
+// the same kernel on the two ends of the rod only: windows of end_len + halo nodes
+inline TemporalKGeom temporal_k_ends_geom(int k, int tb, int64_t end_len, size_t elem) {
+    TemporalKGeom g;
+    g.k = k; g.tb = tb; g.end_len = end_len;
+    g.halo = tb * (k + 1) + 2 * k + 2;
+    g.valid = (int)end_len;
+    g.window = g.valid + g.halo;                       // one side of an end window is the rod's end
+    g.threads = (g.window / (2 * k) + 2 + 31) / 32 * 32;
+    g.tiles = 2;
+    g.smem = (size_t)((int64_t)g.window + 4 + (g.window + 4) / 32 + 1) * elem;
+    if (g.threads > 1024) { g.valid = 0; g.tiles = 0; }
+    return g;
+}
 
 template <typename T>
 __global__ void __launch_bounds__(1024)
@@ -321,8 +335,10 @@ ge1d_temporal_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t 
     const int64_t N = nx;
     const int t = threadIdx.x;
     // nodes of this tile: valid [v0, v1), window [w0, w1) clipped to the rod with its Dirichlet nodes 0 and N+1
-    const int64_t v0 = 1 + (int64_t)blockIdx.x * g.valid;
-    const int64_t v1 = v0 + g.valid < N + 1 ? v0 + g.valid : N + 1;
+    const int64_t v0 = g.end_len > 0 ? (blockIdx.x == 0 ? 1 : (N + 1 - g.end_len > 1 ? N + 1 - g.end_len : 1))
+                                     : 1 + (int64_t)blockIdx.x * g.valid;
+    const int64_t v1 = g.end_len > 0 ? (blockIdx.x == 0 ? (1 + g.end_len < N + 1 ? 1 + g.end_len : N + 1) : N + 1)
+                                     : (v0 + g.valid < N + 1 ? v0 + g.valid : N + 1);
     const int64_t w0 = v0 - g.halo > 0 ? v0 - g.halo : 0;
     const int64_t w1 = v1 + g.halo < N + 2 ? v1 + g.halo : N + 2;
     const int len = (int)(w1 - w0);

@@ -5,7 +5,7 @@ _TORCH_DT = {"f32": "float32", "f64": "float64"}
 
 
 def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc=0, hl=0, sync=None, rtb=0,
-            chunks=None, k=1, coop=None, form3d=None):
+            chunks=None, k=1, coop=None, form3d=None, kform=None):
     """Run `steps` levels on cuda:0 and return the final state as a numpy array."""
     import torch
     from paper_1310_3422_b200 import libge
@@ -22,6 +22,8 @@ def run_gpu(cfg, steps, kernel="auto", tb=0, level0=0, via="run", tc=0, hp=0, rc
             plan.tune(libge.GE_TUNE_STRIP_COOP, coop)
         if form3d is not None:
             plan.tune(libge.GE_TUNE_FORM_3D, form3d)
+        if kform is not None:
+            plan.tune(libge.GE_TUNE_K_FORM, kform)
         if rc:
             plan.tune(libge.GE_TUNE_RESIDENT_C, rc)
         if hl:

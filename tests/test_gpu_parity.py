@@ -257,7 +257,7 @@ def test_general_k_temporal(oracle, dtype, k, n, tb):
     for bit against the per-level kernel."""
     cfg = inputs.random_rods(2, n, dtype, seed=13 * k + n % 1000)
     for level0, steps in ((0, 1), (1, 2 * tb + 3), (0, 203)):
-        got, info = run_gpu(cfg, steps, level0=level0, k=k, kernel="temporal", tb=tb)
+        got, info = run_gpu(cfg, steps, level0=level0, k=k, kernel="temporal", tb=tb, kform=0)
         assert info["kernel"] == "temporal" and info["tb"] == tb, info
         assert info["launches"] == -(-steps // tb), info
         ref = run_oracle(oracle, cfg, steps, level0=level0, k=k)
@@ -267,17 +267,42 @@ def test_general_k_temporal(oracle, dtype, k, n, tb):
         np.testing.assert_array_equal(got, same, err_msg=str((k, n, level0, steps)))
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("k,n,tb,batch", [(2, 40000, 8, 1), (4, 100000, 16, 1), (8, 70001, 8, 1), (16, 2 ** 18 - 2, 16, 1),
+                                          (16, 100003, 5, 1), (16, 40000, 8, 3), (32, 200000, 8, 1), (16, 2 ** 20, 16, 1)])
+def test_general_k_register_units(oracle, dtype, k, n, tb, batch):
+    """The register-resident form of strategy B for k >= 2 (ge1d_unit_k_kernel: a thread holds 2k nodes for tb
+    levels, one value crosses a lane boundary per level) + the shared-memory kernel on the two ends of the rod:
+    several tiles, ragged and odd lengths, batched rods, both starting phases, odd level counts.  Against the
+    oracle and bit for bit against the per-level kernel and the shared-memory form."""
+    if k == 32 and dtype == "f64":
+        pytest.skip("k = 32 is compiled for fp32 only")
+    cfg = inputs.random_rods(batch, n, dtype, seed=7 * k + n % 1000)
+    for level0, steps in ((0, 1), (1, 2 * tb + 3), (0, 203)):
+        got, info = run_gpu(cfg, steps, level0=level0, k=k, kernel="temporal", tb=tb, kform=1)
+        assert info["kernel"] == "temporal" and info["launches"] == 2 * -(-steps // tb), info   # unit kernel + end windows
+        ref = run_oracle(oracle, cfg, steps, level0=level0, k=k)
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (k, n, level0, steps, info)
+        same, _ = run_gpu(cfg, steps, level0=level0, k=k, kernel="per_step")
+        np.testing.assert_array_equal(got, same, err_msg=str((k, n, level0, steps)))
+        smem, i3 = run_gpu(cfg, steps, level0=level0, k=k, kernel="temporal", tb=tb, kform=0)
+        assert i3["launches"] == -(-steps // tb)
+        np.testing.assert_array_equal(got, smem)
+
+
 def test_general_k_auto_takes_the_blocked_kernel_on_long_rods():
     cfg = inputs.random_rods(1, 2 ** 20 - 2, "f64", seed=4)
-    _, info = run_gpu(cfg, 24, k=16)
-    assert info["kernel"] == "temporal" and info["tb"] == 8 and info["launches"] == 3, info
-    assert info["tile_loaded"] - info["tile_valid"] == 2 * (8 * 17 + 2 * 16 + 2)
+    _, info = run_gpu(cfg, 48, k=16, kform=0)
+    assert info["kernel"] == "temporal" and info["tb"] == 16 and info["launches"] == 3, info
+    assert info["tile_loaded"] - info["tile_valid"] == 2 * (16 * 17 + 2 * 16 + 2)
+    _, info = run_gpu(cfg, 48, k=16)
+    assert info["kernel"] == "temporal" and info["launches"] == 6, info        # register units + end windows
 
 
 def test_general_k_resident_needs_the_rod_to_fit():
     cfg = inputs.random_rods(1, 100000, "f64", seed=1)           # 800 KB: more than a CTA's shared memory
     _, info = run_gpu(cfg, 3, k=16)
-    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 1
+    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 2
     _, info = run_gpu(cfg, 3, k=16, kernel="per_step")
     assert info["kernel"] == "per_step" and info["launches"] == 3
     cfg = inputs.random_rods(1, 40000, "f32", seed=1)            # fits, but 10 001 units > 1024 threads at k = 2
