@@ -476,6 +476,7 @@ def device_timing(cfg, args_like, dev, stream_obj, steps, warmup, world=1, clock
         clocks.close()
     info0["group_k"] = k
     info0["form3d"] = 0 if args_like.get("form3d") == 0 else 1
+    info0["kform"] = 0 if args_like.get("kform") == 0 else 1
     out = {"value": job_value(units(cfg), steps, world, total_ms_max), "ms_per_step": total_ms_max / steps,
            "total_ms_this_rank": total_ms, "per_step": per_step, "launches": launches, "meetings": meetings,
            "finite": finite and not fault, "info": info0, "clocks": clocks.summary() if clocks else None,
@@ -801,11 +802,11 @@ def roofline(cfg, info, total_ms, launches, steps, alu=None):
     gk = info.get("group_k", 1)
     if gk >= 2:
         names["per_step"] = "ge%dd_level_k_kernel"
-        names["temporal"] = "ge%dd_temporal_k_kernel"
+        names["temporal"] = "ge%dd_temporal_k_kernel" if info.get("kform") == 0 or gk not in (2, 4, 8, 16, 32) else "ge%dd_unit_k_kernel"
     if cfg["dim"] == 3:
         names["per_step"] = "ge%dd_stream_kernel+shell" if info.get("form3d", 1) else "ge%dd_level_kernel"
     if kernel == "persistent":
-        name = "ge1d_rod_resident_kernel" if info["resident_path"] == 1 else "ge1d_grid_resident_kernel"
+        name = {1: "ge1d_rod_resident_kernel", 2: "ge1d_grid_resident_kernel", 3: "ge1d_rod_k_resident_kernel"}[info["resident_path"]]
     elif kernel == "temporal" and gk == 1 and info.get("temporal_c") in (18, 22, 26, 36, 44, 52):
         name = "ge1d_stream_kernel"                      # the TMA-staged form of strategy B
     elif kernel == "temporal" and cfg["dim"] == 2 and cfg["nx"] % 4 == 0 and cfg["nx"] >= 128:

@@ -728,7 +728,8 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     if (d->group_k >= 2) {                                  // k >= 2 (ge_level_k.cuh): strategy A, or C when the rod fits in shared memory
         const bool want_c = kernel == GE_KERNEL_AUTO || kernel == GE_KERNEL_PERSISTENT;
         const bool want_b = kernel != GE_KERNEL_PER_STEP;
-        const int tbk = d->tb > 0 ? d->tb : 16;    // measured on the C4-shaped rod
+        // measured on the C4-shaped rod: 32 for the register-resident form, 16 for the shared-memory one
+        const int tbk = d->tb > 0 ? d->tb : (ge::unit_k_compiled(d->dtype, d->group_k) ? 32 : 16);
         kernel = GE_KERNEL_PER_STEP;
         if (want_c && rod_k_fits(p)) { kernel = GE_KERNEL_PERSISTENT; p->res_path = 3; }
         else if (want_b && temporal_k_ok(p, tbk)) { kernel = GE_KERNEL_TEMPORAL; p->tb = tbk; }

@@ -26,7 +26,13 @@
 
 namespace ge {
 
-constexpr int kUnitWarps = 8;                     // warps of a CTA = one tile of 256 units
+#ifndef GE_UNIT_WARPS
+#define GE_UNIT_WARPS 8
+#endif
+#ifndef GE_UNIT_MINB
+#define GE_UNIT_MINB 3
+#endif
+constexpr int kUnitWarps = GE_UNIT_WARPS;         // warps of a CTA = one tile of 32 * kUnitWarps units
 
 struct UnitKGeom {
     int halo_lanes;        // units per side of a tile that are not stored
@@ -124,7 +130,7 @@ __device__ __forceinline__ void unit_level_p1(T (&v)[2 * K], const T from_prev, 
 }
 
 template <typename T, int K>
-__global__ void __launch_bounds__(32 * kUnitWarps, 2)
+__global__ void __launch_bounds__(32 * kUnitWarps, GE_UNIT_MINB)
 ge1d_unit_k_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, const Coef1<T>* __restrict__ coef,
                    const UnitKGeom g, int phase0, int levels) {
     constexpr int U = 2 * K, V = UnitPad<T, K>::V, CPL = UnitPad<T, K>::chunks, S = UnitPad<T, K>::stride;

@@ -292,11 +292,13 @@ def test_general_k_register_units(oracle, dtype, k, n, tb, batch):
 
 def test_general_k_auto_takes_the_blocked_kernel_on_long_rods():
     cfg = inputs.random_rods(1, 2 ** 20 - 2, "f64", seed=4)
-    _, info = run_gpu(cfg, 48, k=16, kform=0)
-    assert info["kernel"] == "temporal" and info["tb"] == 16 and info["launches"] == 3, info
-    assert info["tile_loaded"] - info["tile_valid"] == 2 * (16 * 17 + 2 * 16 + 2)
-    _, info = run_gpu(cfg, 48, k=16)
+    _, info = run_gpu(cfg, 96, k=16, kform=0)
+    assert info["kernel"] == "temporal" and info["tb"] == 32 and info["launches"] == 3, info
+    assert info["tile_loaded"] - info["tile_valid"] == 2 * (32 * 17 + 2 * 16 + 2)
+    _, info = run_gpu(cfg, 96, k=16)
     assert info["kernel"] == "temporal" and info["launches"] == 6, info        # register units + end windows
+    _, info = run_gpu(inputs.random_rods(1, 2 ** 20 - 2, "f64", seed=4), 48, k=3)
+    assert info["kernel"] == "temporal" and info["tb"] == 16 and info["launches"] == 3, info   # k = 3: shared-memory form
 
 
 def test_general_k_resident_needs_the_rod_to_fit():
