@@ -62,7 +62,7 @@ def make_cfg(name, scale=1.0):
     if name == "paper":                       # PAPER.md:204-218 run shape; use with --k 16
         return inputs.make_paper()
     if name in ("box_f32", "box_f64"):        # 3-D (NEXT-4), not a BASELINE.json config
-        n = int(512 * scale ** (1.0 / 3.0))
+        n = int(int(os.environ.get("GE_BOX_N", "512")) * scale ** (1.0 / 3.0))
         return inputs.make_box(n=n - n % 2, dtype=name[4:])
     raise SystemExit("unknown --config %s" % name)
 

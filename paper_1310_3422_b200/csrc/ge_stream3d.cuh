@@ -13,9 +13,9 @@
 //     plane -- both already in registers; per group 8 vector loads (4 own, 4 for the rows y-1 and y+2,
 //     which the warp above / below loads as its own: L1 / L2 hits), 4 vector stores;
 //   * the x neighbours (columns x-1, x+2) are the adjacent lanes' values: 8 shuffles; lanes 0 and 31 fetch
-//     theirs with one predicated scalar load each per row;
-//   * the next pair is loaded while a pair is computed (a second pair ahead, a cp.async ring in shared memory
-//     and L2 prefetches were measured and bring nothing: DESIGN.md section 7);
+//     theirs with one predicated scalar copy each per row, together with the pair (not when it is needed);
+//   * the pairs ahead travel through a lane-private cp.async ring in shared memory (depth 2; deeper rings, a
+//     second pair ahead in registers and L2 prefetches were measured and bring nothing: DESIGN.md section 7);
 //   * no boundary logic at all: only "deep" groups (the group and its 24 out-of-group neighbours interior,
 //     ge_level3d.cuh) are stored; addresses of anything else are clamped into the grid and the results
 //     dropped.  The outermost layer of groups -- first and last group index of every axis -- is left to
@@ -58,12 +58,13 @@ __device__ __forceinline__ void st2(T* __restrict__ p, T a, T b) {
 }
 
 // one group plane pair as a lane holds it: own[plane][row] = rows y, y+1; halo[plane][0 / 1] = rows y-1 / y+2
+// xe[plane][row]: lanes 0 / 31 only -- the column left / right of the warp's 64 (the x neighbour no lane holds)
 template <typename T>
-struct S3Pair { T own[2][2][2]; T halo[2][2][2]; };
+struct S3Pair { T own[2][2][2]; T halo[2][2][2]; T xe[2][2]; };
 
 template <typename T, bool VEC>
 __device__ __forceinline__ void s3_load_pair(const T* __restrict__ uin, int64_t sz, const int64_t (&ro)[4], int xa,
-                                             int xb, int z, int nz, S3Pair<T>& p) {
+                                             int xb, int z, int nz, S3Pair<T>& p, bool edge_lane, int xe_col) {
 #pragma unroll
     for (int pl = 0; pl < 2; ++pl) {
         int zz = z + pl;
@@ -73,11 +74,77 @@ __device__ __forceinline__ void s3_load_pair(const T* __restrict__ uin, int64_t 
         ld2<T, VEC>(b + ro[2], xa, xb, p.own[pl][1]);
         ld2<T, VEC>(b + ro[0], xa, xb, p.halo[pl][0]);
         ld2<T, VEC>(b + ro[3], xa, xb, p.halo[pl][1]);
+        // with the pair, not when it is needed: a load consumed in the iteration that issues it costs every warp a
+        // full memory latency per pair (that is what held the first form of this kernel at half the copy rate)
+        if (edge_lane) { p.xe[pl][0] = __ldg(b + ro[1] + xe_col); p.xe[pl][1] = __ldg(b + ro[2] + xe_col); }
     }
 }
 
+// ---- the pairs ahead wait in a lane-private shared-memory ring, not in registers ----
+// A load that waits in a register is issued where ptxas puts it (it batches or sinks look-ahead loads at will) and
+// caps the bytes in flight; cp.async does neither: every thread copies the row vectors of the pair RING-1 ahead
+// into its own slots ([slot][vector][thread]: conflict-free, no barrier -- a thread only reads what it copied).
+// Slot layout per thread: 8 vectors (own rows y, y+1, halo rows y-1, y+2 of the two planes), then 2 vectors holding
+// the four edge values of lanes 0 / 31.
+constexpr int kS3SlotVecs = 10;
+__device__ __forceinline__ void s3_cp_async(void* smem_dst, const void* gmem_src, int bytes) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    if (bytes == 16)     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+    else if (bytes == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+    else                 asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+template <typename T, bool VEC>
+__device__ __forceinline__ void s3_request_pair(const T* __restrict__ uin, int64_t sz, const int64_t (&ro)[4], int xa,
+                                                int xb, int z, int nz, T* __restrict__ slot, int stride, bool edge_lane,
+                                                int xe_col) {
+    constexpr int rows[4] = {1, 2, 0, 3};            // own rows y, y+1, then halo rows y-1, y+2
+#pragma unroll
+    for (int pl = 0; pl < 2; ++pl) {
+        int zz = z + pl;
+        zz = zz < 0 ? 0 : (zz > nz - 1 ? nz - 1 : zz);
+        const T* __restrict__ b = uin + zz * sz;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            T* dst = slot + (pl * 4 + i) * stride;
+            if constexpr (VEC) s3_cp_async(dst, b + ro[rows[i]] + xa, 2 * (int)sizeof(T));
+            else { s3_cp_async(dst, b + ro[rows[i]] + xa, (int)sizeof(T)); s3_cp_async(dst + 1, b + ro[rows[i]] + xb, (int)sizeof(T)); }
+        }
+        if (edge_lane) {
+            T* dst = slot + (8 + pl) * stride;
+            s3_cp_async(dst, b + ro[1] + xe_col, (int)sizeof(T));
+            s3_cp_async(dst + 1, b + ro[2] + xe_col, (int)sizeof(T));
+        }
+    }
+}
+template <typename T>
+__device__ __forceinline__ void s3_read_pair(const T* __restrict__ slot, int stride, S3Pair<T>& p) {
+#pragma unroll
+    for (int pl = 0; pl < 2; ++pl) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const typename Vec2<T>::type q = *reinterpret_cast<const typename Vec2<T>::type*>(slot + (pl * 4 + i) * stride);
+            if (i < 2) { p.own[pl][i][0] = q.x; p.own[pl][i][1] = q.y; }
+            else       { p.halo[pl][i - 2][0] = q.x; p.halo[pl][i - 2][1] = q.y; }
+        }
+        const typename Vec2<T>::type q = *reinterpret_cast<const typename Vec2<T>::type*>(slot + (8 + pl) * stride);
+        p.xe[pl][0] = q.x; p.xe[pl][1] = q.y;
+    }
+}
+__device__ __forceinline__ void s3_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void s3_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+#ifndef GE_S3D_RING_F32
+#define GE_S3D_RING_F32 2
+#endif
+#ifndef GE_S3D_RING_F64
+#define GE_S3D_RING_F64 2
+#endif
+template <typename T> struct S3Ring { static constexpr int n = sizeof(T) == 4 ? GE_S3D_RING_F32 : GE_S3D_RING_F64; };
+
+// RING: pairs of the ring (0: the next pair waits in registers instead).
 // Group indices start at 1 in every axis: index 0 and the last one are the shell's.
-template <typename T, int PH, bool VEC>
+template <typename T, int PH, bool VEC, int RING>
 __global__ void __launch_bounds__(32 * kS3Wy, GE_S3D_MINB)
 ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
                    const Coef3<T>* __restrict__ coef, int kseg) {
@@ -102,6 +169,11 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
     const int xl = x0 - 1;                                           // lane 0's left / lane 31's right neighbour column
     const int xr = x0 + 2 > nx - 1 ? nx - 1 : x0 + 2;
 
+    extern __shared__ __align__(16) unsigned char s3_smem[];
+    const int stride = 2 * 32 * kS3Wy;                               // elements between two vectors of a thread
+    T* ring = reinterpret_cast<T*>(s3_smem) + 2 * ((int)threadIdx.y * 32 + lane);
+    constexpr int kSlot = kS3SlotVecs * 2 * 32 * kS3Wy;              // elements of one ring slot (all threads)
+
     T prevU[2][2];                    // rows y, y+1 of the plane below the current pair
     S3Pair<T> cur, nxt;
     {
@@ -109,13 +181,33 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
         ld2<T, VEC>(b + ro[1], xa, xb, prevU[0]);
         ld2<T, VEC>(b + ro[2], xa, xb, prevU[1]);
     }
-    s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * k0 - PH, nz, cur);
-    s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * (k0 + 1) - PH, nz, nxt);
+    const bool edge_lane = lane == 0 || lane == 31;
+    const int xe_col = lane == 0 ? xl : xr;
+    s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * k0 - PH, nz, cur, edge_lane, xe_col);
+    int rslot = 0;                    // ring slot of pair k+1
+    if constexpr (RING > 0) {
+#pragma unroll
+        for (int q = 0; q < RING - 1; ++q) {
+            s3_request_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * (k0 + 1 + q) - PH, nz, ring + q * kSlot, stride, edge_lane, xe_col);
+            s3_commit();
+        }
+    } else {
+        s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, 2 * (k0 + 1) - PH, nz, nxt, edge_lane, xe_col);
+    }
 
     // unrolled by the period of the register rotation (cur <- nxt): no moves
 #pragma unroll(kS3Unroll ? 2 : 1)
     for (int k = k0; k < k1; ++k) {
         const int z0 = 2 * k - PH;
+        if constexpr (RING > 0) {
+            // pair k+RING goes into the slot pair k held (read at the previous iteration); then pair k+1 must have landed
+            const int wslot = rslot == 0 ? RING - 1 : rslot - 1;
+            s3_request_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 2 * RING, nz, ring + wslot * kSlot, stride, edge_lane, xe_col);
+            s3_commit();
+            s3_wait<RING - 1>();
+            s3_read_pair<T>(ring + rslot * kSlot, stride, nxt);
+            rslot = rslot + 1 == RING ? 0 : rslot + 1;
+        }
         // x neighbours of the four rows of the pair: columns x0-1 (left) and x0+2 (right)
         T lf[2][2], rt[2][2];
 #pragma unroll
@@ -125,15 +217,13 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
                 lf[pl][rr] = __shfl_up_sync(FULL, cur.own[pl][rr][1], 1);
                 rt[pl][rr] = __shfl_down_sync(FULL, cur.own[pl][rr][0], 1);
             }
-        if (lane == 0 || lane == 31) {
-            const T* __restrict__ pa = uin + (int64_t)z0 * sz + (lane == 0 ? xl : xr);
+#pragma unroll
+        for (int pl = 0; pl < 2; ++pl)
 #pragma unroll
             for (int rr = 0; rr < 2; ++rr) {
-                const T va = __ldg(pa + ro[1 + rr]);
-                const T vb = __ldg(pa + sz + ro[1 + rr]);
-                if (lane == 0) { lf[0][rr] = va; lf[1][rr] = vb; } else { rt[0][rr] = va; rt[1][rr] = vb; }
+                if (lane == 0) lf[pl][rr] = cur.xe[pl][rr];
+                if (lane == 31) rt[pl][rr] = cur.xe[pl][rr];
             }
-        }
         // right-hand sides, member d = dx + 2 dy + 4 dz (ge_level3d.cuh group3d)
         T R[8];
 #pragma unroll
@@ -167,7 +257,7 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 #pragma unroll
         for (int rr = 0; rr < 2; ++rr) { prevU[rr][0] = cur.own[1][rr][0]; prevU[rr][1] = cur.own[1][rr][1]; }
         cur = nxt;
-        s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 4, nz, nxt);
+        if constexpr (RING == 0) s3_load_pair<T, VEC>(uin, sz, ro, xa, xb, z0 + 4, nz, nxt, edge_lane, xe_col);
     }
 }
 
@@ -197,7 +287,13 @@ ge3d_shell_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int n
 template <typename T, int PH, bool VEC>
 inline cudaError_t stream3d_launch_one(const T* uin, T* uout, int nx, int ny, int nz, const Coef3<T>* coef, int kseg,
                                        dim3 grid, cudaStream_t s) {
-    ge3d_stream_kernel<T, PH, VEC><<<grid, dim3(32, kS3Wy), 0, s>>>(uin, uout, nx, ny, nz, coef, kseg);
+    constexpr int RING = S3Ring<T>::n;
+    constexpr size_t smem = (size_t)RING * kS3SlotVecs * 2 * 32 * kS3Wy * sizeof(T);
+    if (smem > 48 * 1024) {                    // idempotent, a few microseconds against a level of >= 100
+        const cudaError_t e = cudaFuncSetAttribute(ge3d_stream_kernel<T, PH, VEC, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    ge3d_stream_kernel<T, PH, VEC, RING><<<grid, dim3(32, kS3Wy), smem, s>>>(uin, uout, nx, ny, nz, coef, kseg);
     return cudaGetLastError();
 }
 
