@@ -49,6 +49,10 @@ def _load():
         lib.ge_ref_run_1d.restype = ctypes.c_int
         lib.ge_ref_run_batched_1d.argtypes = [_f64p, _i64, _i64, _f64p, _i64, _f64p, _f64p, _i64, _i64]
         lib.ge_ref_run_batched_1d.restype = ctypes.c_int
+        lib.ge_ref_level_1d_var.argtypes = [_f64p, _f64p, _i64, _f64p, _i64, _i64]
+        lib.ge_ref_level_1d_var.restype = None
+        lib.ge_ref_run_1d_var.argtypes = [_f64p, _i64, _f64p, _i64, _f64, _f64, _i64, _i64]
+        lib.ge_ref_run_1d_var.restype = ctypes.c_int
         lib.ge_ref_level_2d.argtypes = [_f64p, _f64p, _i64, _i64, _f64, _i64]
         lib.ge_ref_level_2d.restype = None
         lib.ge_ref_run_2d.argtypes = [_f64p, _i64, _i64, _f64, _f64p, _i64, _i64]
@@ -89,6 +93,30 @@ def level_1d_src(u, r, phase, bc_old, bc_new, s=None, k=1):
     _load().ge_ref_level_1d_src(old, new, n, float(r), int(k), int(phase),
                                 sp.ctypes.data if sp is not None else None, float(bc_new[0]), float(bc_new[1]))
     return new[1:-1].copy()
+
+
+def level_1d_var(u, rl, phase, bc_lo=0.0, bc_hi=0.0, k=1):
+    """One level with variable diffusivity (reading R-VAR): rl[j] = tau a_{j+1/2} / h^2 for the link between
+    nodes j and j+1, j = 0..N (N+1 numbers)."""
+    u = np.asarray(u, dtype=np.float64)
+    n = u.shape[0]
+    rl = np.ascontiguousarray(rl, dtype=np.float64)
+    assert rl.shape == (n + 1,)
+    old = np.empty(n + 2, dtype=np.float64)
+    old[0], old[-1] = bc_lo, bc_hi
+    old[1:-1] = u
+    new = np.empty_like(old)
+    _load().ge_ref_level_1d_var(old, new, n, rl, int(k), int(phase))
+    return new[1:-1].copy()
+
+
+def run_1d_var(u0, rl, steps, bc_lo=0.0, bc_hi=0.0, k=1, level0=0):
+    u = np.array(u0, dtype=np.float64, order="C", copy=True)
+    rl = np.ascontiguousarray(rl, dtype=np.float64)
+    assert rl.shape == (u.shape[0] + 1,)
+    if _load().ge_ref_run_1d_var(u, u.shape[0], rl, int(k), float(bc_lo), float(bc_hi), int(level0), int(steps)):
+        raise MemoryError("ge_ref_run_1d_var")
+    return u
 
 
 def run_1d(u0, r, steps, bc_lo=0.0, bc_hi=0.0, k=1, level0=0):

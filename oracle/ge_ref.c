@@ -434,3 +434,74 @@ int ge_ref_run_3d(double *u, int64_t Nx, int64_t Ny, int64_t Nz, double r, const
     free(a); free(b);
     return 0;
 }
+
+/*
+ * One level in 1-D with VARIABLE DIFFUSIVITY (reading R-VAR; SURVEY.md 8(f) NEXT-3 -- the paper's
+ * model problem has a constant coefficient; PAPER.md:37 names diffusion steps inside an
+ * operator splitting of full transport equations as the use):   u_t = (a(x) u_x)_x  in flux form,
+ *     (u_i^{n+1} - u_i^n)/tau = [ a_{i+1/2} (u_{i+1} - u_i) - a_{i-1/2} (u_i - u_{i-1}) ] / h^2 ,
+ * with one number per LINK:  rl[j] = tau a_{j+1/2} / h^2 > 0 for the link between nodes j and j+1, j = 0..N.
+ * Saul'yev's asymmetric equations take the flux through one link at the new level and through the other at
+ * the old level:
+ *   Eq (1) (ascending):  (1 + rl[i-1]) new_i = rl[i-1] new_{i-1} + (1 - rl[i]) old_i + rl[i] old_{i+1}
+ *   Eq (2) (descending): (1 + rl[i])   new_i = rl[i] new_{i+1} + (1 - rl[i-1]) old_i + rl[i-1] old_{i-1}
+ * and a confluence pair (i, i+1) is Eq (2) at i coupled with Eq (1) at i+1 -- its inner link rm = rl[i] at
+ * the new level, its outer links rl[i-1], rl[i+1] at the old level:
+ *   (1 + rm) new_i - rm new_{i+1} = p := (1 - rl[i-1]) old_i + rl[i-1] old_{i-1}
+ *   -rm new_i + (1 + rm) new_{i+1} = q := (1 - rl[i+1]) old_{i+1} + rl[i+1] old_{i+2}
+ * whose solution is written out below (determinant 1 + 2 rm).  With every rl[j] = r these are Eqs (1)-(4)
+ * of the paper.  Node classes, sweep order and boundary truncation are those of ge_ref_level_1d.
+ * old_, new_: length N+2 with the boundary values in [0] and [N+1]; rl: length N+1.
+ */
+void ge_ref_level_1d_var(const double *old_, double *new_, int64_t N, const double *rl,
+                         int64_t k, int64_t phase)
+{
+    const int64_t two_k = 2 * k;
+    int64_t i;
+    new_[0] = old_[0];
+    new_[N + 1] = old_[N + 1];
+    for (i = 0; i <= N; ++i) {
+        if (pmod(i - phase * k, two_k) != two_k - 1) continue;
+        if (i >= 1 && i + 1 <= N) {
+            const double rm = rl[i];
+            const double p = (1.0 - rl[i - 1]) * old_[i] + rl[i - 1] * old_[i - 1];
+            const double q = (1.0 - rl[i + 1]) * old_[i + 1] + rl[i + 1] * old_[i + 2];
+            new_[i] = ((1.0 + rm) * p + rm * q) / (1.0 + 2.0 * rm);
+            new_[i + 1] = (rm * p + (1.0 + rm) * q) / (1.0 + 2.0 * rm);
+        } else if (i == 0 && N >= 1) {
+            new_[1] = (rl[0] * new_[0] + (1.0 - rl[1]) * old_[1] + rl[1] * old_[2]) / (1.0 + rl[0]);
+        } else if (i == N && N >= 1) {
+            new_[N] = (rl[N] * new_[N + 1] + (1.0 - rl[N - 1]) * old_[N] + rl[N - 1] * old_[N - 1]) / (1.0 + rl[N]);
+        }
+    }
+    for (i = 1; i <= N; ++i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= 1 && c <= k - 1)
+            new_[i] = (rl[i - 1] * new_[i - 1] + (1.0 - rl[i]) * old_[i] + rl[i] * old_[i + 1]) / (1.0 + rl[i - 1]);
+    }
+    for (i = N; i >= 1; --i) {
+        int64_t c = pmod(i - phase * k, two_k);
+        if (c >= k && c <= two_k - 2)
+            new_[i] = (rl[i] * new_[i + 1] + (1.0 - rl[i - 1]) * old_[i] + rl[i - 1] * old_[i - 1]) / (1.0 + rl[i]);
+    }
+}
+
+/* `steps` levels with variable diffusivity; u: N interior values, overwritten; rl: N+1 link numbers. */
+int ge_ref_run_1d_var(double *u, int64_t N, const double *rl, int64_t k, double bc_lo, double bc_hi,
+                      int64_t level0, int64_t steps)
+{
+    double *a = (double *)malloc((size_t)(N + 2) * sizeof(double));
+    double *b = (double *)malloc((size_t)(N + 2) * sizeof(double));
+    int64_t s;
+    if (!a || !b) { free(a); free(b); return -1; }
+    a[0] = bc_lo; a[N + 1] = bc_hi;
+    memcpy(a + 1, u, (size_t)N * sizeof(double));
+    for (s = 0; s < steps; ++s) {
+        double *t;
+        ge_ref_level_1d_var(a, b, N, rl, k, pmod(level0 + s, 2));
+        t = a; a = b; b = t;
+    }
+    memcpy(u, a + 1, (size_t)N * sizeof(double));
+    free(a); free(b);
+    return 0;
+}

@@ -79,6 +79,50 @@ def level_1d_dense_src(u, r, k, phase, bc_old, bc_new, s=None):
     return np.linalg.solve(A, B @ np.asarray(u, dtype=np.float64) + c)
 
 
+def system_1d_var(n, rl, k, phase, bc_lo, bc_hi, num=float):
+    """Variable diffusivity (reading R-VAR): rl[j] belongs to the link between nodes j and j+1.  Node by node:
+    (1 + r_new) new_i - r_new new_{jn} = (1 - r_old) old_i + r_old old_{jo}, the rule table only deciding which
+    neighbour jn is taken at the new level.  Returns (A, B, c) with A new = B old + c."""
+    zero, one = num(0), num(1)
+    A = [[zero] * n for _ in range(n)]
+    B = [[zero] * n for _ in range(n)]
+    c = [zero] * n
+    bval = {0: num(bc_lo), n + 1: num(bc_hi)}
+    side = classes_1d(n, k, phase)
+    for i in range(1, n + 1):
+        jn, jo = i + side[i], i - side[i]
+        rn, ro = num(rl[min(i, jn)]), num(rl[min(i, jo)])
+        A[i - 1][i - 1] = one + rn
+        B[i - 1][i - 1] = one - ro
+        if jn in bval:
+            c[i - 1] += rn * bval[jn]
+        else:
+            A[i - 1][jn - 1] -= rn
+        if jo in bval:
+            c[i - 1] += ro * bval[jo]
+        else:
+            B[i - 1][jo - 1] += ro
+    return A, B, c
+
+
+def level_1d_var_exact(u, rl, k, phase, bc_lo=0, bc_hi=0):
+    n = len(u)
+    A, B, c = system_1d_var(n, [Fraction(x) for x in rl], k, phase, bc_lo, bc_hi, num=Fraction)
+    rhs = [sum(B[i][j] * Fraction(u[j]) for j in range(n)) + c[i] for i in range(n)]
+    return solve_exact(A, rhs)
+
+
+def level_1d_var_dense(u, rl, k, phase, bc_lo=0.0, bc_hi=0.0):
+    n = len(u)
+    A, B, c = system_1d_var(n, [float(x) for x in rl], k, phase, bc_lo, bc_hi)
+    return np.linalg.solve(np.array(A), np.array(B) @ np.asarray(u, dtype=np.float64) + np.array(c))
+
+
+def operator_1d_var(n, rl, k, phase):
+    A, B, _ = system_1d_var(n, [float(x) for x in rl], k, phase, 0.0, 0.0)
+    return np.linalg.solve(np.array(A), np.array(B))
+
+
 def solve_exact(A, b):
     """Gaussian elimination over Fractions."""
     n = len(A)
