@@ -116,6 +116,15 @@ int ge_step_3d(ge_plan *p, const void *u_in, void *u_out, ge_stream_t stream);
 int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f, const double *bc4,
                    ge_stream_t stream);
 
+/* One level of a single rod (batch == 1, group_k == 1) with VARIABLE DIFFUSIVITY (DESIGN.md
+ * reading R-VAR; the paper's coefficient is constant): u_t = (a(x) u_x)_x in flux form.
+ *   rl: device pointer, nx + 1 elements of dtype: rl[j] = tau * a(x_{j+1/2}) / h^2 > 0 for the link between nodes j
+ *       and j+1, j = 0 .. N (the plan's own r is not used; the boundary values are the plan's).
+ * Otherwise as ge_step_1d.  ge_run_var: `steps` such levels in place (one launch per level, result in u).
+ * GE_EINVAL for batch > 1, dim != 1 or a null / misaligned pointer, GE_EUNSUPPORTED for group_k >= 2. */
+int ge_step_1d_var(ge_plan *p, const void *u_in, void *u_out, const void *rl, ge_stream_t stream);
+int ge_run_var(ge_plan *p, void *u, int64_t steps, const void *rl, ge_stream_t stream);
+
 /* `steps` >= 0 levels of ge_step_1d_src in place (same restrictions: one rod, group_k == 1; one launch per level,
  * ping-pong with the plan's scratch level, result in u, level += steps):
  *   tau_f:          device pointer or NULL.  f_level_stride == 0: one stationary source of nx elements used at

@@ -23,6 +23,7 @@
 #include "ge_level_src.cuh"
 #include "ge_probe.cuh"
 #include "ge_tail.cuh"
+#include "ge_level_var.cuh"
 
 namespace {
 
@@ -784,6 +785,40 @@ int ge_step_1d_src(ge_plan* p, const void* u_in, void* u_out, const void* tau_f,
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     p->launches += 1;
     p->level += 1;
+    return GE_OK;
+}
+
+int ge_step_1d_var(ge_plan* p, const void* u_in, void* u_out, const void* rl, ge_stream_t stream) {
+    if (!p || !u_in || !u_out || u_in == u_out || !rl || p->dim != 1 || p->batch != 1) return GE_EINVAL;
+    if (p->group_k != 1) return GE_EUNSUPPORTED;
+    const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)u_in % es || (uintptr_t)u_out % es || (uintptr_t)rl % es) return GE_EINVAL;
+    const char* a = (const char*)u_in; const char* b = (const char*)u_out;
+    const size_t bytes = (size_t)p->count * es;
+    if ((a < b + bytes) && (b < a + bytes)) return GE_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    p->last_stream = s;
+    const int phase = (int)(p->level & 1);
+    const cudaError_t e = p->dtype == GE_F64
+        ? ge::level_var_launch<double>((const double*)u_in, (double*)u_out, (const double*)rl, p->nx, (const ge::Coef1<double>*)p->coef, phase, s)
+        : ge::level_var_launch<float>((const float*)u_in, (float*)u_out, (const float*)rl, p->nx, (const ge::Coef1<float>*)p->coef, phase, s);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += 1;
+    return GE_OK;
+}
+
+int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t stream) {
+    if (!p || !u || steps < 0 || !rl) return GE_EINVAL;
+    NvtxRange nvtx("ge_run_var");
+    void* cur = u;
+    void* oth = p->scratch;
+    for (int64_t n = 0; n < steps; ++n) {
+        const int rc = ge_step_1d_var(p, cur, oth, rl, stream);
+        if (rc != GE_OK) return rc;
+        void* t = cur; cur = oth; oth = t;
+    }
+    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * elem_size(p->dtype), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return GE_OK;
 }
 

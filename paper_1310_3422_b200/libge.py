@@ -33,7 +33,7 @@ _KERNEL_IDS = {v: k for k, v in KERNEL_NAMES.items()}
 _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 
 # every symbol include/ge.h declares
-EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_run_src", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
+EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_run_src", "ge_step_1d_var", "ge_run_var", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
            "ge_fma_probe", "ge_strerror", "ge_version")
 
@@ -80,6 +80,8 @@ def load() -> ctypes.CDLL:
     lib.ge_step_3d.argtypes = [vp, vp, vp, vp]
     lib.ge_step_1d_src.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run.argtypes = [vp, vp, i64, vp]
+    lib.ge_step_1d_var.argtypes = [vp, vp, vp, vp, vp]
+    lib.ge_run_var.argtypes = [vp, vp, i64, vp, vp]
     lib.ge_run_src.argtypes = [vp, vp, i64, vp, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_run_host.argtypes = [vp, vp, i64, vp]
     lib.ge_plan_get_level.argtypes = [vp, ctypes.POINTER(i64)]
@@ -170,6 +172,15 @@ def ge_run_src(plan: int, u: int, steps: int, tau_f: int, f_level_stride: int, b
     _check(load().ge_run_src(plan, u, steps, tau_f or None, f_level_stride, lo, hi, stream), "ge_run_src")
 
 
+def ge_step_1d_var(plan: int, u_in: int, u_out: int, rl: int, stream: int = 0):
+    """rl: device pointer to nx + 1 link numbers tau * a_{j+1/2} / h^2."""
+    _check(load().ge_step_1d_var(plan, u_in, u_out, rl, stream), "ge_step_1d_var")
+
+
+def ge_run_var(plan: int, u: int, steps: int, rl: int, stream: int = 0):
+    _check(load().ge_run_var(plan, u, steps, rl, stream), "ge_run_var")
+
+
 def ge_run_host(plan: int, u_host: int, steps: int, stream: int = 0):
     _check(load().ge_run_host(plan, u_host, steps, stream), "ge_run_host")
 
@@ -238,6 +249,12 @@ class Plan:
 
     def run_src(self, u: int, steps: int, tau_f: int, f_level_stride: int, bc_lo_t, bc_hi_t, stream: int = 0):
         ge_run_src(self.handle, u, steps, tau_f, f_level_stride, bc_lo_t, bc_hi_t, stream)
+
+    def step_var(self, u_in: int, u_out: int, rl: int, stream: int = 0):
+        ge_step_1d_var(self.handle, u_in, u_out, rl, stream)
+
+    def run_var(self, u: int, steps: int, rl: int, stream: int = 0):
+        ge_run_var(self.handle, u, steps, rl, stream)
 
     def run_host(self, u_host: int, steps: int, stream: int = 0):
         ge_run_host(self.handle, u_host, steps, stream)
