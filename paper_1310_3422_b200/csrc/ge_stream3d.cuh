@@ -36,7 +36,12 @@ namespace ge {
 #define GE_S3D_UNROLL 1
 #endif
 constexpr int kS3Unroll = GE_S3D_UNROLL;
-constexpr int kS3Wy = GE_S3D_WY;          // warps of a CTA, stacked in y (their halo rows are each other's own rows)
+#ifndef GE_S3D_WX
+#define GE_S3D_WX 1
+#endif
+constexpr int kS3Wx = GE_S3D_WX;          // warps of a CTA side by side in x (a CTA then reads kS3Wx * 64 consecutive nodes of a row)
+constexpr int kS3Wy = GE_S3D_WY;          // ... and stacked in y (their halo rows are each other's own rows)
+constexpr int kS3Warps = kS3Wx * kS3Wy;
 
 template <typename T> struct Vec2;
 template <> struct Vec2<float>  { using type = float2; };
@@ -145,13 +150,14 @@ template <typename T> struct S3Ring { static constexpr int n = sizeof(T) == 4 ? 
 // RING: pairs of the ring (0: the next pair waits in registers instead).
 // Group indices start at 1 in every axis: index 0 and the last one are the shell's.
 template <typename T, int PH, bool VEC, int RING>
-__global__ void __launch_bounds__(32 * kS3Wy, GE_S3D_MINB)
+__global__ void __launch_bounds__(32 * kS3Warps, GE_S3D_MINB)
 ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
                    const Coef3<T>* __restrict__ coef, int kseg) {
     constexpr unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x;
-    const int x0 = 2 * (1 + (int)blockIdx.x * 32 + lane) - PH;       // anchor element of the lane's group column
-    const int y0 = 2 * (1 + (int)blockIdx.y * kS3Wy + (int)threadIdx.y) - PH;
+    const int wx = (int)threadIdx.y % kS3Wx, wy = (int)threadIdx.y / kS3Wx;
+    const int x0 = 2 * (1 + ((int)blockIdx.x * kS3Wx + wx) * 32 + lane) - PH;   // anchor element of the lane's group column
+    const int y0 = 2 * (1 + (int)blockIdx.y * kS3Wy + wy) - PH;
     if (!(y0 + 2 < ny)) return;                                      // the whole warp: its group row is shell or beyond
     const bool deep_x = x0 + 2 < nx;
     const int klast = (nz - 1 + PH) / 2;                             // last group plane pair (shell)
@@ -170,9 +176,9 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
     const int xr = x0 + 2 > nx - 1 ? nx - 1 : x0 + 2;
 
     extern __shared__ __align__(16) unsigned char s3_smem[];
-    const int stride = 2 * 32 * kS3Wy;                               // elements between two vectors of a thread
+    const int stride = 2 * 32 * kS3Warps;                            // elements between two vectors of a thread
     T* ring = reinterpret_cast<T*>(s3_smem) + 2 * ((int)threadIdx.y * 32 + lane);
-    constexpr int kSlot = kS3SlotVecs * 2 * 32 * kS3Wy;              // elements of one ring slot (all threads)
+    constexpr int kSlot = kS3SlotVecs * 2 * 32 * kS3Warps;           // elements of one ring slot (all threads)
 
     T prevU[2][2];                    // rows y, y+1 of the plane below the current pair
     S3Pair<T> cur, nxt;
@@ -288,12 +294,12 @@ template <typename T, int PH, bool VEC>
 inline cudaError_t stream3d_launch_one(const T* uin, T* uout, int nx, int ny, int nz, const Coef3<T>* coef, int kseg,
                                        dim3 grid, cudaStream_t s) {
     constexpr int RING = S3Ring<T>::n;
-    constexpr size_t smem = (size_t)RING * kS3SlotVecs * 2 * 32 * kS3Wy * sizeof(T);
+    constexpr size_t smem = (size_t)RING * kS3SlotVecs * 2 * 32 * kS3Warps * sizeof(T);
     if (smem > 48 * 1024) {                    // idempotent, a few microseconds against a level of >= 100
         const cudaError_t e = cudaFuncSetAttribute(ge3d_stream_kernel<T, PH, VEC, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    ge3d_stream_kernel<T, PH, VEC, RING><<<grid, dim3(32, kS3Wy), smem, s>>>(uin, uout, nx, ny, nz, coef, kseg);
+    ge3d_stream_kernel<T, PH, VEC, RING><<<grid, dim3(32, kS3Warps), smem, s>>>(uin, uout, nx, ny, nz, coef, kseg);
     return cudaGetLastError();
 }
 
@@ -326,12 +332,13 @@ inline cudaError_t stream3d_launch(const T* uin, T* uout, int64_t nx, int64_t ny
     if (side) { e = cudaEventRecord(ev_out, aux); if (e != cudaSuccess) return e; }
     if (gx > 0 && gy > 0 && gz > 0) {
         // z segments: enough CTAs for ~8 resident CTAs on every SM, at least 8 pairs per segment
-        const int64_t ctas_xy = ((gx + 31) / 32) * ((gy + kS3Wy - 1) / kS3Wy);
+        const int64_t bx = (gx + 32 * kS3Wx - 1) / (32 * kS3Wx);
+        const int64_t ctas_xy = bx * ((gy + kS3Wy - 1) / kS3Wy);
         int64_t segs = (8 * (int64_t)sm_count + ctas_xy - 1) / ctas_xy;
         if (segs > gz / 8) segs = gz / 8;
         if (segs < 1) segs = 1;
         const int kseg = (int)((gz + segs - 1) / segs);
-        dim3 grid((unsigned)((gx + 31) / 32), (unsigned)((gy + kS3Wy - 1) / kS3Wy), (unsigned)((gz + kseg - 1) / kseg));
+        dim3 grid((unsigned)bx, (unsigned)((gy + kS3Wy - 1) / kS3Wy), (unsigned)((gz + kseg - 1) / kseg));
         const bool vec = phase == 0 && nx % 2 == 0 && (((uintptr_t)uin | (uintptr_t)uout) % (2 * sizeof(T))) == 0;
         if (phase == 0) e = vec ? stream3d_launch_one<T, 0, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s)
                                 : stream3d_launch_one<T, 0, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s);

@@ -8,6 +8,7 @@
 #include "../paper_1310_3422_b200/csrc/ge_temporal.cuh"
 #include "../paper_1310_3422_b200/csrc/ge_strip2d.cuh"
 #include "../paper_1310_3422_b200/csrc/ge_level_k.cuh"
+#include "../paper_1310_3422_b200/csrc/ge_unit_k.cuh"
 
 static int fails = 0;
 #define CHECK(cond, ...) do { if (!(cond)) { if (fails < 20) { std::printf("FAIL %s: ", #cond); std::printf(__VA_ARGS__); std::printf("\n"); } ++fails; } } while (0)
@@ -66,7 +67,56 @@ static void check_units(int k, int phase, int64_t nx) {
     CHECK(r.threads == 0 || r.threads >= g.units, "rod threads k=%d nx=%lld", k, (long long)nx);
 }
 
+// blocked k >= 2 kernels (r02): the shared-memory windows must deliver every node exactly once with at least
+// tb (k+1) nodes between an output and a cut end of its window; the register form's tiles must deliver every unit
+// exactly once with enough halo lanes, and the end windows must cover what the rod's ends spoil.
+static void check_temporal_k(int k, int tb, int64_t nx) {
+    const ge::TemporalKGeom g = ge::temporal_k_geom(k, tb, nx, 8, 64 * 1024);
+    if (g.valid <= 0) return;
+    CHECK(g.halo >= tb * (k + 1) && g.window == g.valid + 2 * g.halo && g.threads <= 1024 && g.threads * 2 * k >= g.window + 2 * k,
+          "temporal_k geom k=%d tb=%d nx=%lld", k, tb, (long long)nx);
+    CHECK(g.smem <= 64 * 1024 + 1024, "temporal_k smem k=%d tb=%d", k, tb);
+    int64_t covered = 0;
+    for (int64_t t = 0; t < g.tiles; ++t) {
+        const int64_t v0 = 1 + t * g.valid, v1 = v0 + g.valid < nx + 1 ? v0 + g.valid : nx + 1;
+        CHECK(v0 == covered + 1 && v1 > v0, "temporal_k cover k=%d nx=%lld t=%lld", k, (long long)nx, (long long)t);
+        covered = v1 - 1;
+    }
+    CHECK(covered == nx, "temporal_k total k=%d tb=%d nx=%lld covered=%lld", k, tb, (long long)nx, (long long)covered);
+}
+static void check_unit_k(int k, int tb, int64_t nx) {
+    const ge::UnitKGeom g = ge::unit_k_geom(k, tb, nx);
+    if (g.valid_lanes < 64) return;
+    CHECK(g.halo_lanes * 2 * k >= tb * (k + 1) + 2 * k, "unit halo k=%d tb=%d lanes=%d", k, tb, g.halo_lanes);
+    const int64_t units = (nx + 2 * k - 1) / (2 * k);
+    CHECK(g.tiles * g.valid_lanes >= units && (g.tiles - 1) * g.valid_lanes < units, "unit tiles k=%d nx=%lld", k, (long long)nx);
+    // the end windows of ge_api.cu: tb (k+1) + 4k + 8 nodes, and their shared-memory window fits
+    const int64_t end_len = (int64_t)tb * (k + 1) + 4 * k + 8;
+    const ge::TemporalKGeom e = ge::temporal_k_ends_geom(k, tb, end_len, 8);
+    CHECK(e.valid == end_len && e.threads * 2 * k >= e.window && e.smem <= 64 * 1024, "end windows k=%d tb=%d", k, tb);
+    CHECK(end_len >= g.halo_lanes * 0 + tb * (k + 1) + 2 * k, "end length k=%d tb=%d", k, tb);
+}
+// cooperative 2-D strips: COOP warps share one strip
+static void check_coop_strips(int C, int V, int TB, int COOP, int64_t nx) {
+    if (nx < (int64_t)COOP * 32 * C || nx % 4) return;
+    const ge::Strip2dGeom g = ge::strip2d_coop_geom(C, V, TB, COOP, nx, 64, 8);
+    const int64_t W = (int64_t)COOP * 32 * C;
+    std::vector<int> hits((size_t)nx, 0);
+    for (int s = 0; s < g.nstrips; ++s) {
+        const bool first = s == 0, last = s == g.nreg;
+        const int64_t a0 = first ? 0 : (last ? nx - W : (int64_t)s * g.valid - g.halo);
+        const int64_t lo = (int64_t)s * g.valid, hi = last ? nx : lo + g.valid;
+        CHECK(a0 >= 0 && a0 + W <= nx && a0 % V == 0 && (first || lo - a0 >= TB) && (last || a0 + W - hi >= TB),
+              "coop strip nx=%lld s=%d", (long long)nx, s);
+        for (int64_t e = lo; e < hi; ++e) hits[(size_t)e]++;
+    }
+    for (int64_t e = 0; e < nx; ++e) if (hits[(size_t)e] != 1) { CHECK(false, "coop cover nx=%lld e=%lld hits=%d", (long long)nx, (long long)e, hits[(size_t)e]); break; }
+}
+
 int main() {
+    for (int k : {2, 3, 5, 16, 64, 200}) for (int tb : {1, 4, 8, 16, 32}) for (int64_t nx : {40000, 70001, 262142, 1048576}) check_temporal_k(k, tb, nx);
+    for (int k : {2, 4, 8, 16, 32}) for (int tb : {1, 5, 8, 16, 32, 48}) for (int64_t nx : {40000, 70001, 262142, 1048576, 268435456}) check_unit_k(k, tb, nx);
+    for (int coop : {2, 4, 8}) for (int64_t nx : {512, 1024, 1032, 2600, 4104, 8192}) { check_coop_strips(4, 4, 6, coop, nx); check_coop_strips(2, 2, 6, coop, nx); }
     const int Cs64[] = {8, 16, 18, 22, 26, 32}, Cs32[] = {16, 32, 36, 44, 52, 64};
     const int64_t extra[] = {0, 2, 4, 8, 100, 576, 1000, 4098, 65536};
     for (int phase = 0; phase < 2; ++phase)
