@@ -297,6 +297,15 @@ def fma_peaks(dev, stream_obj):
             torch.cuda.synchronize(dev)
             best = max(best, flops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
         out[dt + "_tflops"] = best
+        # the same with three distinct registers per FMA (what real kernels look like to the register file): context,
+        # not the roofline denominator
+        libge.ge_fma_probe(dt, 1 << 12, sink.data_ptr(), stream_obj.cuda_stream, 1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream_obj)
+        flops = libge.ge_fma_probe(dt, iters, sink.data_ptr(), stream_obj.cuda_stream, 1)
+        e1.record(stream_obj)
+        torch.cuda.synchronize(dev)
+        out[dt + "_tflops_distinct_operands"] = flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
     clk = float(measured_peaks()[0].get("sm_max_mhz", 1965.0)) * 1e6
     out["derived"] = {dt + "_tflops": 2.0 * LANES[dt] * SMS * clk / 1e12 for dt in ("f32", "f64")}
     out["how"] = ("ge_fma_probe (csrc/ge_probe.cuh): 8 independent dependent-FMA chains per thread, 2048 threads per SM, "

@@ -212,6 +212,10 @@ int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
  * sink: device pointer to at least 8 writable bytes (never written in practice).  GE_EINVAL for a bad
  * dtype, iters < 1 or a null pointer. */
 int ge_fma_probe(int32_t dtype, int64_t iters, void *sink, double *flops, ge_stream_t stream);
+/* The same with a choice of operand pattern: variant 0 = ge_fma_probe (x <- x*a + b, a and b shared by all chains: the
+ * pipe's own rate), 1 = three DISTINCT registers per FMA (x <- x*y_c + z_c, y and z per chain), which is what the
+ * arithmetic of the kernels looks like to the register file.  GE_EINVAL for any other variant. */
+int ge_fma_probe_ex(int32_t dtype, int32_t variant, int64_t iters, void *sink, double *flops, ge_stream_t stream);
 
 /* Frees the plan's device buffers (stream-ordered on the stream last used) and the plan. */
 int ge_plan_destroy(ge_plan *p);

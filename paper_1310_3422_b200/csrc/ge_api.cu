@@ -1255,12 +1255,16 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
 }
 
 int ge_fma_probe(int32_t dtype, int64_t iters, void* sink, double* flops, ge_stream_t stream) {
-    if ((dtype != GE_F32 && dtype != GE_F64) || iters < 1 || !sink || !flops) return GE_EINVAL;
+    return ge_fma_probe_ex(dtype, 0, iters, sink, flops, stream);
+}
+
+int ge_fma_probe_ex(int32_t dtype, int32_t variant, int64_t iters, void* sink, double* flops, ge_stream_t stream) {
+    if ((dtype != GE_F32 && dtype != GE_F64) || iters < 1 || !sink || !flops || variant < 0 || variant > 1) return GE_EINVAL;
     int dev = 0, sms = 0;
     GE_CUDA(cudaGetDevice(&dev));
     GE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const cudaError_t e = dtype == GE_F64 ? ge::fma_probe_launch<double>((double*)sink, iters, sms, flops, (cudaStream_t)stream)
-                                          : ge::fma_probe_launch<float>((float*)sink, iters, sms, flops, (cudaStream_t)stream);
+    const cudaError_t e = dtype == GE_F64 ? ge::fma_probe_launch<double>((double*)sink, iters, sms, flops, (cudaStream_t)stream, variant == 1)
+                                          : ge::fma_probe_launch<float>((float*)sink, iters, sms, flops, (cudaStream_t)stream, variant == 1);
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     return GE_OK;
 }

@@ -17,19 +17,26 @@ constexpr int kProbeUnroll = 32;
 constexpr int kProbeThreads = 256;
 constexpr int kProbeBlocksPerSm = 8;      // 2048 threads per SM
 
-template <typename T>
+// DISTINCT: every FMA reads three different registers (x <- x*y[c] + z[c], y and z per chain) instead of sharing its
+// multiplier and addend with the other chains -- what the arithmetic of a real kernel looks like to the register
+// file: the difference between the two variants is what operand delivery costs on top of the pipe itself.
+template <typename T, bool DISTINCT>
 __global__ void __launch_bounds__(kProbeThreads, kProbeBlocksPerSm)
 ge_fma_probe_kernel(T* __restrict__ sink, T a, T b, int64_t iters) {
-    T x[kProbeChains];
+    T x[kProbeChains], y[kProbeChains], z[kProbeChains];
 #pragma unroll
-    for (int c = 0; c < kProbeChains; ++c) x[c] = T(threadIdx.x + c) * a;
+    for (int c = 0; c < kProbeChains; ++c) {
+        x[c] = T(threadIdx.x + c) * a;
+        y[c] = DISTINCT ? a - T(c) * T(0.001) : a;
+        z[c] = DISTINCT ? b + T(c) * T(0.001) : b;
+    }
     // 32 x 8 = 256 FMAs per trip: the counter, compare and branch are 1 % of the issue slots
 #pragma unroll 1
     for (int64_t i = 0; i < iters; i += kProbeUnroll) {
 #pragma unroll
         for (int u = 0; u < kProbeUnroll; ++u)
 #pragma unroll
-            for (int c = 0; c < kProbeChains; ++c) x[c] = fma(x[c], a, b);
+            for (int c = 0; c < kProbeChains; ++c) x[c] = fma(x[c], y[c], z[c]);
     }
     T s = T(0);
 #pragma unroll
@@ -41,10 +48,11 @@ ge_fma_probe_kernel(T* __restrict__ sink, T a, T b, int64_t iters) {
 
 // Enqueues one launch; returns the flops it performs (an FMA counts 2).
 template <typename T>
-inline cudaError_t fma_probe_launch(T* sink, int64_t iters, int sm_count, double* flops, cudaStream_t s) {
+inline cudaError_t fma_probe_launch(T* sink, int64_t iters, int sm_count, double* flops, cudaStream_t s, bool distinct = false) {
     iters = (iters + kProbeUnroll - 1) / kProbeUnroll * kProbeUnroll;
     const int blocks = sm_count * kProbeBlocksPerSm;
-    ge_fma_probe_kernel<T><<<blocks, kProbeThreads, 0, s>>>(sink, T(0.999), T(0.001), iters);
+    if (distinct) ge_fma_probe_kernel<T, true><<<blocks, kProbeThreads, 0, s>>>(sink, T(0.999), T(0.001), iters);
+    else          ge_fma_probe_kernel<T, false><<<blocks, kProbeThreads, 0, s>>>(sink, T(0.999), T(0.001), iters);
     *flops = 2.0 * kProbeChains * (double)iters * (double)blocks * kProbeThreads;
     return cudaGetLastError();
 }

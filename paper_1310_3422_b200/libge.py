@@ -35,7 +35,7 @@ _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 # every symbol include/ge.h declares
 EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_run_src", "ge_step_1d_var", "ge_run_var", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
-           "ge_fma_probe", "ge_strerror", "ge_version")
+           "ge_fma_probe", "ge_fma_probe_ex", "ge_strerror", "ge_version")
 
 
 class ge_desc(ctypes.Structure):
@@ -90,6 +90,7 @@ def load() -> ctypes.CDLL:
     lib.ge_plan_tune.argtypes = [vp, i32, i64]
     lib.ge_plan_destroy.argtypes = [vp]
     lib.ge_fma_probe.argtypes = [i32, i64, vp, ctypes.POINTER(ctypes.c_double), vp]
+    lib.ge_fma_probe_ex.argtypes = [i32, i32, i64, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_strerror.argtypes = [ctypes.c_int]
     lib.ge_strerror.restype = ctypes.c_char_p
     lib.ge_version.argtypes = []
@@ -205,11 +206,12 @@ def ge_plan_tune(plan: int, what: int, value: int):
     _check(load().ge_plan_tune(plan, what, value), "ge_plan_tune")
 
 
-def ge_fma_probe(dtype, iters: int, sink: int, stream: int = 0) -> float:
-    """Enqueue one launch of the FMA throughput probe; returns the flops of that launch."""
+def ge_fma_probe(dtype, iters: int, sink: int, stream: int = 0, variant: int = 0) -> float:
+    """Enqueue one launch of the FMA throughput probe; returns the flops of that launch.  variant 1: three distinct
+    registers per FMA (ge_fma_probe_ex)."""
     v = ctypes.c_double()
-    _check(load().ge_fma_probe(_DTYPES[dtype] if isinstance(dtype, str) else int(dtype), iters, sink,
-                               ctypes.byref(v), stream), "ge_fma_probe")
+    _check(load().ge_fma_probe_ex(_DTYPES[dtype] if isinstance(dtype, str) else int(dtype), variant, iters, sink,
+                                  ctypes.byref(v), stream), "ge_fma_probe_ex")
     return v.value
 
 
