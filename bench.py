@@ -717,8 +717,10 @@ def run_sweep(args):
 
 
 def run_src(args):
-    """NEXT-3 measurement: `levels` launches of ge_step_1d_src (source array + moving boundary values) on
-    the C4-shaped rod; HBM-bound, 3*sizeof(T) algorithmic bytes per update (u in, tau*f in, u out)."""
+    """NEXT-3 measurement on the C4-shaped rod: the source term + moving boundary values (--src) or variable diffusivity
+    (--var), temporally blocked through ge_run_src / ge_run_var (stationary data, 16 levels per launch) or, with
+    --kernel per_step, one launch of ge_step_1d_src / ge_step_1d_var per level (HBM-bound: 3*sizeof(T) algorithmic bytes
+    per update -- u in, tau*f or the link numbers in, u out)."""
     import torch
     from paper_1310_3422_b200 import build as gebuild, libge
     gebuild.build()
@@ -731,18 +733,35 @@ def run_src(args):
     stream = stream_obj.cuda_stream
     u = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
     v = torch.empty_like(u)
-    src = torch.full_like(u, 1e-9)
+    n = cfg["nx"]
+    per_level = args.kernel == "per_step"
+    what = "var" if args.var else "src"
+    if args.var:
+        data = torch.full((n + 1,), 2.0, dtype=u.dtype, device=dev)
+        data += 0.5 * torch.sin(torch.arange(n + 1, device=dev, dtype=u.dtype) * 1e-3)
+    else:
+        data = torch.full_like(u, 1e-9)
+    lo = [1e-3 * i for i in range(levels + 1)]
+    hi = [-1e-3 * i for i in range(levels + 1)]
     plan = libge.Plan(cfg, kernel="per_step", stream=stream)
 
     def step():
-        a, b = u, v
-        for n in range(levels):
-            t = 1e-3 * n
-            plan.step_src(a.data_ptr(), b.data_ptr(), src.data_ptr(), (t, t + 1e-3, -t, -t - 1e-3), stream)
-            a, b = b, a
+        if per_level:
+            a, b = u, v
+            for i in range(levels):
+                if args.var:
+                    plan.step_var(a.data_ptr(), b.data_ptr(), data.data_ptr(), stream)
+                else:
+                    plan.step_src(a.data_ptr(), b.data_ptr(), data.data_ptr(), (lo[i], lo[i + 1], hi[i], hi[i + 1]), stream)
+                a, b = b, a
+        elif args.var:
+            plan.run_var(u.data_ptr(), levels, data.data_ptr(), stream)
+        else:
+            plan.run_src(u.data_ptr(), levels, data.data_ptr(), 0, lo, hi, stream)
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize(dev)
+    l0 = plan.info()["launches"]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream_obj)
     for _ in range(args.steps):
@@ -750,21 +769,32 @@ def run_src(args):
     e1.record(stream_obj)
     torch.cuda.synchronize(dev)
     ms = e0.elapsed_time(e1)
+    launches = plan.info()["launches"] - l0
     peaks, srcp = measured_peaks()
-    upd = cfg["nx"] * levels * args.steps
-    gbs = 3.0 * es * upd / (ms * 1e-3) / 1e9
+    upd = n * levels * args.steps
+    glups = upd / (ms * 1e-3) / 1e9
+    kname = ("ge1d_level_%s_kernel" % what if per_level else "ge1d_window_kernel[%s]" % what) + "<%s>" % cfg["dtype"]
+    if per_level:
+        gbs = 3.0 * es * glups
+        roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                "traffic": traffic_of("%s/%s" % (cfg["name"], kname)), "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * n}
+    else:
+        # blocked: HBM sees (2 u + 1 data) * sizeof(T) per node and launch of <= 16 levels; the kernel is bound by shared memory
+        lv = levels * args.steps / max(launches, 1)
+        gbs = 3.0 * es * glups / lv
+        roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                "traffic": None, "peak_source": srcp, "levels_per_launch": lv, "algorithmic_bytes_per_launch": 3.0 * es * n,
+                "note": "shared-memory bound (two 8-byte reads and one write per node update plus the data window), not HBM-bound: "
+                        "frac says how far from the HBM roof the blocked kernel runs", "effective_gbs": 2.0 * es * glups,
+                "effective_frac_of_hbm": 2.0 * es * glups / peaks["hbm_gbs"]}
     print(json.dumps({
-        "metric": METRIC, "value": upd / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "metric": METRIC, "value": glups, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
-        "config": {"workload": workload_desc(cfg) + ", source term + moving boundary values (NEXT-3)",
-                   "levels_per_step": levels, "kernel": "per_step"},
-        "gpu_launches": levels * args.steps, "finite": bool(torch.isfinite(u).all().item()),
-        "roofline": {"kernel": "ge1d_level_src_kernel<%s>" % cfg["dtype"], "bound": "hbm", "achieved": gbs,
-                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
-                     "traffic": traffic_of("%s/ge1d_level_src_kernel<%s>" % (cfg["name"], cfg["dtype"])),
-                     "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * cfg["nx"]},
-        "e2e": None, "cpu_baseline": None}), flush=True)
+        "config": {"workload": workload_desc(cfg) + (", variable diffusivity (NEXT-3)" if args.var else ", source term + moving boundary values (NEXT-3)"),
+                   "levels_per_step": levels, "kernel": "per_step" if per_level else "temporal"},
+        "gpu_launches": launches, "finite": bool(torch.isfinite(u).all().item()),
+        "roofline": roof, "e2e": None, "cpu_baseline": None}), flush=True)
     plan.close()
 
 
@@ -872,7 +902,8 @@ def main():
     ap.add_argument("--kform", type=int, default=-1, help="k >= 2 blocked kernel: 1 register-resident units, 0 shared-memory windows (-1 = plan default)")
     ap.add_argument("--form3d", type=int, default=-1, help="3-D: 1 streaming + shell kernels, 0 a thread per group (-1 = plan default)")
     ap.add_argument("--levels", type=int, default=0, help="override levels per step (experiments only)")
-    ap.add_argument("--src", action="store_true", help="measure ge_step_1d_src (source term + moving boundaries, NEXT-3)")
+    ap.add_argument("--src", action="store_true", help="measure ge_run_src (source term + moving boundaries, NEXT-3; --kernel per_step: ge_step_1d_src)")
+    ap.add_argument("--var", action="store_true", help="measure ge_run_var (variable diffusivity, NEXT-3; --kernel per_step: ge_step_1d_var)")
     ap.add_argument("--sweep", default="", choices=["", "sync"], help="sync: the synchronisation study on the C2-shaped rod (NEXT-2)")
     ap.add_argument("--sweep-n", type=int, default=2 ** 20, help="--sweep: nodes of the rod")
     ap.add_argument("--md", default="", help="--sweep: also write a markdown table to this file")
@@ -886,7 +917,7 @@ def main():
         sys.stderr.write("bench.py: warning: fewer than 3 warm-up steps; the number is not reportable\n")
     if args.sweep:
         run_sweep(args)
-    elif args.src:
+    elif args.src or args.var:
         run_src(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -120,20 +120,24 @@ int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f,
  * reading R-VAR; the paper's coefficient is constant): u_t = (a(x) u_x)_x in flux form.
  *   rl: device pointer, nx + 1 elements of dtype: rl[j] = tau * a(x_{j+1/2}) / h^2 > 0 for the link between nodes j
  *       and j+1, j = 0 .. N (the plan's own r is not used; the boundary values are the plan's).
- * Otherwise as ge_step_1d.  ge_run_var: `steps` such levels in place (one launch per level, result in u).
- * GE_EINVAL for batch > 1, dim != 1 or a null / misaligned pointer, GE_EUNSUPPORTED for group_k >= 2. */
+ * Otherwise as ge_step_1d (batch == 1).  ge_run_var: `steps` such levels in place, temporally blocked (16 levels per HBM
+ * round trip, the window and its link numbers resident in shared memory; ge_window.cuh), batched rods included: rl is
+ * then [batch][nx + 1].  GE_EINVAL for dim != 1 or a null / misaligned pointer (ge_step_1d_var: also batch > 1),
+ * GE_EUNSUPPORTED for group_k >= 2. */
 int ge_step_1d_var(ge_plan *p, const void *u_in, void *u_out, const void *rl, ge_stream_t stream);
 int ge_run_var(ge_plan *p, void *u, int64_t steps, const void *rl, ge_stream_t stream);
 
-/* `steps` >= 0 levels of ge_step_1d_src in place (same restrictions: one rod, group_k == 1; one launch per level,
- * ping-pong with the plan's scratch level, result in u, level += steps):
- *   tau_f:          device pointer or NULL.  f_level_stride == 0: one stationary source of nx elements used at
- *                   every level; f_level_stride >= nx: level n of the run reads tau_f + n * f_level_stride
- *                   (`steps` rows);
- *   bc_lo_t, bc_hi_t: HOST arrays of steps + 1 entries: the values of nodes 0 and N+1 at the run's levels
- *                   0 .. steps (entry n is the old-level value of step n and the new-level value of step n-1).
- * GE_EINVAL for batch > 1, dim != 1, a non-finite boundary value or 0 < f_level_stride < nx; GE_EUNSUPPORTED
- * for group_k >= 2.  Nothing is enqueued on an argument error. */
+/* `steps` >= 0 levels with a source term and moving boundary values in place (group_k == 1; result in u, level += steps):
+ *   tau_f:          device pointer or NULL.  f_level_stride == 0: ONE STATIONARY source, [batch][nx] elements, used at
+ *                   every level -- the run is temporally blocked (16 levels per HBM round trip, the source and the
+ *                   window resident in shared memory; ge_window.cuh), batched rods included (per-rod r);
+ *                   f_level_stride >= nx: level n of the run reads tau_f + n * f_level_stride (`steps` rows) -- one
+ *                   launch of ge_step_1d_src per level, batch must be 1;
+ *   bc_lo_t, bc_hi_t: HOST arrays, [batch][steps + 1] entries: the values of nodes 0 and N+1 of every rod at the run's
+ *                   levels 0 .. steps (entry n is the old-level value of step n and the new-level value of step n-1).
+ * GE_EINVAL for dim != 1, a non-finite boundary value, 0 < f_level_stride < nx or f_level_stride > 0 with batch > 1;
+ * GE_EUNSUPPORTED for group_k >= 2.  Nothing is enqueued on an argument error.  Synchronises `stream` once (the
+ * boundary values are staged through a host buffer of the call). */
 int ge_run_src(ge_plan *p, void *u, int64_t steps, const void *tau_f, int64_t f_level_stride,
                const double *bc_lo_t, const double *bc_hi_t, ge_stream_t stream);
 

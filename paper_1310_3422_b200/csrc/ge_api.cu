@@ -24,6 +24,7 @@
 #include "ge_probe.cuh"
 #include "ge_tail.cuh"
 #include "ge_level_var.cuh"
+#include "ge_window.cuh"
 
 namespace {
 
@@ -90,6 +91,9 @@ struct ge_plan {
     bool levelk_attr;         // function attributes of the k >= 2 kernel are set on this device
     bool rodk_attr;           // ... and of its shared-memory-resident form
     bool temporalk_attr;      // ... and of its temporally blocked form
+    bool win_attr;            // ... and of the window kernels (source term / variable diffusivity)
+    void* bc_dev;             // device: boundary values level by level of a ge_run_src call (grown on demand)
+    size_t bc_cap;
 };
 
 namespace {
@@ -643,6 +647,26 @@ bool resident_ok(const ge_plan* p, const void* u) {
     return p->res_path != 0 && ((uintptr_t)u % 16 == 0);
 }
 
+// ---- strategy B with non-constant data (ge_window.cuh): `levels` <= kWindowTb levels per launch ----
+constexpr int kWindowTb = 16;
+template <typename T, bool SRC, bool VAR>
+int launch_window(ge_plan* p, const void* uin, void* uout, const void* src, const void* rl, const void* bc, int64_t bc_lev,
+                  int64_t bc_stride, int levels, cudaStream_t s) {
+    const ge::WinGeom g = ge::win_geom(kWindowTb, p->nx);
+    if (g.valid <= 0 || levels < 1 || levels > kWindowTb) return GE_EINVAL;
+    auto* fn = ge::ge1d_window_kernel<T, SRC, VAR>;
+    GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ge::win_smem<T>()));
+    GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    dim3 grid((unsigned)g.tiles, (unsigned)(p->batch < 65535 ? p->batch : 65535));
+    fn<<<grid, ge::kWinThreads, ge::win_smem<T>(), s>>>((const T*)uin, (T*)uout, (const T*)src, (const T*)rl, (const T*)bc, bc_lev,
+                                                         bc_stride, p->nx, p->batch, (const ge::Coef1<T>*)p->coef, g,
+                                                         (int)(p->level & 1), levels);
+    GE_CUDA(cudaGetLastError());
+    p->launches += 1;
+    p->level += levels;
+    return GE_OK;
+}
+
 int step_common(ge_plan* p, int dim, const void* uin, void* uout, cudaStream_t s) {
     if (!p || !uin || !uout || uin == uout || p->dim != dim) return GE_EINVAL;
     const size_t es = elem_size(p->dtype);
@@ -809,38 +833,87 @@ int ge_step_1d_var(ge_plan* p, const void* u_in, void* u_out, const void* rl, ge
 }
 
 int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t stream) {
-    if (!p || !u || steps < 0 || !rl) return GE_EINVAL;
+    if (!p || !u || steps < 0 || !rl || p->dim != 1) return GE_EINVAL;
+    if (p->group_k != 1) return GE_EUNSUPPORTED;
+    const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)u % es || (uintptr_t)rl % es) return GE_EINVAL;
     NvtxRange nvtx("ge_run_var");
+    cudaStream_t s = (cudaStream_t)stream;
+    p->last_stream = s;
     void* cur = u;
     void* oth = p->scratch;
-    for (int64_t n = 0; n < steps; ++n) {
-        const int rc = ge_step_1d_var(p, cur, oth, rl, stream);
+    int64_t left = steps;
+    while (left > 0) {
+        // equal-sized blocks of at most kWindowTb levels, the link numbers resident in shared memory beside the window
+        const int64_t nl = (left + kWindowTb - 1) / kWindowTb;
+        const int lv = (int)((left + nl - 1) / nl);
+        const int rc = p->dtype == GE_F64 ? launch_window<double, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s)
+                                          : launch_window<float, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s);
         if (rc != GE_OK) return rc;
+        left -= lv;
         void* t = cur; cur = oth; oth = t;
     }
-    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * elem_size(p->dtype), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * es, cudaMemcpyDeviceToDevice, s));
     return GE_OK;
 }
 
 int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_level_stride, const double* bc_lo_t,
                const double* bc_hi_t, ge_stream_t stream) {
-    if (!p || !u || steps < 0 || !bc_lo_t || !bc_hi_t || f_level_stride < 0 || p->dim != 1 || p->batch != 1) return GE_EINVAL;
+    if (!p || !u || steps < 0 || !bc_lo_t || !bc_hi_t || f_level_stride < 0 || p->dim != 1) return GE_EINVAL;
     if (p->group_k != 1) return GE_EUNSUPPORTED;
-    if (tau_f && f_level_stride != 0 && f_level_stride < p->nx) return GE_EINVAL;
-    for (int64_t n = 0; n <= steps; ++n)
+    const bool per_level = tau_f && f_level_stride != 0;
+    if (per_level && (f_level_stride < p->nx || p->batch != 1)) return GE_EINVAL;
+    const int64_t nb = p->batch * (steps + 1);
+    for (int64_t n = 0; n < nb; ++n)
         if (!std::isfinite(bc_lo_t[n]) || !std::isfinite(bc_hi_t[n])) return GE_EINVAL;
-    NvtxRange nvtx("ge_run_src");
     const size_t es = elem_size(p->dtype);
+    if ((uintptr_t)u % es || (uintptr_t)tau_f % es) return GE_EINVAL;
+    NvtxRange nvtx("ge_run_src");
+    cudaStream_t s = (cudaStream_t)stream;
+    p->last_stream = s;
     void* cur = u;
     void* oth = p->scratch;
-    for (int64_t n = 0; n < steps; ++n) {
-        const double bc4[4] = {bc_lo_t[n], bc_lo_t[n + 1], bc_hi_t[n], bc_hi_t[n + 1]};
-        const void* f = tau_f ? (const char*)tau_f + (size_t)(n * f_level_stride) * es : nullptr;
-        const int rc = ge_step_1d_src(p, cur, oth, f, bc4, stream);
-        if (rc != GE_OK) return rc;
-        void* t = cur; cur = oth; oth = t;
+    if (per_level) {
+        // a different source array every level: one launch per level (ge_level_src.cuh)
+        for (int64_t n = 0; n < steps; ++n) {
+            const double bc4[4] = {bc_lo_t[n], bc_lo_t[n + 1], bc_hi_t[n], bc_hi_t[n + 1]};
+            const void* f = (const char*)tau_f + (size_t)(n * f_level_stride) * es;
+            const int rc = ge_step_1d_src(p, cur, oth, f, bc4, stream);
+            if (rc != GE_OK) return rc;
+            void* t = cur; cur = oth; oth = t;
+        }
+    } else if (steps > 0) {
+        // stationary source (or none): blocked -- the boundary values of all levels go to the device first
+        const size_t bytes = (size_t)nb * 2 * es;
+        if (p->bc_cap < bytes) {
+            GE_CUDA(cudaStreamSynchronize(s));                 // an earlier run may still read the old buffer
+            cudaFree(p->bc_dev); p->bc_dev = nullptr; p->bc_cap = 0;
+            GE_CUDA(cudaMalloc(&p->bc_dev, bytes));
+            p->bc_cap = bytes;
+        }
+        if (p->dtype == GE_F64) {
+            std::vector<double> h((size_t)nb * 2);
+            for (int64_t n = 0; n < nb; ++n) { h[2 * n] = bc_lo_t[n]; h[2 * n + 1] = bc_hi_t[n]; }
+            GE_CUDA(cudaMemcpyAsync(p->bc_dev, h.data(), bytes, cudaMemcpyHostToDevice, s));
+            GE_CUDA(cudaStreamSynchronize(s));                 // h is a stack-owned staging buffer
+        } else {
+            std::vector<float> h((size_t)nb * 2);
+            for (int64_t n = 0; n < nb; ++n) { h[2 * n] = (float)bc_lo_t[n]; h[2 * n + 1] = (float)bc_hi_t[n]; }
+            GE_CUDA(cudaMemcpyAsync(p->bc_dev, h.data(), bytes, cudaMemcpyHostToDevice, s));
+            GE_CUDA(cudaStreamSynchronize(s));
+        }
+        int64_t left = steps, done = 0;
+        while (left > 0) {
+            const int64_t nl = (left + kWindowTb - 1) / kWindowTb;
+            const int lv = (int)((left + nl - 1) / nl);
+            const int rc = p->dtype == GE_F64 ? launch_window<double, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s)
+                                              : launch_window<float, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s);
+            if (rc != GE_OK) return rc;
+            left -= lv; done += lv;
+            void* t = cur; cur = oth; oth = t;
+        }
     }
-    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * es, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    if (cur != u) GE_CUDA(cudaMemcpyAsync(u, cur, (size_t)p->count * es, cudaMemcpyDeviceToDevice, s));
     return GE_OK;
 }
 
@@ -1278,6 +1351,7 @@ int ge_plan_destroy(ge_plan* p) {
     cudaFree(p->hostpath);
     cudaFree(p->res_xbuf);
     cudaFree(p->res_flags);
+    cudaFree(p->bc_dev);
     if (p->aux3d) { cudaStreamSynchronize(p->aux3d); cudaStreamDestroy(p->aux3d); }
     if (p->ev3d[0]) cudaEventDestroy(p->ev3d[0]);
     if (p->ev3d[1]) cudaEventDestroy(p->ev3d[1]);

@@ -168,8 +168,8 @@ def ge_run_src(plan: int, u: int, steps: int, tau_f: int, f_level_stride: int, b
                bc_hi_t: Sequence[float], stream: int = 0):
     """bc_lo_t / bc_hi_t: steps + 1 boundary values (levels 0 .. steps of the run); tau_f = device pointer or 0."""
     lo, hi = _darr(bc_lo_t), _darr(bc_hi_t)
-    if len(lo) != steps + 1 or len(hi) != steps + 1:
-        raise GeError(GE_EINVAL, "ge_run_src (boundary arrays need steps + 1 values)")
+    if len(lo) != len(hi) or len(lo) < steps + 1 or len(lo) % (steps + 1):
+        raise GeError(GE_EINVAL, "ge_run_src (boundary arrays need batch * (steps + 1) values)")
     _check(load().ge_run_src(plan, u, steps, tau_f or None, f_level_stride, lo, hi, stream), "ge_run_src")
 
 

@@ -121,7 +121,9 @@ def test_run_src_matches_the_oracle_marched_level_by_level(oracle, dtype, n, ste
         plan.level = level0
         plan.run_src(u.data_ptr(), steps, d_src.data_ptr(), n if per_level else 0, walk[:, 0], walk[:, 1], s)
         torch.cuda.synchronize(dev)
-        assert plan.level == level0 + steps and plan.info()["launches"] == steps
+        assert plan.level == level0 + steps
+        # a source per level: one launch per level; a stationary source: 16 levels per launch (ge_window.cuh)
+        assert plan.info()["launches"] == (steps if per_level else -(-steps // 16))
     ref = cfg["u0"].reshape(-1).astype(np.float64)
     for i in range(steps):
         ref = oracle.level_1d_src(ref, float(cfg["r"][0]), (level0 + i) % 2, (walk[i, 0], walk[i, 1]),
@@ -143,3 +145,37 @@ def test_run_src_argument_errors():
             plan.run_src(u.data_ptr(), 1, 0, 0, (0, float("inf")), (0, 0))
         plan.run_src(u.data_ptr(), 0, 0, 0, (0.0,), (0.0,))
         assert plan.level == 0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("batch,n,steps,level0", [(1, 100000, 203, 0), (5, 4099, 77, 1), (3, 1980, 40, 0), (2, 7, 33, 1),
+                                                  (64, 4096, 50, 0)])
+def test_run_src_blocked_with_a_stationary_source(oracle, dtype, batch, n, steps, level0):
+    """ge_run_src with one stationary source array: temporally blocked (windows of the rods with their source values in
+    shared memory, 16 levels per launch), batched rods with per-rod r, boundary values that move every level and
+    differ from rod to rod; several windows per rod, ragged last window, odd and tiny N, both starting phases.
+    Against the oracle marched level by level."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    dt = _NP[dtype]
+    cfg = inputs.random_rods(batch, n, dtype, seed=n + steps)
+    rng = np.random.default_rng(n + batch)
+    src = rng.uniform(-0.1, 0.1, (batch, n)).astype(dt)
+    walk = (rng.uniform(-1, 1, (batch, 1, 2)) + 0.05 * np.cumsum(rng.uniform(-1, 1, (batch, steps + 1, 2)), axis=1)).astype(dt).astype(np.float64)
+    dev = torch.device("cuda:0")
+    u = torch.from_numpy(cfg["u0"].copy()).to(dev)
+    d_src = torch.from_numpy(src).to(dev)
+    s = torch.cuda.current_stream(dev).cuda_stream
+    with libge.Plan(cfg, stream=s) as plan:
+        plan.level = level0
+        plan.run_src(u.data_ptr(), steps, d_src.data_ptr(), 0, walk[:, :, 0].reshape(-1), walk[:, :, 1].reshape(-1), s)
+        torch.cuda.synchronize(dev)
+        assert plan.level == level0 + steps and plan.info()["launches"] == -(-steps // 16)
+    got = u.cpu().numpy().astype(np.float64)
+    for b in range(batch):
+        ref = cfg["u0"][b].astype(np.float64)
+        for i in range(steps):
+            ref = oracle.level_1d_src(ref, float(cfg["r"][b]), (level0 + i) % 2, (walk[b, i, 0], walk[b, i, 1]),
+                                      (walk[b, i + 1, 0], walk[b, i + 1, 1]), src[b].astype(np.float64))
+        scale = max(np.abs(ref).max(), np.abs(walk[b]).max())
+        assert np.abs(got[b] - ref).max() / scale <= TOL[dtype], (b, n, steps)

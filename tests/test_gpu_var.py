@@ -27,7 +27,8 @@ def _run(cfg, rl, steps, level0, via="run"):
                 plan.step_var(u.data_ptr(), v.data_ptr(), d_rl.data_ptr(), s)
                 u, v = v, u
         torch.cuda.synchronize(dev)
-        assert plan.level == level0 + steps and plan.info()["launches"] == steps
+        # ge_run_var is temporally blocked (16 levels per launch, ge_window.cuh), ge_step_1d_var one launch per level
+        assert plan.level == level0 + steps and plan.info()["launches"] == (-(-steps // 16) if via == "run" else steps)
     return u.cpu().numpy().astype(np.float64)
 
 
@@ -89,3 +90,42 @@ def test_var_argument_errors():
             plan.step_var(u.data_ptr(), u.data_ptr() + 8 * 64, 0)
         with pytest.raises(libge.GeError):
             plan.run_var(u.data_ptr(), -1, u.data_ptr() + 8 * 128)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("batch,n,steps,level0", [(1, 100000, 203, 0), (5, 4099, 77, 1), (3, 1980, 40, 0), (2, 7, 33, 1)])
+def test_run_var_blocked_and_batched(oracle, dtype, batch, n, steps, level0):
+    """ge_run_var: windows of the rods with their link numbers in shared memory, 16 levels per launch, batched rods each
+    with its own links and boundary values; several windows per rod, odd and tiny N.  Against the oracle, and against
+    the per-level kernel (same expressions: to rounding of the in-kernel division only -- identical here)."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    dt = _NP[dtype]
+    cfg = inputs.random_rods(batch, n, dtype, seed=n + steps)
+    rl = np.random.default_rng(n).uniform(0.5, 8.0, (batch, n + 1)).astype(dt)
+    dev = torch.device("cuda:0")
+    u = torch.from_numpy(cfg["u0"].copy()).to(dev)
+    d_rl = torch.from_numpy(rl).to(dev)
+    s = torch.cuda.current_stream(dev).cuda_stream
+    with libge.Plan(cfg, stream=s) as plan:
+        plan.level = level0
+        plan.run_var(u.data_ptr(), steps, d_rl.data_ptr(), s)
+        torch.cuda.synchronize(dev)
+        assert plan.info()["launches"] == -(-steps // 16)
+    got = u.cpu().numpy().astype(np.float64)
+    for b in range(batch):
+        ref = oracle.run_1d_var(cfg["u0"][b].astype(np.float64), rl[b].astype(np.float64), steps, cfg["bc_lo"][b],
+                                cfg["bc_hi"][b], level0=level0)
+        scale = max(np.abs(ref).max(), abs(cfg["bc_lo"][b]), abs(cfg["bc_hi"][b]))
+        assert np.abs(got[b] - ref).max() / scale <= TOL[dtype], (b, n, steps)
+    if batch == 1:
+        one = dict(cfg)
+        v = torch.from_numpy(cfg["u0"].reshape(-1).copy()).to(dev)
+        w = torch.empty_like(v)
+        with libge.Plan(one, stream=s) as plan:
+            plan.level = level0
+            for _ in range(steps):
+                plan.step_var(v.data_ptr(), w.data_ptr(), d_rl.data_ptr(), s)
+                v, w = w, v
+            torch.cuda.synchronize(dev)
+        np.testing.assert_array_equal(v.cpu().numpy(), u.cpu().numpy().reshape(-1))
