@@ -8,11 +8,11 @@ cudaError_t level3d_dispatch(int dtype, int form, const void* uin, void* uout, i
                              const void* coef, int phase, int sm_count, cudaStream_t s, int* launches, cudaStream_t aux, cudaEvent_t ev_in,
                              cudaEvent_t ev_out) {
     const bool stream = form == 1;
-    *launches = stream ? 2 : 1;
+    if (!stream) *launches = 1;
     if (dtype == 1)
-        return stream ? stream3d_launch<double>((const double*)uin, (double*)uout, nx, ny, nz, (const Coef3<double>*)coef, phase, sm_count, s, aux, ev_in, ev_out)
+        return stream ? stream3d_launch<double>((const double*)uin, (double*)uout, nx, ny, nz, (const Coef3<double>*)coef, phase, sm_count, s, launches, aux, ev_in, ev_out)
                       : level3d_launch<double>((const double*)uin, (double*)uout, nx, ny, nz, (const Coef3<double>*)coef, phase, s);
-    return stream ? stream3d_launch<float>((const float*)uin, (float*)uout, nx, ny, nz, (const Coef3<float>*)coef, phase, sm_count, s, aux, ev_in, ev_out)
+    return stream ? stream3d_launch<float>((const float*)uin, (float*)uout, nx, ny, nz, (const Coef3<float>*)coef, phase, sm_count, s, launches, aux, ev_in, ev_out)
                   : level3d_launch<float>((const float*)uin, (float*)uout, nx, ny, nz, (const Coef3<float>*)coef, phase, s);
 }
 
