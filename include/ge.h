@@ -221,6 +221,33 @@ int ge_fma_probe(int32_t dtype, int64_t iters, void *sink, double *flops, ge_str
  * arithmetic of the kernels looks like to the register file.  GE_EINVAL for any other variant. */
 int ge_fma_probe_ex(int32_t dtype, int32_t variant, int64_t iters, void *sink, double *flops, ge_stream_t stream);
 
+/* ---- an entry point that allocates NOTHING (for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it; a ge_plan allocates its coefficient block and the second
+ * copy of the state) ----
+ * ge_run_1d_static: `steps` levels of the 1-D scheme with two-point groups (strategy A,
+ * ge1d_level_kernel, the arithmetic of ge_run on a plan with kernel = per_step, bit for bit), one rod, from level
+ * `level0` (phase = level & 1), Dirichlet values bc_lo / bc_hi, r = tau/h^2.
+ *   u_in, u_out: DEVICE pointers to nx elements of `dtype` (ge_dtype), aligned to the element size, owned by the
+ *     caller, not overlapping; u_in is only read.  steps = 0 copies u_in to u_out.
+ *   The second copy of the state and the coefficient block live in a file-scope device array of
+ *   GE_STATIC_MAX_BYTES + 256 bytes that EVERY GPU which loads the library holds until the process exits.
+ *   nx * sizeof(element) > GE_STATIC_MAX_BYTES (nx > 524288 in f64, 1048576 in f32) is rejected with GE_EINVAL and
+ *   nothing is enqueued; ge_static_error gives the text.
+ *   All calls share that array and find the previous call's contents in it (nothing in it needs to start at zero:
+ *   every call rewrites what it reads).  Calls that OVERLAP on the GPU -- two streams, two host threads -- race;
+ *   order them on one stream or with events.
+ *   No cudaMalloc / cudaFree / allocating routine is called; the only set-up is one cudaGetSymbolAddress per
+ *   device, at the first call on that device (ge_static_limit does it too: call it ahead of a capture).
+ *   Enqueues 1 + steps launches on `stream` and returns without synchronising.
+ * ge_static_limit: *max_nodes = the largest nx ge_run_1d_static takes for `dtype` (and the per-device set-up).
+ * ge_static_error: copies the calling thread's last ge_run_1d_static / ge_static_limit message ("ok" after a
+ *   success) into buf[cap], NUL-terminated; GE_EINVAL for a null buf or cap < 1. */
+#define GE_STATIC_MAX_BYTES (4 * 1024 * 1024)
+int ge_run_1d_static(int32_t dtype, const void *u_in, void *u_out, int64_t nx, int64_t steps, int64_t level0,
+                     double r, double bc_lo, double bc_hi, ge_stream_t stream);
+int ge_static_limit(int32_t dtype, int64_t *max_nodes);
+int ge_static_error(char *buf, int64_t cap);
+
 /* Frees the plan's device buffers (stream-ordered on the stream last used) and the plan. */
 int ge_plan_destroy(ge_plan *p);
 

@@ -35,7 +35,7 @@ _DTYPES = {"f32": GE_F32, "f64": GE_F64}
 # every symbol include/ge.h declares
 EXPORTS = ("ge_plan_create", "ge_step_1d", "ge_step_1d_src", "ge_run_src", "ge_step_1d_var", "ge_run_var", "ge_step_2d", "ge_step_3d", "ge_run", "ge_run_host",
            "ge_plan_get_level", "ge_plan_set_level", "ge_plan_info", "ge_plan_tune", "ge_plan_destroy",
-           "ge_fma_probe", "ge_fma_probe_ex", "ge_strerror", "ge_version")
+           "ge_fma_probe", "ge_fma_probe_ex", "ge_run_1d_static", "ge_static_limit", "ge_static_error", "ge_strerror", "ge_version")
 
 
 class ge_desc(ctypes.Structure):
@@ -91,6 +91,9 @@ def load() -> ctypes.CDLL:
     lib.ge_plan_destroy.argtypes = [vp]
     lib.ge_fma_probe.argtypes = [i32, i64, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.ge_fma_probe_ex.argtypes = [i32, i32, i64, vp, ctypes.POINTER(ctypes.c_double), vp]
+    lib.ge_run_1d_static.argtypes = [i32, vp, vp, i64, i64, i64, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp]
+    lib.ge_static_limit.argtypes = [i32, ctypes.POINTER(i64)]
+    lib.ge_static_error.argtypes = [ctypes.c_char_p, i64]
     lib.ge_strerror.argtypes = [ctypes.c_int]
     lib.ge_strerror.restype = ctypes.c_char_p
     lib.ge_version.argtypes = []
@@ -213,6 +216,34 @@ def ge_fma_probe(dtype, iters: int, sink: int, stream: int = 0, variant: int = 0
     _check(load().ge_fma_probe_ex(_DTYPES[dtype] if isinstance(dtype, str) else int(dtype), variant, iters, sink,
                                   ctypes.byref(v), stream), "ge_fma_probe_ex")
     return v.value
+
+
+GE_STATIC_MAX_BYTES = 4 * 1024 * 1024
+
+
+def ge_static_error() -> str:
+    buf = ctypes.create_string_buffer(320)
+    load().ge_static_error(buf, len(buf))
+    return buf.value.decode()
+
+
+def ge_static_limit(dtype) -> int:
+    """Largest nx ge_run_1d_static takes for `dtype` (also does the per-device set-up)."""
+    v = ctypes.c_int64()
+    rc = load().ge_static_limit(_DTYPES[dtype] if isinstance(dtype, str) else int(dtype), ctypes.byref(v))
+    if rc != GE_OK:
+        raise GeError(rc, "ge_static_limit: " + ge_static_error())
+    return v.value
+
+
+def ge_run_1d_static(dtype, u_in: int, u_out: int, nx: int, steps: int, r: float, bc_lo: float = 0.0,
+                     bc_hi: float = 0.0, level0: int = 0, stream: int = 0):
+    """`steps` levels of the 1-D two-point-group scheme from u_in to u_out (device pointers) without any
+    allocation: the scratch is a fixed array inside libge.so (include/ge.h)."""
+    rc = load().ge_run_1d_static(_DTYPES[dtype] if isinstance(dtype, str) else int(dtype), u_in, u_out, nx, steps,
+                                 level0, float(r), float(bc_lo), float(bc_hi), stream)
+    if rc != GE_OK:
+        raise GeError(rc, "ge_run_1d_static: " + ge_static_error())
 
 
 def ge_plan_destroy(plan: Optional[int]):
