@@ -122,6 +122,9 @@ int upload_coef(ge_plan* p, const ge_desc* d, cudaStream_t s) {
         h.c1 = (T)(2.0 * r / (1.0 + 2.0 * r) / 8.0);
         h.c2 = (T)(4.0 * r / (1.0 + 4.0 * r) / 8.0);
         h.c3 = (T)(6.0 * r / (1.0 + 6.0 * r) / 8.0);
+        h.q1 = (T)(r / (1.0 + r) / 4.0);
+        h.q2 = (T)(3.0 * r / (1.0 + 3.0 * r) / 4.0);
+        h.q3 = (T)(5.0 * r / (1.0 + 5.0 * r) / 4.0);
         for (int ax = 0; ax < 3; ++ax) { h.lo[ax] = (T)d->bc_lo[ax]; h.hi[ax] = (T)d->bc_hi[ax]; }
         GE_CUDA(cudaMalloc(&p->coef, sizeof(h)));
         GE_CUDA(cudaMemcpyAsync(p->coef, &h, sizeof(h), cudaMemcpyHostToDevice, s));
@@ -316,7 +319,9 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
         const int form = p->form3d && p->nx >= 8 && p->ny >= 8 && p->nz >= 8 ? 1 : 0;
         int n = 0;
         if (form == 1 && !p->aux3d) {        // side stream of the shell kernel (lazy; a failure just keeps everything on s)
-            if (cudaStreamCreateWithFlags(&p->aux3d, cudaStreamNonBlocking) != cudaSuccess ||
+            int prio_least = 0, prio_greatest = 0;           // GE_S3D_MODE 2: the side stream carries the streaming kernel, ahead of the shell
+            cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
+            if (cudaStreamCreateWithPriority(&p->aux3d, cudaStreamNonBlocking, GE_S3D_MODE == 2 ? prio_greatest : prio_least) != cudaSuccess ||
                 cudaEventCreateWithFlags(&p->ev3d[0], cudaEventDisableTiming) != cudaSuccess ||
                 cudaEventCreateWithFlags(&p->ev3d[1], cudaEventDisableTiming) != cudaSuccess) {
                 cudaGetLastError();

@@ -48,7 +48,8 @@ struct Coef3 {
     T r;
     T c1, c2, c3;          // 2r/(1+2r)/8, 4r/(1+4r)/8, 6r/(1+6r)/8
     T lo[3], hi[3];        // face values: x, y, z
-    T pad[6];
+    T q1, q2, q3;          // group cut by ONE face (4 members): r/(1+r)/4, 3r/(1+3r)/4, 5r/(1+5r)/4
+    T pad[3];
 };
 
 template <typename T> struct VecOf;

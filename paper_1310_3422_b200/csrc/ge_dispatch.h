@@ -4,6 +4,11 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// 3-D: which of the two kernels of a level goes first and on which stream (ge_stream3d.cuh stream3d_launch)
+#ifndef GE_S3D_MODE
+#define GE_S3D_MODE 0
+#endif
+
 namespace ge {
 
 // 2-D strip kernels (ge_strip2d.cu).  dtype: 0 = f32, 1 = f64 (ge_dtype).  coop: 0 = a warp per strip

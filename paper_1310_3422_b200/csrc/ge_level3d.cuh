@@ -84,6 +84,44 @@ __device__ __forceinline__ void truncated_group3d(const T (&R)[8], const bool (&
     for (int d = 0; d < 8; ++d) nw[d] = idx[d] >= 0 ? b[idx[d]] : T(0);
 }
 
+// Group cut by exactly ONE face: its four interior members form a 2x2 square in the face's plane,
+//   (1+3r) x_P - r (x_P' + x_P'') = R_P + r beta     (P', P'' the in-square partners, beta the face value),
+// solved in the Walsh basis of the square like the full group: eigenvalues 1+r, 1+3r (twice), 1+5r,
+// x = b - WHT(q . WHT(b)), q = (1 - 1/lambda)/4.  Members ordered j = d_a + 2 d_b, a < b the in-face axes.
+// (ge3d_stream_kernel computes the x-cut groups of its rows with the same function: bit-identical.)
+template <typename T>
+__device__ __forceinline__ void cut4_solve(const T (&R)[4], T r, T beta, T q1, T q2, T q3, T (&x)[4]) {
+    T b[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = fma(r, beta, R[j]);
+    const T s0 = b[0] + b[1], s1 = b[0] - b[1], s2 = b[2] + b[3], s3 = b[2] - b[3];
+    const T w0 = (s0 + s2) * q1, w1 = (s1 + s3) * q2, w2 = (s0 - s2) * q2, w3 = (s1 - s3) * q3;
+    const T t0 = w0 + w1, t1 = w0 - w1, t2 = w2 + w3, t3 = w2 - w3;
+    x[0] = b[0] - (t0 + t2);
+    x[1] = b[1] - (t1 + t3);
+    x[2] = b[2] - (t0 - t2);
+    x[3] = b[3] - (t1 - t3);
+}
+
+// the group is cut by the low (the member outside is its first) or high face of axis AX: constant indices only
+template <typename T, int AX>
+__device__ __forceinline__ void cut4_group3d(const T (&R)[8], bool low, const Coef3<T>& k, T (&nw)[8]) {
+    constexpr int A = AX == 0 ? 1 : 0, B = AX == 2 ? 1 : 2;
+    T R4[4], x4[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int rest = ((j & 1) << A) | ((j >> 1) << B);
+        R4[j] = low ? R[rest | (1 << AX)] : R[rest];
+    }
+    cut4_solve<T>(R4, k.r, low ? k.lo[AX] : k.hi[AX], k.q1, k.q2, k.q3, x4);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int rest = ((j & 1) << A) | ((j >> 1) << B);
+        nw[rest | (1 << AX)] = low ? x4[j] : T(0);
+        nw[rest] = low ? T(0) : x4[j];
+    }
+}
+
 // one group, anchored at element (g0, g1, g2)
 template <typename T, int PH>
 __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict__ uout, int nx, int ny, int nz,
@@ -153,7 +191,14 @@ __device__ __forceinline__ void group3d(const T* __restrict__ uin, T* __restrict
 #pragma unroll
         for (int d = 0; d < 8; ++d) nw[d] = R[d] - W[d];
     } else {
-        truncated_group3d<T>(R, in, k, nw);
+        const bool c0 = !(g0 >= 0 && g0 + 1 < nx), c1 = !(g1 >= 0 && g1 + 1 < ny), c2 = !(g2 >= 0 && g2 + 1 < nz);
+        if ((int)c0 + (int)c1 + (int)c2 == 1) {
+            if (c0)      cut4_group3d<T, 0>(R, g0 < 0, k, nw);
+            else if (c1) cut4_group3d<T, 1>(R, g1 < 0, k, nw);
+            else         cut4_group3d<T, 2>(R, g2 < 0, k, nw);
+        } else {
+            truncated_group3d<T>(R, in, k, nw);
+        }
     }
     if (full) {
         T* __restrict__ ob = uout + ((int64_t)g2 * ny + g1) * nx + g0;

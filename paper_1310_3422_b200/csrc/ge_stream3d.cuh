@@ -40,6 +40,9 @@ constexpr int kS3Unroll = GE_S3D_UNROLL;
 #ifndef GE_S3D_WX
 #define GE_S3D_WX 1
 #endif
+#ifndef GE_S3D_MODE
+#define GE_S3D_MODE 0
+#endif
 constexpr int kS3Wx = GE_S3D_WX;          // warps of a CTA side by side in x (a CTA then reads kS3Wx * 64 consecutive nodes of a row)
 constexpr int kS3Wy = GE_S3D_WY;          // ... and stacked in y (their halo rows are each other's own rows)
 constexpr int kS3Warps = kS3Wx * kS3Wy;
@@ -173,6 +176,20 @@ __device__ __forceinline__ void s3_read_pair(const T* __restrict__ slot, const T
     }
 }
 
+// a lane's piece, 16-byte stores (E * sizeof(T) is a multiple of 16)
+template <typename T, int E>
+__device__ __forceinline__ void s3_store_piece(T* __restrict__ p, const T (&v)[E]) {
+    constexpr int V = VecOf<T>::V;
+    static_assert(E % V == 0, "piece of 16-byte vectors");
+#pragma unroll
+    for (int c = 0; c < E / V; ++c) {
+        T t[V];
+#pragma unroll
+        for (int e = 0; e < V; ++e) t[e] = v[c * V + e];
+        st_vec(p + c * V, t);
+    }
+}
+
 // v[e] <- the value one node to the left: the left lane's v[E-1] at e = 0 (lane 0: `edge`)
 template <typename T, int E>
 __device__ __forceinline__ void s3_shift(const T (&v)[E], T edge, int lane, T (&out)[E]) {
@@ -225,6 +242,10 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 #pragma unroll
     for (int g = 0; g <= NG; ++g) deep[g] = xg + 2 * g >= 0 && xg + 2 * g + 1 < nx;
     const bool xlo = xg - 1 < 0, xhi = xg + E >= nx;
+    // shifted form: the groups cut by the x faces are computed here as well (cut4_solve of ge_level3d.cuh) -- low:
+    // group (-1, 0), the first group of the lane at x0 = 0; high: group (nx-1, nx), computed by the lane that holds
+    // node nx-1 from its unshifted values
+    const bool cut_lo = SHIFT && x0 == 0, cut_hi = SHIFT && x0 == nx - E;
     const int64_t ro[4] = {(int64_t)(ylo ? 0 : y0 - 1) * sy, (int64_t)y0 * sy, (int64_t)(y0 + 1) * sy,
                            (int64_t)(yhi ? ny - 1 : y0 + 2) * sy};
     const bool edge_lane = SHIFT ? lane == 0 : (lane == 0 || lane == 31);
@@ -240,6 +261,7 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 
     // pair k0 and the upper plane of the pair below it go through the ring as well (slot 0, then it is free)
     T prevU[2][E];                    // rows y, y+1 of the plane below the pair (shifted form: of the nodes xg ..)
+    T prevLast[2];                    // ... of the lane's last node x0+E-1 (shifted form, for the high cut group)
     S3Pair<T, E> cur;
     s3_request_pair<T, E, VEC, SHIFT>(uin, sz, ro, xc, 2 * k0 - PH - 2, nz, ring, ering, stride, lane, xe_col);
     s3_commit();
@@ -252,9 +274,11 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 #pragma unroll
             for (int e = 0; e < E; ++e) prevU[rr][e] = cur.own[1][rr][e];
         }
+        prevLast[rr] = cur.own[1][rr][E - 1];
         if (2 * k0 - PH - 1 < 0) {
 #pragma unroll
             for (int e = 0; e < E; ++e) prevU[rr][e] = lo2;
+            prevLast[rr] = lo2;
         }
     }
     s3_request_pair<T, E, VEC, SHIFT>(uin, sz, ro, xc, 2 * k0 - PH, nz, ring, ering, stride, lane, xe_col);
@@ -283,10 +307,13 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
         // the values the groups are computed from, for the nodes xg .. xg+E-1:
         T O[2][2][E], H[2][2][E], NL[2][E];      // pair, rows y-1 / y+2 of its planes, rows y, y+1 of the plane above
         T lf[2][2], rt[2][2];                    // columns xg-1 and xg+E of the pair's four rows
+        T nlast[2];                              // rows y, y+1 of the plane above at the lane's last node
         {
             T nlow[2][E];
             s3_read_piece<T, E>(nslot + 0 * stride, nlow[0]);
             s3_read_piece<T, E>(nslot + 1 * stride, nlow[1]);
+            nlast[0] = z0 + 2 >= nz ? hi2 : nlow[0][E - 1];
+            nlast[1] = z0 + 2 >= nz ? hi2 : nlow[1][E - 1];
             if constexpr (SHIFT) {
                 T ne[2] = {T(0), T(0)};
                 if (lane == 0) { ne[0] = neslot[1]; ne[1] = neslot[3]; }
@@ -361,13 +388,38 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
             wht8(W);
 #pragma unroll
             for (int d = 0; d < 8; ++d) nw[(d >> 2) & 1][(d >> 1) & 1][2 * g + (d & 1)] = R[d] - W[d];
+            if constexpr (SHIFT) {
+                if (g == 0 && cut_lo) {              // group (-1, 0): its members dx = 1 are node 0
+                    T R4[4], x4[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) R4[j] = R[1 + 2 * j];
+                    cut4_solve<T>(R4, r, lo0, coef->q1, coef->q2, coef->q3, x4);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) nw[j >> 1][j & 1][1] = x4[j];
+                }
+            }
+        }
+        T hi_new[4] = {T(0), T(0), T(0), T(0)};      // new values of node nx-1, j = dy + 2 dz (shifted form, cut_hi)
+        if constexpr (SHIFT) {
+            if (cut_hi) {                            // group (nx-1, nx): its members dx = 0 are node nx-1 = the lane's last
+                T R4[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int dy = j & 1, dz = j >> 1;
+                    const T o = cur.own[dz][dy][E - 1], ox = cur.own[dz][dy][E - 2];
+                    const T oy = dy ? (yhi ? hi1 : cur.halo[dz][1][E - 1]) : (ylo ? lo1 : cur.halo[dz][0][E - 1]);
+                    const T oz = dz ? nlast[dy] : prevLast[dy];
+                    R4[j] = fma(r, ((ox - o) + (oy - o)) + (oz - o), o);
+                }
+                cut4_solve<T>(R4, r, hi0, coef->q1, coef->q2, coef->q3, hi_new);
+            }
         }
         T* __restrict__ ob = uout + (int64_t)z0 * sz + ro[1] + x0;   // the lane's aligned piece (VEC)
         if constexpr (SHIFT) {
-            // out[e] = node x0 + e = nw[e + 1]; the last one is the right lane's nw[0]
-            bool all = lane != 31;
-#pragma unroll
-            for (int g = 0; g <= NG; ++g) all = all && deep[g];
+            // out[e] = node x0 + e = nw[e + 1]; the last one is the right lane's nw[0] (the next warp's lane 0 stores
+            // it itself), or the high cut group's
+            const bool in_row = x0 <= nx - E;
+            const bool has_last = cut_hi || (lane != 31 && x0 < nx - E);
 #pragma unroll
             for (int dz = 0; dz < 2; ++dz)
 #pragma unroll
@@ -376,15 +428,17 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
 #pragma unroll
                     for (int e = 0; e + 1 < E; ++e) out[e] = nw[dz][dy][e + 1];
                     out[E - 1] = __shfl_down_sync(FULL, nw[dz][dy][0], 1);
+                    if (cut_hi) out[E - 1] = hi_new[dy + 2 * dz];
                     T* __restrict__ o2 = ob + dz * sz + dy * sy;
-                    if (E * sizeof(T) == 16 && all) {
-                        if constexpr (E * sizeof(T) == 16) st_vec(o2, out);
-                    } else {
+                    if (in_row) {
+                        if (has_last) {
+                            s3_store_piece<T, E>(o2, out);
+                        } else {
 #pragma unroll
-                        for (int e = 0; e < E; ++e)
-                            if (deep[(e + 1) / 2] && (e + 1 < E || lane != 31)) o2[e] = out[e];
+                            for (int e = 0; e + 1 < E; ++e) o2[e] = out[e];
+                        }
+                        if (lane == 0 && x0 > 0) o2[-1] = nw[dz][dy][0];
                     }
-                    if (lane == 0 && deep[0]) o2[-1] = nw[dz][dy][0];
                 }
         } else {
             bool all = VEC, stored = false;
@@ -418,9 +472,11 @@ ge3d_stream_kernel(const T* __restrict__ uin, T* __restrict__ uout, int nx, int 
         }
         // slide up by one pair: the upper plane becomes the plane below, pair k+1 comes out of its ring slot
 #pragma unroll
-        for (int rr = 0; rr < 2; ++rr)
+        for (int rr = 0; rr < 2; ++rr) {
 #pragma unroll
             for (int e = 0; e < E; ++e) prevU[rr][e] = O[1][rr][e];
+            prevLast[rr] = cur.own[1][rr][E - 1];
+        }
         s3_read_pair<T, E, SHIFT>(nslot, neslot, stride, edge_lane, cur);
         rslot = rslot + 1 == RING ? 0 : rslot + 1;
     }
@@ -476,34 +532,40 @@ inline cudaError_t stream3d_launch(const T* uin, T* uout, int64_t nx, int64_t ny
     // faces with cut groups (anchor -1, or anchor n-1): the shell kernel's
     unsigned faces = 0; int nfaces = 0;
     const int64_t nn[3] = {nx, ny, nz};
+    constexpr int kE = 2 * S3Cfg<T>::ng;
+    const bool vec = nx % kE == 0 && (((uintptr_t)uin | (uintptr_t)uout) % (kE * sizeof(T))) == 0;
+    const bool have_main = gx > 0 && gy > 0 && gz > 0;
+    // the shifted form (vec, phase 1) computes the groups cut by the x faces itself; those cut by another face
+    // as well are on that face's list
+    const bool x_in_main = have_main && vec && phase == 1;
     for (int a = 0; a < 3; ++a) {
+        if (a == 0 && x_in_main) continue;
         if (phase == 1) { faces |= (unsigned)(2 * a) << (3 * nfaces); ++nfaces; }
         if (2 * last(nn[a]) - phase + 1 >= nn[a]) { faces |= (unsigned)(2 * a + 1) << (3 * nfaces); ++nfaces; }
     }
     auto groups = [&](int64_t n) { return last(n) + 1; };
     const int64_t ax = groups(nx), ay = groups(ny), az = groups(nz);
     const int64_t gmax = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
-    cudaError_t e = cudaSuccess;
-    // shell first (it is small and latency-bound: it starts on part of the chip, the streaming kernel fills the rest)
+    // The shell kernel is small and latency-bound; it runs beside the streaming kernel on another stream (both read the
+    // old level and write disjoint parts of the new one).  GE_S3D_MODE 0: shell first on `aux`, the streaming kernel
+    // on `s` fills the rest of the chip; 1: the streaming kernel first on `s`, the shell after it on `aux`; 2: the
+    // streaming kernel on `aux` (a high-priority stream: its CTAs go first), the shell on `s`.
     const bool side = aux && ev_in && ev_out && nfaces > 0;
-    cudaStream_t ss = side ? aux : s;
-    if (side) {
-        e = cudaEventRecord(ev_in, s);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux, ev_in, 0);
-        if (e != cudaSuccess) return e;
-    }
-    if (nfaces > 0) {
+    constexpr int kMode = GE_S3D_MODE;
+    cudaStream_t s_shell = side ? (kMode == 2 ? s : aux) : s;
+    cudaStream_t s_main = side && kMode == 2 ? aux : s;
+    auto launch_shell = [&]() -> cudaError_t {
+        if (nfaces == 0) return cudaSuccess;
         dim3 sblock(32, 4), sgrid((unsigned)((gmax + 31) / 32), (unsigned)((gmax + 3) / 4), (unsigned)nfaces);
 #ifndef GE_S3D_NOSHELL
-        if (phase == 0) ge3d_shell_kernel<T, 0><<<sgrid, sblock, 0, ss>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, faces);
-        else            ge3d_shell_kernel<T, 1><<<sgrid, sblock, 0, ss>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, faces);
+        if (phase == 0) ge3d_shell_kernel<T, 0><<<sgrid, sblock, 0, s_shell>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, faces);
+        else            ge3d_shell_kernel<T, 1><<<sgrid, sblock, 0, s_shell>>>(uin, uout, (int)nx, (int)ny, (int)nz, coef, faces);
 #endif
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
         *launches += 1;
-    }
-    if (side) { e = cudaEventRecord(ev_out, aux); if (e != cudaSuccess) return e; }
-    if (gx > 0 && gy > 0 && gz > 0) {
+        return cudaGetLastError();
+    };
+    auto launch_main = [&]() -> cudaError_t {
+        if (!have_main) return cudaSuccess;
         // z segments: enough CTAs for ~8 resident CTAs on every SM, at least 8 pairs per segment
         // lanes start at group column 0 and hold NG group columns each; the last deep group column is index gx
         const int64_t per_cta = 32 * kS3Wx * S3Cfg<T>::ng;
@@ -518,16 +580,30 @@ inline cudaError_t stream3d_launch(const T* uin, T* uout, int64_t nx, int64_t ny
         if (segs < 1) segs = 1;
         const int kseg = (int)((gz + segs - 1) / segs);
         dim3 grid((unsigned)bx, (unsigned)((gy + kS3Wy - 1) / kS3Wy), (unsigned)((gz + kseg - 1) / kseg));
-        constexpr int E = 2 * S3Cfg<T>::ng;
-        const bool vec = nx % E == 0 && (((uintptr_t)uin | (uintptr_t)uout) % (E * sizeof(T))) == 0;
-        if (phase == 0) e = vec ? stream3d_launch_one<T, 0, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s)
-                                : stream3d_launch_one<T, 0, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s);
-        else            e = vec ? stream3d_launch_one<T, 1, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s)
-                                : stream3d_launch_one<T, 1, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s);
-        if (e != cudaSuccess) return e;
         *launches += 1;
+        if (phase == 0) return vec ? stream3d_launch_one<T, 0, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s_main)
+                                   : stream3d_launch_one<T, 0, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s_main);
+        return vec ? stream3d_launch_one<T, 1, true>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s_main)
+                   : stream3d_launch_one<T, 1, false>(uin, uout, (int)nx, (int)ny, (int)nz, coef, kseg, grid, s_main);
+    };
+    cudaError_t e = cudaSuccess;
+    if (side) {
+        e = cudaEventRecord(ev_in, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux, ev_in, 0);
+        if (e != cudaSuccess) return e;
     }
-    if (side) e = cudaStreamWaitEvent(s, ev_out, 0);
+    if (kMode == 0) {
+        e = launch_shell();
+        if (e == cudaSuccess) e = launch_main();
+    } else {
+        e = launch_main();
+        if (e == cudaSuccess) e = launch_shell();
+    }
+    if (e != cudaSuccess) return e;
+    if (side) {
+        e = cudaEventRecord(ev_out, aux);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ev_out, 0);
+    }
     return e;
 }
 
