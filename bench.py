@@ -20,7 +20,8 @@ Beside the contract's keys the default line carries: `alu_peaks` (FFMA / DFMA th
 run by libge's ge_fma_probe, the denominator of every "bound": "alu" roofline), `parity` (sampled
 dependency cones of a run from the config's initial state against the oracle), `cpu_baseline` with a
 one-thread and an all-cores leg on ONE sample (the same one --impl reference times), `secondary` (C5 f32,
-C5 f64, C2, C3 device-resident, so that the 2-D half of the north_star target is in the driver's record),
+C5 f64, C2, C3 and the 3-D boxes device-resident, so that the 2-D half of the north_star target and the 3-D
+row are in the driver's record),
 and the PCIe ceiling beside `e2e`.  `--sweep sync` is the synchronisation study.
 """
 from __future__ import annotations
@@ -356,6 +357,20 @@ def _window_2d(oracle, u0, r, steps, bc, x0, y0, w):
     return out[y0 - ay:y0 - ay + w, x0 - ax:x0 - ax + w]
 
 
+def _window_3d(oracle, u0, r, steps, bc, x0, y0, z0, w):
+    nz, ny, nx = u0.shape
+    halo = 2 * steps + 4
+    lo = [max(0, v - halo) for v in (x0, y0, z0)]
+    lo = [v - v % 2 for v in lo]
+    hi = [min(n, v + w + halo) for n, v in zip((nx, ny, nz), (x0, y0, z0))]
+    fake = (0.1, -0.2, 0.3, -0.4, 0.5, -0.6)          # a cut face of the sub-box: any value, the cone keeps it out
+    sbc = []
+    for a, n in enumerate((nx, ny, nz)):
+        sbc += [bc[2 * a] if lo[a] == 0 else fake[2 * a], bc[2 * a + 1] if hi[a] == n else fake[2 * a + 1]]
+    out = oracle.run_3d(u0[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].astype(np.float64), r, steps, tuple(sbc))
+    return out[z0 - lo[2]:z0 - lo[2] + w, y0 - lo[1]:y0 - lo[1] + w, x0 - lo[0]:x0 - lo[0] + w]
+
+
 def parity_check(cfg, plan, dev, stream, k=1, budget=4e8):
     """A run from the config's initial state in the timed launch configuration, compared with the oracle on
     sampled dependency cones (rods: whole sampled rods).  Where the cones of the full level count would cost
@@ -363,12 +378,15 @@ def parity_check(cfg, plan, dev, stream, k=1, budget=4e8):
     with fewer levels -- the full-length comparison is tests/test_gpu_longrun.py's."""
     import torch
     from oracle import ge_oracle
-    if cfg["dim"] == 3 or k != 1:
+    if k != 1:
         return None
     ge_oracle.build()
     tol = 1e-12 if cfg["dtype"] == "f64" else 1e-5
     levels = cfg["steps"]
-    if cfg["dim"] == 2:
+    if cfg["dim"] == 3:
+        while (16 + 4 * levels + 8) ** 3 * levels > budget / 20 and levels > 4:    # the 3-D oracle eliminates every group
+            levels //= 2
+    elif cfg["dim"] == 2:
         while (24 + 4 * levels + 8) ** 2 * levels > budget and levels > 8:
             levels //= 2
     elif cfg["dim"] == 1 and cfg["batch"] == 1:
@@ -382,7 +400,19 @@ def parity_check(cfg, plan, dev, stream, k=1, budget=4e8):
     del u
     rng = np.random.default_rng(12345)
     worst, what = 0.0, ""
-    if cfg["dim"] == 2:
+    if cfg["dim"] == 3:
+        nz, ny, nx = cfg["u0"].shape
+        w = 16
+        bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1], cfg["bc_lo"][2], cfg["bc_hi"][2])
+        pts = [(0, 0, 0), (nx - w, ny - w, nz - w), (nx - w, 0, (nz - w) // 2)]
+        pts += [tuple(int(v) for v in rng.integers(0, min(nx, ny, nz) - w, size=3)) for _ in range(2)]
+        for x0, y0, z0 in pts:
+            x0 -= x0 % 2; y0 -= y0 % 2; z0 -= z0 % 2
+            ref = _window_3d(ge_oracle, cfg["u0"], cfg["r"][0], levels, bc, x0, y0, z0, w)
+            worst = max(worst, float(np.abs(got[z0:z0 + w, y0:y0 + w, x0:x0 + w] - ref).max()))
+        scale = float(np.abs(cfg["u0"]).max())
+        what = "%d windows of %dx%dx%d nodes on their dependency cones" % (len(pts), w, w, w)
+    elif cfg["dim"] == 2:
         ny, nx = cfg["u0"].shape
         w = 24
         bc = (cfg["bc_lo"][0], cfg["bc_hi"][0], cfg["bc_lo"][1], cfg["bc_hi"][1])
@@ -579,9 +609,9 @@ def run_ours(args):
     secondary = None
     if rank == 0 and world == 1 and args.config == "c4" and not args.no_secondary and args.kernel == "auto" and not args.levels:
         secondary = {}
-        for name in ("c5_f32", "c5_f64", "c2", "c3"):
+        for name in ("c5_f32", "c5_f64", "c2", "c3", "box_f32", "box_f64"):
             scfg = make_cfg(name)
-            sn = scfg["nx"] * scfg["ny"] * scfg["batch"] * ESIZE[scfg["dtype"]]
+            sn = scfg["nx"] * scfg["ny"] * scfg.get("nz", 1) * scfg["batch"] * ESIZE[scfg["dtype"]]
             sm_, splan = device_timing(scfg, {}, dev, stream_obj, 3, 3, clocks_index=local, flush_l2=sn <= 126e6)
             sroof = roofline(scfg, sm_["info"], sm_["total_ms_this_rank"], sm_["launches"], 3, peaks_alu)
             spar = parity_check(scfg, splan, dev, stream) if not args.no_cpu else None
@@ -909,7 +939,7 @@ def main():
     ap.add_argument("--md", default="", help="--sweep: also write a markdown table to this file")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle legs (parity, cpu_baseline)")
-    ap.add_argument("--no-secondary", action="store_true", help="skip the C5 / C2 / C3 block of the default line")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the C5 / C2 / C3 / 3-D block of the default line")
     ap.add_argument("--cpu-scale", type=float, default=1 / 128, help="grid fraction of the cpu_baseline sample")
     ap.add_argument("--ref-scale", type=float, default=1 / 128, help="grid fraction of the --impl reference sample (the same sample)")
     args = ap.parse_args()
