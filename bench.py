@@ -679,7 +679,9 @@ def run_sweep(args):
     stream = stream_obj.cuda_stream
     u0 = torch.from_numpy(cfg["u0"].reshape(-1)).to(dev)
     sync_names = {libge.GE_SYNC_FLAGS: "flag + fence", libge.GE_SYNC_GRID: "grid barrier",
-                  libge.GE_SYNC_LINES: "flag-in-data", libge.GE_SYNC_STAGGER: "staggered flag-in-data"}
+                  libge.GE_SYNC_LINES: "flag-in-data", libge.GE_SYNC_STAGGER: "staggered flag-in-data",
+                  libge.GE_SYNC_CLUSTER2: "clusters of 2 (DSMEM)", libge.GE_SYNC_CLUSTER4: "clusters of 4 (DSMEM)",
+                  libge.GE_SYNC_CLUSTER8: "clusters of 8 (DSMEM)", libge.GE_SYNC_CLUSTER16: "clusters of 16 (DSMEM)"}
     settings = [("A: launch per level", dict(kernel="per_step"), {}),
                 ("B: warp-per-tile, tb 16", dict(kernel="temporal", tb=16), {libge.GE_TUNE_TEMPORAL_C: 16}),
                 ("B: TMA-staged, tb 20", dict(kernel="temporal", tb=20), {})]
@@ -698,6 +700,16 @@ def run_sweep(args):
         settings.append(("C: C=%d, halo %d, %s" % (c, hl, sync_names[libge.GE_SYNC_STAGGER]), dict(kernel="persistent"),
                          {libge.GE_TUNE_RESIDENT_C: c, libge.GE_TUNE_HALO_LANES: hl,
                           libge.GE_TUNE_SYNC_MODE: libge.GE_SYNC_STAGGER}))
+    # thread-block clusters: shared memory + the cluster barrier inside a cluster, flags between clusters
+    for c, hl in ((32, 2), (32, 1), (16, 2), (64, 2)):
+        for sync in (libge.GE_SYNC_CLUSTER2, libge.GE_SYNC_CLUSTER4, libge.GE_SYNC_CLUSTER8, libge.GE_SYNC_CLUSTER16):
+            settings.append(("C: C=%d, halo %d, %s" % (c, hl, sync_names[sync]), dict(kernel="persistent"),
+                             {libge.GE_TUNE_RESIDENT_C: c, libge.GE_TUNE_HALO_LANES: hl, libge.GE_TUNE_SYNC_MODE: sync}))
+    for tb in (8, 16, 32):
+        for sync in (libge.GE_SYNC_CLUSTER4, libge.GE_SYNC_CLUSTER8):
+            settings.append(("C: C=32, halo 2, %s, tb %d" % (sync_names[sync], tb), dict(kernel="persistent"),
+                             {libge.GE_TUNE_RESIDENT_C: 32, libge.GE_TUNE_HALO_LANES: 2,
+                              libge.GE_TUNE_SYNC_MODE: sync, libge.GE_TUNE_TB: tb}))
     rows, first = [], None
     for name, kw, tune in settings:
         try:

@@ -204,7 +204,11 @@ enum {
                                   tile, acquire), 1 = grid-wide barrier (cooperative groups), 2 = neighbour
                                   flag-in-data lines (no fence, no separate flag), 3 = the same lines published
                                   every tb/2 levels and consumed every other time, the CTAs that share an SM
-                                  taking opposite turns (needs tb >= 8); default 1, the fastest measured            */
+                                  taking opposite turns (needs tb >= 8); 4, 5, 6, 7 = thread-block CLUSTERS of 2, 4, 8,
+                                  16 CTAs: shared memory (the CTA's own or, through distributed shared memory, the
+                                  adjacent CTA's) and the cluster's hardware barrier inside a cluster, mode 0's flags
+                                  between clusters; GE_EINVAL when the rod cannot stay resident with clusters of that
+                                  size; default 1, the fastest measured                                              */
 };
 int ge_plan_tune(ge_plan *p, int32_t what, int64_t value);
 

@@ -8,6 +8,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -552,19 +553,66 @@ int launch_rod_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
 
 // Path 2: the grid-resident kernel is instantiated for the three largest C of the dtype.
 template <typename T, int C>
-const void* grid_resident_fn() { return (const void*)&ge::ge1d_grid_resident_kernel<T, C>; }
+const void* grid_resident_fn(bool cl) {
+    return cl ? (const void*)&ge::ge1d_grid_resident_kernel<T, C, true> : (const void*)&ge::ge1d_grid_resident_kernel<T, C, false>;
+}
 
-const void* grid_resident_fn_for(int dtype, int c) {
+// cl: the instantiation whose tiles meet inside thread-block clusters (sync modes 4 .. 7)
+const void* grid_resident_fn_for(int dtype, int c, bool cl = false) {
     if (dtype == GE_F64) {
-        if (c == 16) return grid_resident_fn<double, 16>();
-        if (c == 32) return grid_resident_fn<double, 32>();
-        if (c == 64) return grid_resident_fn<double, 64>();
+        if (c == 16) return grid_resident_fn<double, 16>(cl);
+        if (c == 32) return grid_resident_fn<double, 32>(cl);
+        if (c == 64) return grid_resident_fn<double, 64>(cl);
     } else {
-        if (c == 32) return grid_resident_fn<float, 32>();
-        if (c == 64) return grid_resident_fn<float, 64>();
-        if (c == 128) return grid_resident_fn<float, 128>();
+        if (c == 32) return grid_resident_fn<float, 32>(cl);
+        if (c == 64) return grid_resident_fn<float, 64>(cl);
+        if (c == 128) return grid_resident_fn<float, 128>(cl);
     }
     return nullptr;
+}
+
+// Launch geometry of the cluster form: CTAs rounded up to whole clusters, the shared-memory exchange buffer
+// (2 parities x kGridWarps tiles x 2 sides x hl*C), cooperative + cluster attributes.
+struct ClusterLaunch {
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[2];
+};
+int cluster_launch_config(const ge_plan* p, int sync_mode, cudaStream_t s, ClusterLaunch* cl, const void** fn_out) {
+    const int cs = ge::sync_cluster_size(sync_mode);
+    const void* fn = grid_resident_fn_for(p->dtype, p->res_c, true);
+    if (!fn || cs < 2) return GE_EINVAL;
+    const size_t smem = (size_t)2 * ge::kGridWarps * 2 * p->res_hl * p->res_c * elem_size(p->dtype);
+    if (smem > 48 * 1024) GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (cs > 8) GE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    unsigned ctas = (unsigned)((p->res_tiles + ge::kGridWarps - 1) / ge::kGridWarps);
+    ctas = (ctas + cs - 1) / cs * cs;
+    std::memset(cl, 0, sizeof(*cl));
+    cl->cfg.gridDim = dim3(ctas);
+    cl->cfg.blockDim = dim3(32 * ge::kGridWarps);
+    cl->cfg.dynamicSmemBytes = smem;
+    cl->cfg.stream = s;
+    cl->attr[0].id = cudaLaunchAttributeClusterDimension;
+    cl->attr[0].val.clusterDim.x = (unsigned)cs; cl->attr[0].val.clusterDim.y = 1; cl->attr[0].val.clusterDim.z = 1;
+    cl->attr[1].id = cudaLaunchAttributeCooperative;
+    cl->attr[1].val.cooperative = 1;
+    cl->cfg.attrs = cl->attr;
+    cl->cfg.numAttrs = 2;
+    *fn_out = fn;
+    return GE_OK;
+}
+// can the whole rod be resident when its CTAs come in clusters of this size?
+int cluster_mode_fits(const ge_plan* p, int sync_mode, bool* fits) {
+    ClusterLaunch cl;
+    const void* fn = nullptr;
+    *fits = false;
+    const int rc = cluster_launch_config(p, sync_mode, nullptr, &cl, &fn);
+    if (rc != GE_OK) return rc;
+    cl.cfg.numAttrs = 1;                                  // the occupancy query takes the cluster shape only
+    int nclusters = 0;
+    const cudaError_t e = cudaOccupancyMaxActiveClusters(&nclusters, fn, &cl.cfg);
+    if (e != cudaSuccess) { cudaGetLastError(); return GE_OK; }      // this cluster size is not available: does not fit
+    *fits = (int64_t)nclusters * ge::sync_cluster_size(sync_mode) >= (int64_t)cl.cfg.gridDim.x;
+    return GE_OK;
 }
 
 // (Re)derive path-2 geometry from res_c / res_hl / res_tb and (re)allocate its buffers.
@@ -602,6 +650,11 @@ int grid_resident_configure(ge_plan* p) {
     p->res_tiles = tiles;
     p->res_tb = tb;
     p->res_path = 2;
+    if (ge::sync_cluster_size(p->res_sync) > 1) {        // a cluster mode chosen for the old geometry must still fit
+        bool fits = false;
+        const int rc = cluster_mode_fits(p, p->res_sync, &fits);
+        if (rc != GE_OK || !fits) p->res_sync = ge::kSyncGrid;
+    }
     return GE_OK;
 }
 
@@ -616,9 +669,18 @@ int launch_grid_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     if (p->res_sync == ge::kSyncStagger)
         GE_CUDA(cudaMemsetAsync(p->res_flags + p->res_tiles + 1, 0, 256 * sizeof(unsigned), s));
     void* args[] = {&u, &xbuf, &coef, &flags, &fault, &a};
-    const void* fn = grid_resident_fn_for(p->dtype, p->res_c);
-    const unsigned ctas = (unsigned)((p->res_tiles + ge::kGridWarps - 1) / ge::kGridWarps);
-    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(ctas), dim3(32 * ge::kGridWarps), args, 0, s);
+    cudaError_t e;
+    if (ge::sync_cluster_size(p->res_sync) > 1) {
+        ClusterLaunch cl;
+        const void* fn = nullptr;
+        const int rc = cluster_launch_config(p, p->res_sync, s, &cl, &fn);
+        if (rc != GE_OK) return rc;
+        e = cudaLaunchKernelExC(&cl.cfg, fn, args);
+    } else {
+        const void* fn = grid_resident_fn_for(p->dtype, p->res_c);
+        const unsigned ctas = (unsigned)((p->res_tiles + ge::kGridWarps - 1) / ge::kGridWarps);
+        e = cudaLaunchCooperativeKernel(fn, dim3(ctas), dim3(32 * ge::kGridWarps), args, 0, s);
+    }
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     const int64_t meet = ge::grid_resident_meetings(steps, a.phase0, a.tb);
     // every launch moves the epoch past all flag values / line tags it used (one extra meeting is held
@@ -1302,8 +1364,14 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         }
         case GE_TUNE_SYNC_MODE:
             if (p->kernel != GE_KERNEL_PERSISTENT || p->res_path != 2) return GE_EINVAL;
-            if (value < ge::kSyncFlags || value > ge::kSyncStagger) return GE_EINVAL;
+            if (value < ge::kSyncFlags || value > ge::kSyncCluster16) return GE_EINVAL;
             if (value == ge::kSyncStagger && p->res_tb < 8) return GE_EINVAL;
+            if (ge::sync_cluster_size((int)value) > 1) {         // clusters: the whole rod must still be co-resident
+                bool fits = false;
+                const int rc = cluster_mode_fits(p, (int)value, &fits);
+                if (rc != GE_OK) return rc;
+                if (!fits) return GE_EINVAL;
+            }
             p->res_sync = (int32_t)value;
             return GE_OK;
         case GE_TUNE_TB:

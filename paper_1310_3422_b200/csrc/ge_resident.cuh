@@ -284,6 +284,12 @@ constexpr int kGridWarps = 4;              // warps (tiles) per CTA
 // 2 = flag-in-data lines, no fence and no separate flag (neighbours only), 3 = the same, published every
 // tb/2 levels and consumed in opposite turns by the CTAs that share an SM
 constexpr int kSyncFlags = 0, kSyncGrid = 1, kSyncLL = 2, kSyncStagger = 3;
+// 4 .. 7 = thread-block CLUSTERS of 2 / 4 / 8 / 16 CTAs (kernel instantiation CL = true): the tiles of a cluster
+// publish into their CTA's shared memory, meet at the cluster's hardware barrier and read their neighbours' sides
+// from shared memory -- their own CTA's or, through distributed shared memory, the adjacent CTA's; only the two
+// tiles at the ends of a cluster exchange through L2 with a flag, as in mode 0
+constexpr int kSyncCluster2 = 4, kSyncCluster16 = 7;
+inline int sync_cluster_size(int mode) { return mode >= kSyncCluster2 && mode <= kSyncCluster16 ? 2 << (mode - kSyncCluster2) : 1; }
 constexpr int kLineSlots = 4;          // exchange slots of the flag-in-data modes (2 are used by kSyncLL)
 
 struct GridResidentArgs {
@@ -380,7 +386,7 @@ template <> struct Line<float> {
     }
 };
 
-template <typename T, int C>
+template <typename T, int C, bool CL = false>
 __global__ void __launch_bounds__(32 * kGridWarps)
 ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsigned* flags, unsigned* fault,
                           const GridResidentArgs a) {
@@ -430,7 +436,7 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
         if (lane == 0) { __threadfence(); st_relaxed_u32(flags + tile, stage); }
     };
     auto await = [&]() {
-        if (a.sync_mode != kSyncFlags || !active) return;
+        if (!(a.sync_mode == kSyncFlags || CL) || !active) return;
         // lane 0 acquires for the warp; __syncwarp orders the other lanes' reads after it
         if (lane == 0 && (has_l || has_r))
             wait_flags(has_l ? flags + tile - 1 : nullptr, has_r ? flags + tile + 1 : nullptr, stage, fault);
@@ -490,7 +496,75 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
         consume_lines(parity, stage);
         parity ^= 1;
     };
+    // cluster meeting (CL): shared memory [2 parities][kGridWarps tiles][2 sides][hl*C]; double-buffered, so the one
+    // cluster barrier of a meeting also orders the reads of the meeting before the last against the next writes
+    auto meet_cluster = [&]() {
+        if constexpr (CL) {
+            extern __shared__ __align__(16) unsigned char gr_smem[];
+            T* xs = reinterpret_cast<T*>(gr_smem);
+            cg::cluster_group cluster = cg::this_cluster();
+            const unsigned crank = cluster.block_rank(), csize = cluster.num_blocks();
+            const bool cross_l = has_l && warp == 0 && crank == 0;                        // the neighbour is in another cluster
+            const bool cross_r = has_r && warp == kGridWarps - 1 && crank == csize - 1;
+            ++stage;
+            if (active && (own_l || own_r)) {
+                T* dst = xs + ((size_t)(parity * kGridWarps + warp) * 2 + (own_l ? 0 : 1)) * side +
+                         (size_t)(own_l ? lane - hl : lane - (32 - 2 * hl)) * C;
+                T* gdst = nullptr;
+                if ((own_l && cross_l) || (own_r && cross_r))
+                    gdst = xbuf + ((size_t)parity * a.ntiles + tile) * 2 * side +
+                           (own_l ? (size_t)(lane - hl) * C : side + (size_t)(lane - (32 - 2 * hl)) * C);
+#pragma unroll
+                for (int j = 0; j < C / V; ++j) {
+                    T t[V];
+#pragma unroll
+                    for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
+                    st_vec(dst + j * V, t);
+                    if (gdst) st_vec_cg(gdst + j * V, t);
+                }
+            }
+            if (active && (cross_l || cross_r)) {
+                __syncwarp();
+                if (lane == 0) { __threadfence(); st_relaxed_u32(flags + tile, stage); }
+            }
+            cluster.sync();
+            if (active && (cross_l || cross_r)) {
+                if (lane == 0) wait_flags(cross_l ? flags + tile - 1 : nullptr, cross_r ? flags + tile + 1 : nullptr, stage, fault);
+                __syncwarp();
+            }
+            if (active) {
+                const T* src = nullptr;
+                bool global = false;
+                if (halo_l && has_l) {
+                    if (cross_l) { src = xbuf + ((size_t)parity * a.ntiles + tile - 1) * 2 * side + side + (size_t)lane * C; global = true; }
+                    else {
+                        const T* base = warp > 0 ? xs : cluster.map_shared_rank(xs, crank - 1);
+                        const int w = warp > 0 ? warp - 1 : kGridWarps - 1;
+                        src = base + ((size_t)(parity * kGridWarps + w) * 2 + 1) * side + (size_t)lane * C;
+                    }
+                } else if (halo_r && has_r) {
+                    if (cross_r) { src = xbuf + ((size_t)parity * a.ntiles + tile + 1) * 2 * side + (size_t)(lane - (32 - hl)) * C; global = true; }
+                    else {
+                        const T* base = warp < kGridWarps - 1 ? xs : cluster.map_shared_rank(xs, crank + 1);
+                        const int w = warp < kGridWarps - 1 ? warp + 1 : 0;
+                        src = base + ((size_t)(parity * kGridWarps + w) * 2 + 0) * side + (size_t)(lane - (32 - hl)) * C;
+                    }
+                }
+                if (src) {
+#pragma unroll
+                    for (int j = 0; j < C / V; ++j) {
+                        T t[V];
+                        if (global) ld_vec_cg(src + j * V, t); else ld_vec_plain(src + j * V, t);
+#pragma unroll
+                        for (int i = 0; i < V; ++i) v[j * V + i] = t[i];
+                    }
+                }
+            }
+            parity ^= 1;
+        }
+    };
     auto meet = [&]() {
+        if constexpr (CL) { meet_cluster(); return; }
         if (a.sync_mode == kSyncLL) { meet_lines(); return; }
         // publish the outermost valid lanes, meet the neighbours, refresh the halo lanes
         ++stage;
@@ -621,6 +695,8 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
             st_vec(u + e0 + j * V, t);
         }
     }
+    // a CTA's shared memory must outlive its neighbours' reads of it
+    if constexpr (CL) cg::this_cluster().sync();
 }
 
 }  // namespace ge

@@ -72,7 +72,7 @@ def _c2_windows(oracle, cfg, w):
     return _C2_WINDOWS
 
 
-@pytest.mark.parametrize("sync", [1, 0, 2, 3])
+@pytest.mark.parametrize("sync", [1, 0, 2, 3, 6])
 def test_c2_all_levels_every_meeting_kind_against_the_oracle(oracle, sync):
     """C2 (N = 2^20 fp64, r = 4, 10 000 levels) on the whole-chip persistent kernel: grid barrier (1, the
     default), neighbour flags (0), flag-in-data lines (2), staggered lines (3)."""
@@ -91,7 +91,7 @@ def test_c2_all_levels_every_meeting_kind_against_the_oracle(oracle, sync):
     assert np.isfinite(got).all()
 
 
-@pytest.mark.parametrize("sync,rtb", [(0, 8), (2, 8), (3, 8), (2, 2)])
+@pytest.mark.parametrize("sync,rtb", [(0, 8), (2, 8), (3, 8), (2, 2), (6, 8), (4, 2)])
 def test_whole_chip_many_meetings_against_the_oracle(oracle, sync, rtb):
     """The same kernel with a meeting every 8 (2) levels -- 250 (1000) meetings in 2000 levels -- on a rod of
     ~60 tiles, whole array against the oracle."""
