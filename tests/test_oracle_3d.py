@@ -104,3 +104,66 @@ def test_exact_rational_fixture(oracle):
         np.testing.assert_allclose(g1, a1, rtol=0, atol=1e-12)
         np.testing.assert_allclose(oracle.level_3d(g1, r, 1, bc), a2, rtol=0, atol=1e-12)
         np.testing.assert_allclose(oracle.run_3d(a0, r, 2, bc), a2, rtol=0, atol=1e-12)
+
+
+def _walsh_group(R, r, axes):
+    """Closed form of one group in exact rationals, a derivation that never assembles a matrix: the group's block
+    is (1+3r) I - r (sum of the partner swaps along the group's `axes`), the swaps commute, their common
+    eigenvectors are the Walsh functions h_m[d] = (-1)^popcount(d & m) with eigenvalue
+    1 + 3r - r (number of axes) + 2 r popcount(m); new = sum_m h_m <h_m, b> / (2^axes lambda_m)."""
+    n = 1 << axes
+    out = []
+    for d in range(n):
+        acc = F(0)
+        for m in range(n):
+            lam = 1 + 3 * r - r * axes + 2 * r * bin(m).count("1")
+            coef = sum(F((-1) ** bin(e & m).count("1")) * R[e] for e in range(n))
+            acc += F((-1) ** bin(d & m).count("1")) * coef / (n * lam)
+        out.append(acc)
+    return out
+
+
+@pytest.mark.parametrize("r", [F(1, 2), F(2), F(7)])
+def test_walsh_closed_form_in_exact_rationals(oracle, r):
+    """The oracle eliminates every group's block numerically; here the same level comes from the Walsh / Kronecker
+    closed form in exact rationals (a second derivation: no matrix, no elimination) -- a full 2x2x2 group whose
+    out-of-group neighbours are all boundary values, a full group with interior out-of-group neighbours, and the
+    groups cut by one face (a 2x2 square: eigenvalues 1+r, 1+3r, 1+3r, 1+5r -- the form the CUDA kernels use,
+    csrc/ge_level3d.cuh cut4_solve), by an edge (a pair: 1+2r, 1+4r) and by a corner (one node: 1+3r)."""
+    rng = np.random.default_rng(int(r * 2))
+    bc = (F(3), F(-1), F(2), F(5), F(-4), F(1))                      # x_lo, x_hi, y_lo, y_hi, z_lo, z_hi
+    bcf = tuple(float(v) for v in bc)
+    for phase, shape in ((0, (2, 2, 2)), (0, (1, 2, 2)), (1, (3, 3, 3)), (1, (2, 3, 3)), (0, (3, 3, 3))):
+        nz, ny, nx = shape
+        u = rng.integers(-9, 10, size=shape)
+        val = lambda x, y, z: (bc[0] if x < 0 else bc[1] if x >= nx else bc[2] if y < 0 else bc[3] if y >= ny
+                               else bc[4] if z < 0 else bc[5] if z >= nz else F(int(u[z, y, x])))
+        expect = np.zeros(shape)
+        first = lambda n: range(-phase, n, 2)                        # anchors -phase, 2 - phase, ... <= n - 1
+        for gz in first(nz):
+            for gy in first(ny):
+                for gx in first(nx):
+                    # the axes along which both nodes of the group are inside, and its interior members
+                    inside = [[g + t for t in (0, 1) if 0 <= g + t < n] for g, n in ((gx, nx), (gy, ny), (gz, nz))]
+                    full = [a for a in range(3) if len(inside[a]) == 2]
+                    members = [(x, y, z) for z in inside[2] for y in inside[1] for x in inside[0]]   # x fastest
+                    b = []
+                    for (x, y, z) in members:
+                        o = val(x, y, z)
+                        s = F(0)
+                        for a, (p, g) in enumerate(((x, gx), (y, gy), (z, gz))):
+                            q = [x, y, z]
+                            q[a] = p - 1 if p == g else p + 1        # the neighbour OUTSIDE the group along axis a
+                            s += val(*q) - o
+                        rhs = o + r * s                              # (1 - 3r) old + r (three out-of-group neighbours)
+                        for a in range(3):                           # an in-group partner that is a boundary node: new level
+                            if a not in full:
+                                q = [x, y, z]
+                                q[a] = -1 if [gx, gy, gz][a] < 0 else [nx, ny, nz][a]
+                                rhs += r * val(*q)
+                        b.append(rhs)
+                    new = _walsh_group(b, r, len(full))
+                    for (x, y, z), v in zip(members, new):
+                        expect[z, y, x] = float(v)
+        got = oracle.level_3d(u.astype(np.float64), float(r), phase, bcf)
+        np.testing.assert_allclose(got, expect, rtol=0, atol=2e-13 * max(1.0, float(r)), err_msg=str((phase, shape)))
