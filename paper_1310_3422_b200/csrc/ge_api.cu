@@ -476,6 +476,26 @@ bool temporal_ok(const ge_plan* p, const void* u) {
     return p->nx % V == 0 && ((uintptr_t)u % 16 == 0) && ((uintptr_t)p->scratch % 16 == 0);
 }
 
+// Rows the aligned kernels do not take (batched rods with nx % V != 0, unaligned pointers): the warp-per-tile kernel
+// with coalesced scalar accesses transposed through shared memory (ge_temporal.cuh, UA).  C = 2 C0 when the rod
+// holds two such tiles, else C0.
+template <typename T>
+int launch_temporal_1d_unaligned(ge_plan* p, const void* uin, void* uout, int tb, cudaStream_t s) {
+    const int phase = (int)(p->level & 1);
+    auto* in = (const T*)uin;
+    auto* out = (T*)uout;
+    auto* c = (const ge::Coef1<T>*)p->coef;
+    constexpr int C0 = 16 / (int)sizeof(T) * 4;     // 8 (f64) / 16 (f32)
+    if (tb < 1 || tb > ge::temporal1d_max_tb(C0)) return GE_EINVAL;
+    const cudaError_t e = p->nx >= 128 * (int64_t)C0
+                              ? ge::temporal1d_unaligned_launch<T, 2 * C0>(in, out, p->nx, p->batch, c, tb, phase, s)
+                              : ge::temporal1d_unaligned_launch<T, C0>(in, out, p->nx, p->batch, c, tb, phase, s);
+    if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+    p->launches += 1;
+    p->level += tb;
+    return GE_OK;
+}
+
 int stream_tc(int dtype) { return dtype == GE_F64 ? 22 : 52; }     // measured on C4 / C3
 bool is_stream_tc(int dtype, int64_t tc) { const int64_t b = dtype == GE_F64 ? 8 : 4; return tc * b == 144 || tc * b == 176 || tc * b == 208; }
 // the TMA-staged kernel when the rod holds at least two tiles, else the warp-per-tile one
@@ -1018,7 +1038,9 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     }
     const bool blocked = (p->kernel == GE_KERNEL_TEMPORAL || p->kernel == GE_KERNEL_PERSISTENT) && p->group_k == 1;
     const int64_t prefix = blocked ? temporal_prefix(p, u) : 0;
-    const bool temporal = blocked && (prefix > 0 || temporal_ok(p, u));
+    const bool temporal_al = blocked && (prefix > 0 || temporal_ok(p, u));
+    const bool unaligned = blocked && !temporal_al && p->dim == 1 && p->tb >= 1 && p->tb + 2 <= 64;
+    const bool temporal = temporal_al || unaligned;
     const bool temporal_k = p->kernel == GE_KERNEL_TEMPORAL && p->group_k >= 2;
     while (left > 0 && rc == GE_OK) {
         if (temporal_k) {
@@ -1061,7 +1083,10 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                 const int64_t nl = (left + p->tb - 1) / p->tb;
                 tbn = (int)((left + nl - 1) / nl);
             }
-            if (prefix) {
+            if (unaligned) {
+                rc = p->dtype == GE_F64 ? launch_temporal_1d_unaligned<double>(p, cur, oth, tbn, s)
+                                        : launch_temporal_1d_unaligned<float>(p, cur, oth, tbn, s);
+            } else if (prefix) {
                 // the prefix as a rod of its own (tile geometry and kernel choice follow its length), then the end piece
                 const int64_t nx0 = p->nx;
                 const int ph0 = (int)(p->level & 1);

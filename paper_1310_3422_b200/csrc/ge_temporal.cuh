@@ -76,16 +76,36 @@ inline Temporal1dGeom temporal1d_geom(int C, int V, int tb, int phase) {
 }
 inline int temporal1d_max_tb(int C) { return 8 * C; }      // keeps at least half of every tile valid
 
-template <typename T, int C, bool EDGE>
+// UA ("unaligned"): rows of any length at any element alignment (batched rods with nx % V != 0, unaligned user
+// pointers).  The tile's 32*C elements are read and written with COALESCED scalar accesses -- lane t takes element
+// i*32 + t of the window -- and transposed through the warp's own piece of shared memory `sm` (32 rows of C + 1
+// elements: conflict-free both ways), so no global access depends on alignment.  Same arithmetic.
+template <typename T, int C, bool EDGE, bool UA = false>
 __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __restrict__ out, int64_t nx,
                                                 const Coef1<T>& k, const Temporal1dGeom g,
-                                                int64_t tile, int lane) {
+                                                int64_t tile, int lane, T* __restrict__ sm = nullptr) {
     constexpr int V = VecOf<T>::V;
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(C % 2 == 0 && C % V == 0, "C must hold whole pairs and whole vectors");
     // element index of v[0] at load time
     const int64_t a0 = tile * g.valid - g.shift + (int64_t)lane * C;
     T v[C];
+    if constexpr (UA) {
+        const int64_t w0 = tile * g.valid - g.shift;                 // the warp's first element
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int q = i * 32 + lane;
+            const int64_t e = w0 + q;
+            T x;
+            if (!EDGE || (e >= 0 && e < nx)) x = in[e];
+            else x = e == -1 ? k.lo : (e == nx ? k.hi : T(0));
+            sm[(q / C) * (C + 1) + q % C] = x;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < C; ++j) v[j] = sm[lane * (C + 1) + j];
+        __syncwarp();
+    } else
 #pragma unroll
     for (int c = 0; c < C / V; ++c) {
         const int64_t idx = a0 + c * V;
@@ -149,6 +169,18 @@ __device__ __forceinline__ void temporal1d_tile(const T* __restrict__ in, T* __r
     for (int s = 0; s < g.post; ++s) shift_window<T, C>(v);
     // window start is now a0 + shift = tile*valid + lane*C: store what stayed inside the cone
     const int64_t o0 = tile * g.valid + (int64_t)lane * C;
+    if constexpr (UA) {
+#pragma unroll
+        for (int j = 0; j < C; ++j) sm[lane * (C + 1) + j] = v[j];
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int q = i * 32 + lane;
+            const int64_t e = tile * g.valid + q;
+            if (q < g.valid && e < nx) out[e] = sm[(q / C) * (C + 1) + q % C];
+        }
+        __syncwarp();
+    } else
 #pragma unroll
     for (int c = 0; c < C / V; ++c) {
         const int64_t idx = o0 + c * V;
@@ -273,6 +305,37 @@ ge1d_temporal_generic_kernel(const T* __restrict__ uin, T* __restrict__ uout, in
         if (edge) temporal1d_tile<T, C, true>(in, out, nx, k, g, tile, lane);
         else      temporal1d_tile<T, C, false>(in, out, nx, k, g, tile, lane);
     }
+}
+
+// The same tiles for rows of any length and alignment (temporal1d_tile UA).
+template <typename T, int C>
+__global__ void __launch_bounds__(kTemporalWarps * 32)
+ge1d_temporal_unaligned_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t batch,
+                               const Coef1<T>* __restrict__ coef, const Temporal1dGeom g, int64_t tiles_per_rod) {
+    __shared__ T sm_all[kTemporalWarps][32 * (C + 1)];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kTemporalWarps + warp;
+    if (tile >= tiles_per_rod) return;
+    const int64_t lo_idx = tile * g.valid - g.shift;          // first element loaded
+    const bool edge = lo_idx < 0 || lo_idx + 32 * C > nx;
+    for (int64_t rod = blockIdx.y; rod < batch; rod += gridDim.y) {
+        const Coef1<T> k = coef[rod];
+        const T* __restrict__ in = uin + rod * nx;
+        T* __restrict__ out = uout + rod * nx;
+        if (edge) temporal1d_tile<T, C, true, true>(in, out, nx, k, g, tile, lane, sm_all[warp]);
+        else      temporal1d_tile<T, C, false, true>(in, out, nx, k, g, tile, lane, sm_all[warp]);
+    }
+}
+// Requires only 1 <= tb <= temporal1d_max_tb(C).
+template <typename T, int C>
+inline cudaError_t temporal1d_unaligned_launch(const T* uin, T* uout, int64_t nx, int64_t batch, const Coef1<T>* coef,
+                                               int tb, int phase, cudaStream_t s) {
+    const Temporal1dGeom g = temporal1d_geom(C, VecOf<T>::V, tb, phase);
+    const int64_t tiles = (nx + g.valid - 1) / g.valid;
+    dim3 grid((unsigned)((tiles + kTemporalWarps - 1) / kTemporalWarps), (unsigned)(batch < 65535 ? batch : 65535));
+    ge1d_temporal_unaligned_kernel<T, C><<<grid, kTemporalWarps * 32, 0, s>>>(uin, uout, nx, batch, coef, g, tiles);
+    return cudaGetLastError();
 }
 
 // Host launcher: tb levels starting at a level of the given phase.

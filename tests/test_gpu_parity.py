@@ -104,12 +104,15 @@ def test_temporal_1d_bitwise_equals_per_step():
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_temporal_1d_odd_n_batched_falls_back_to_per_step(oracle, dtype):
-    """Batched rods of odd length start at alternating alignments: no vector kernel, one launch per level."""
+def test_temporal_1d_odd_n_batched_stays_blocked(oracle, dtype):
+    """Batched rods of odd length start at alternating alignments: no vector kernel, but still tb levels per launch
+    (the unaligned form of the warp-per-tile kernel; r01 fell back to one launch per level here)."""
     cfg = inputs.random_rods(2, 1001, dtype, seed=77)
     got, info = run_gpu(cfg, 33, kernel="temporal")
-    assert info["launches"] == 33
+    assert info["launches"] <= 3, info
     assert rel_err_rows(got, run_oracle(oracle, cfg, 33)) <= TOL[dtype]
+    same, _ = run_gpu(cfg, 33, kernel="per_step")
+    np.testing.assert_array_equal(got, same)
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -131,6 +134,58 @@ def test_awkward_lengths_stay_on_the_blocked_kernels(oracle, dtype, n, kernel):
             assert info["launches"] < steps, info            # blocked launches + one end piece each
         same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
         np.testing.assert_array_equal(got, same, err_msg=str((dtype, n, kernel, level0, steps, info)))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("batch,n", [(7, 1001), (5, 4098), (3, 4097), (40, 99), (33, 100), (2, 40001), (9, 515), (4, 31)])
+def test_batched_rods_of_awkward_lengths_stay_blocked(oracle, dtype, batch, n):
+    """Batched rods whose length is not a multiple of the 16-byte vector start at unaligned addresses: the
+    warp-per-tile kernel reads and writes them with coalesced scalar accesses transposed through shared memory
+    (ge_temporal.cuh, UA) instead of falling to one launch per level.  Per-rod r and boundary values, both starting
+    phases, odd level counts; against the oracle and bit for bit against the per-level kernel."""
+    cfg = inputs.random_rods(batch, n, dtype, seed=batch * 1000 + n, r_hi=4.0)
+    v = 2 if dtype == "f64" else 4
+    for level0, steps in ((0, 1), (1, 40), (0, 101), (1, 23)):
+        got, info = run_gpu(cfg, steps, kernel="temporal", level0=level0)
+        ref = run_oracle(oracle, cfg, steps, level0=level0)
+        assert rel_err_rows(got, ref, cfg) <= TOL[dtype], (batch, n, level0, steps, info)
+        if n % v and steps >= 23:
+            assert info["launches"] <= steps // 8 + 2, info
+        same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+        np.testing.assert_array_equal(got, same, err_msg=str((dtype, batch, n, level0, steps, info)))
+        auto, _ = run_gpu(cfg, steps, level0=level0)
+        np.testing.assert_array_equal(auto, same)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("batch,n,off", [(1, 2 ** 16, 1), (1, 4099, 1), (6, 2048, 1), (3, 1000, 3), (1, 2 ** 20, 2)])
+def test_unaligned_pointers_stay_blocked(oracle, dtype, batch, n, off):
+    """A state that starts `off` elements after a 16-byte boundary (a slice of a larger buffer): ge_run must neither
+    fault nor fall to one launch per level."""
+    import torch
+    from paper_1310_3422_b200 import libge
+    cfg = inputs.random_rods(batch, n, dtype, seed=n % 991 + off)
+    dev = torch.device("cuda:0")
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    big = torch.zeros(batch * n + 8, dtype=torch.float64 if dtype == "f64" else torch.float32, device=dev)
+    es = big.element_size()
+    if off * es % 16 == 0:
+        pytest.skip("this offset is 16-byte aligned for the dtype")
+    u = big[off:off + batch * n]
+    u.copy_(torch.from_numpy(cfg["u0"].reshape(-1)).to(dev))
+    assert u.data_ptr() % 16 != 0
+    steps = 61
+    with libge.Plan(cfg, kernel="temporal", stream=stream) as plan:
+        plan.run(u.data_ptr(), steps, stream)
+        torch.cuda.synchronize(dev)
+        info = plan.info()
+    got = u.cpu().numpy().reshape(cfg["u0"].shape)
+    assert info["launches"] <= steps // 8 + 2, info
+    assert float(big[:off].abs().max()) == 0.0 and float(big[off + batch * n:].abs().max()) == 0.0   # nothing outside
+    same, _ = run_gpu(cfg, steps, kernel="per_step")
+    np.testing.assert_array_equal(got, same)
+    ref = run_oracle(oracle, cfg, steps)
+    assert rel_err_rows(got, ref, cfg) <= TOL[dtype]
 
 
 def test_run_is_deterministic():
@@ -212,10 +267,10 @@ def test_persistent_whole_chip(oracle, dtype, n, rc, hl, rtb, sync):
 
 
 def test_persistent_falls_back_when_the_shape_does_not_fit(oracle):
-    # odd N, batched: no resident kernel, no vector kernel either -> per-level launches
+    # odd N, batched: no resident kernel, no vector kernel either -> the unaligned blocked kernel
     cfg = inputs.random_rods(2, 1001, "f64", seed=5)
     got, info = run_gpu(cfg, 20, kernel="persistent")
-    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] == 20
+    assert info["kernel"] == "temporal" and info["resident_path"] == 0 and info["launches"] <= 2
     assert rel_err_rows(got, run_oracle(oracle, cfg, 20), cfg) <= TOL["f64"]
     # 2-D: strategy C is 1-D only
     cfg = inputs.random_grid(64, 64, "f32", seed=6)
