@@ -188,7 +188,7 @@ enum {
     GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
                                   2-D: one of the compiled-in block lengths 4, 6, 8; 6 needs the strip kernel)                            */
     GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64) */
-    GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 8..64, f32: 16..128, powers of two; one
+    GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 2..64, f32: 4..128, powers of two; one
                                   long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
     GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */
     GE_TUNE_STRIP_COOP = 6,    /* 2-D strip kernel: warps of a CTA that share ONE strip and exchange their edge columns

@@ -510,8 +510,11 @@ int clamp_tb(const ge_plan* p, int64_t tb) {
 // ---- strategy C (ge_resident.cuh) ------------------------------------------
 // Values per lane the resident kernels are instantiated for (ascending).
 template <typename T> struct ResidentC;
-template <> struct ResidentC<float>  { static constexpr int n = 4; static constexpr int c[4] = {16, 32, 64, 128}; };
-template <> struct ResidentC<double> { static constexpr int n = 4; static constexpr int c[4] = {8, 16, 32, 64}; };
+// (the two smallest serve short batched rods -- a rod of 100 nodes in 25 lanes of one warp; the whole-chip kernel
+// takes the three largest)
+constexpr int kResidentCs = 6;
+template <> struct ResidentC<float>  { static constexpr int n = kResidentCs; static constexpr int c[kResidentCs] = {4, 8, 16, 32, 64, 128}; };
+template <> struct ResidentC<double> { static constexpr int n = kResidentCs; static constexpr int c[kResidentCs] = {2, 4, 8, 16, 32, 64}; };
 constexpr int kRodMaxWarps = 8;
 
 inline const int* resident_c_list(int dtype) { return dtype == GE_F64 ? ResidentC<double>::c : ResidentC<float>::c; }
@@ -523,7 +526,7 @@ bool rod_resident_pick(int dtype, int64_t nx, int want_c, int* c_out, int* w_out
     if (nx % 2) return false;
     if (want_c) {
         bool known = false;
-        for (int i = 0; i < 4; ++i) known |= cs[i] == want_c;
+        for (int i = 0; i < kResidentCs; ++i) known |= cs[i] == want_c;
         if (!known || nx % want_c) return false;
         const int64_t lanes = nx / want_c;
         int w = 1;
@@ -532,9 +535,9 @@ bool rod_resident_pick(int dtype, int64_t nx, int want_c, int* c_out, int* w_out
         *c_out = want_c; *w_out = w;
         return true;
     }
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < kResidentCs; ++i)
         if (nx % cs[i] == 0 && nx / cs[i] <= 32) { *c_out = cs[i]; *w_out = 1; return true; }
-    for (int i = 3; i >= 0; --i) {
+    for (int i = kResidentCs - 1; i >= 0; --i) {
         if (nx % cs[i]) continue;
         const int64_t lanes = nx / cs[i];
         int w = 1;
@@ -565,6 +568,8 @@ int launch_rod_resident(ge_plan* p, void* u, int64_t steps, cudaStream_t s) {
     else if (p->res_c == cs[1]) e = rod_resident_dispatch_w<T, cs[1]>(p, (T*)u, phase0, steps, s);
     else if (p->res_c == cs[2]) e = rod_resident_dispatch_w<T, cs[2]>(p, (T*)u, phase0, steps, s);
     else if (p->res_c == cs[3]) e = rod_resident_dispatch_w<T, cs[3]>(p, (T*)u, phase0, steps, s);
+    else if (p->res_c == cs[4]) e = rod_resident_dispatch_w<T, cs[4]>(p, (T*)u, phase0, steps, s);
+    else if (p->res_c == cs[5]) e = rod_resident_dispatch_w<T, cs[5]>(p, (T*)u, phase0, steps, s);
     if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
     p->launches += 1;
     p->level += steps;
@@ -722,7 +727,7 @@ int resident_configure(ge_plan* p, int want_c) {
     const bool rod = rod_resident_pick(p->dtype, p->nx, want_c, &c, &w);
     // one rod that needs more than one warp: spread it over the chip when it fits there
     if (p->batch == 1 && (!rod || w > 1)) {
-        p->res_c = want_c ? want_c : cs[2];
+        p->res_c = want_c ? want_c : cs[4];
         const int rc = grid_resident_configure(p);
         if (rc != GE_OK || p->res_path == 2) return rc;
     }

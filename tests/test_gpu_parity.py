@@ -206,7 +206,11 @@ def test_run_host_matches_run(oracle):
 @pytest.mark.parametrize("dtype,n,rc", [("f32", 64, 0), ("f32", 512, 16), ("f32", 4096, 0), ("f32", 4096, 64),
                                         ("f32", 4096, 32), ("f32", 2048 + 128, 0), ("f32", 96, 0), ("f32", 16384, 0),
                                         ("f64", 8, 0), ("f64", 64, 0), ("f64", 2048, 0), ("f64", 2048, 32),
-                                        ("f64", 2048, 16), ("f64", 1000, 8), ("f64", 16384, 64)])
+                                        ("f64", 2048, 16), ("f64", 1000, 8), ("f64", 16384, 64),
+                                        # short rods on the small lane widths (C = 4, 8 fp32 / 2, 4 fp64)
+                                        ("f32", 4, 0), ("f32", 8, 0), ("f32", 100, 0), ("f32", 100, 4), ("f32", 1000, 0), ("f32", 1000, 8),
+                                        ("f32", 1016, 0), ("f64", 2, 0), ("f64", 4, 0), ("f64", 6, 0), ("f64", 50, 0), ("f64", 100, 4),
+                                        ("f64", 62, 2), ("f64", 500, 2), ("f64", 510, 0)])
 def test_persistent_rods(oracle, dtype, n, rc):
     """Strategy C, path 1 (a rod per CTA, state in registers for the whole run): one launch whatever
     the number of levels; one warp (shuffles only) and several warps (shared-memory edge exchange);
