@@ -1017,6 +1017,48 @@ int ge_step_3d(ge_plan* p, const void* u_in, void* u_out, ge_stream_t stream) {
     return step_common(p, 3, u_in, u_out, (cudaStream_t)stream);
 }
 
+// Levels of the next launch of strategy B in 1-D, `left` levels to go from level `level`.
+static int temporal1d_block(int64_t left, int64_t level, int tb, int tc) {
+    int tbn;
+    if (tb % 2 == 0 && tb >= 4) {
+        // blocks that start at an odd level and have an even length are pure R/L pairs: a run from
+        // an even level opens with one block of tb-1 levels (in-lane level I first), a tail of one
+        // or two levels joins the last block (which may then end with R + shift back)
+        const int64_t nl = left > 2 ? (left - 2 + tb - 1) / tb : 1;   // launches to go (a block may take tb+2)
+        int64_t q = (left + nl - 1) / nl;
+        q += q & 1;
+        tbn = (int)((level & 1) ? q : q - 1);
+        if (tbn > left) tbn = (int)left;
+        if (left - tbn <= 2 && left <= ge::temporal1d_max_tb(tc)) tbn = (int)left;
+    } else {
+        // equal-sized blocks: ceil(left / tb) launches of (almost) the same number of levels
+        const int64_t nl = (left + tb - 1) / tb;
+        tbn = (int)((left + nl - 1) / nl);
+    }
+    return tbn;
+}
+static int64_t temporal1d_launch_count(int64_t left, int64_t level, int tb, int tc) {
+    int64_t n = 0;
+    while (left > 0) { const int t = temporal1d_block(left, level, tb, tc); left -= t; level += t; ++n; }
+    return n;
+}
+// The state ping-pongs between the caller's buffer and the plan's scratch level: an ODD number of launches leaves
+// the result in the scratch level and costs a copy of the whole state.  Three or more launches: a block length up
+// to a quarter larger (one launch fewer) or, failing that, smaller (one launch more: the price of the copy, no
+// more) makes the count even.  Returns the block length to run with.
+static int temporal1d_even_tb(int64_t left, int64_t level, int tb, int tc, int tb_max) {
+    const int64_t n0 = temporal1d_launch_count(left, level, tb, tc);
+    if (n0 < 3 || (n0 & 1) == 0) return tb;
+    const int step = (tb % 2 == 0 && tb >= 4) ? 2 : 1;             // an even tb keeps the R/L block form
+    int cap = tb + tb / 4;
+    if (cap > tb_max) cap = tb_max;
+    for (int t = tb + step; t <= cap; t += step)
+        if ((temporal1d_launch_count(left, level, t, tc) & 1) == 0) return t;
+    for (int t = tb - step; t >= 4 && 2 * t >= tb; t -= step)
+        if ((temporal1d_launch_count(left, level, t, tc) & 1) == 0) return t;
+    return tb;
+}
+
 int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     if (!p || !u || steps < 0) return GE_EINVAL;
     NvtxRange nvtx("ge_run");
@@ -1047,6 +1089,13 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
     const bool unaligned = blocked && !temporal_al && p->dim == 1 && p->tb >= 1 && p->tb + 2 <= 64;
     const bool temporal = temporal_al || unaligned;
     const bool temporal_k = p->kernel == GE_KERNEL_TEMPORAL && p->group_k >= 2;
+    int tb1d = p->tb;
+    if (temporal && p->dim == 1) {
+        // largest block the kernel of this run takes: the unaligned form has the smaller tiles, the end piece a window limit
+        int tb_max = unaligned ? ge::temporal1d_max_tb(16 / (int)es * 4) - 2 : ge::temporal1d_max_tb(p->tc) - 2;
+        if (prefix && tb_max > p->tb) tb_max = p->tb;
+        tb1d = temporal1d_even_tb(left, p->level, p->tb, p->tc, tb_max);
+    }
     while (left > 0 && rc == GE_OK) {
         if (temporal_k) {
             // equal-sized blocks of at most tb levels (any starting phase)
@@ -1072,22 +1121,7 @@ int ge_run(ge_plan* p, void* u, int64_t steps, ge_stream_t stream) {
                 left -= 1;
             }
         } else if (temporal) {
-            int tbn;
-            if (p->tb % 2 == 0 && p->tb >= 4) {
-                // blocks that start at an odd level and have an even length are pure R/L pairs: a run from
-                // an even level opens with one block of tb-1 levels (in-lane level I first), a tail of one
-                // or two levels joins the last block (which may then end with R + shift back)
-                const int64_t nl = left > 2 ? (left - 2 + p->tb - 1) / p->tb : 1;   // launches to go (a block may take tb+2)
-                int64_t q = (left + nl - 1) / nl;
-                q += q & 1;
-                tbn = (int)((p->level & 1) ? q : q - 1);
-                if (tbn > left) tbn = (int)left;
-                if (left - tbn <= 2 && left <= ge::temporal1d_max_tb(p->tc)) tbn = (int)left;
-            } else {
-                // equal-sized blocks: ceil(left / tb) launches of (almost) the same number of levels
-                const int64_t nl = (left + p->tb - 1) / p->tb;
-                tbn = (int)((left + nl - 1) / nl);
-            }
+            const int tbn = temporal1d_block(left, p->level, tb1d, p->tc);
             if (unaligned) {
                 rc = p->dtype == GE_F64 ? launch_temporal_1d_unaligned<double>(p, cur, oth, tbn, s)
                                         : launch_temporal_1d_unaligned<float>(p, cur, oth, tbn, s);

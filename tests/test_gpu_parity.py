@@ -188,6 +188,22 @@ def test_unaligned_pointers_stay_blocked(oracle, dtype, batch, n, off):
     assert rel_err_rows(got, ref, cfg) <= TOL[dtype]
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_blocked_1d_runs_take_an_even_number_of_launches(oracle, dtype):
+    """The state ping-pongs between the caller's buffer and the plan's scratch level; ge_run picks the block length
+    so that runs of three or more launches end in the caller's buffer (no copy of the whole state).  Results do not
+    depend on the split: bit for bit the per-level kernel's."""
+    for batch, n in ((1, 2 ** 17), (3, 8192), (2, 4097)):
+        cfg = inputs.random_rods(batch, n, dtype, seed=n % 97)
+        for level0, steps in ((0, 100), (1, 100), (0, 220), (1, 61), (0, 59), (0, 300)):
+            got, info = run_gpu(cfg, steps, kernel="temporal", tb=20, level0=level0)
+            assert info["kernel"] == "temporal" and info["launches"] % 2 == 0 and info["launches"] <= steps // 8 + 2, (batch, n, level0, steps, info)
+            same, _ = run_gpu(cfg, steps, kernel="per_step", level0=level0)
+            np.testing.assert_array_equal(got, same, err_msg=str((dtype, batch, n, level0, steps, info)))
+    ref = run_oracle(oracle, cfg, 300)
+    assert rel_err_rows(got, ref, cfg) <= TOL[dtype]
+
+
 def test_run_is_deterministic():
     cfg = inputs.random_rods(4, 4096, "f32", seed=3)
     a, _ = run_gpu(cfg, 100)
