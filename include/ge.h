@@ -195,8 +195,10 @@ enum {
                                   every level through shared memory and named barriers instead of each recomputing
                                   tb stale columns per side (0 = a warp per strip; 4, 8; needs tb = 6 and
                                   nx >= value * 32 * columns per lane)                                              */
-    GE_TUNE_FORM_3D = 7,       /* 3-D per-level kernels: 1 = streaming kernel for the deep groups + shell kernel for the
-                                  outermost layer of groups (default, two launches per level), 0 = a thread per group    */
+    GE_TUNE_FORM_3D = 7,       /* 3-D per-level kernels: 1 (default) = streaming kernel for the full groups + shell kernel
+                                  for the groups cut by a face (one or two launches per level) where rows are a multiple
+                                  of 16 bytes and the buffers aligned, a thread per group elsewhere; 0 = a thread per
+                                  group always; 2 = the streaming kernel always (its scalar form on other rows)           */
     GE_TUNE_K_FORM = 8,        /* group_k >= 2, TEMPORAL: 1 = units of 2k nodes held in registers for tb levels + the two ends of the
                                   rod recomputed by the shared-memory kernel (default where compiled: k = 2, 4, 8, 16, fp32 also 32),
                                   0 = windows in shared memory throughout                                                  */

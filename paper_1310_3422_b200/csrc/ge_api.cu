@@ -317,9 +317,9 @@ int launch_level(ge_plan* p, const void* uin, void* uout, cudaStream_t s) {
                                 : launch_level_k<float>(p, uin, uout, phase, s);
     else if (p->dim == 3) {
         // the streaming form (deep groups) + shell, unless the grid is too small to have deep groups worth a launch
-        const int form = p->form3d && p->nx >= 8 && p->ny >= 8 && p->nz >= 8 ? 1 : 0;
+        const int form = p->form3d && p->nx >= 8 && p->ny >= 8 && p->nz >= 8 ? p->form3d : 0;
         int n = 0;
-        if (form == 1 && !p->aux3d) {        // side stream of the shell kernel (lazy; a failure just keeps everything on s)
+        if (form != 0 && !p->aux3d) {        // side stream of the shell kernel (lazy; a failure just keeps everything on s)
             int prio_least = 0, prio_greatest = 0;           // GE_S3D_MODE 2: the side stream carries the streaming kernel, ahead of the shell
             cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
             if (cudaStreamCreateWithPriority(&p->aux3d, cudaStreamNonBlocking, GE_S3D_MODE == 2 ? prio_greatest : prio_least) != cudaSuccess ||
@@ -1381,7 +1381,7 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
             p->kform = (int32_t)value;
             return GE_OK;
         case GE_TUNE_FORM_3D:
-            if (p->dim != 3 || (value != 0 && value != 1)) return GE_EINVAL;
+            if (p->dim != 3 || value < 0 || value > 2) return GE_EINVAL;
             p->form3d = (int32_t)value;
             return GE_OK;
         case GE_TUNE_STRIP_COOP:

@@ -34,11 +34,16 @@ def test_per_step_3d_streaming(oracle, dtype, nx, ny, nz):
     in for neighbours outside the box) + ge3d_shell_kernel for the
     outermost layer of groups.  Against the oracle, and bit for bit against the thread-per-group kernel."""
     cfg = inputs.random_box(nx, ny, nz, dtype, seed=nx * 100 + ny * 10 + nz, r=1.7)
+    vec = nx % (2 if dtype == "f64" else 4) == 0
     for level0, steps in ((0, 1), (1, 1), (0, 2), (1, 7)):
-        got, info = run_gpu(cfg, steps, level0=level0)
+        # form 2 = the streaming kernel whatever the row length (the default takes it for 16-byte rows only)
+        got, info = run_gpu(cfg, steps, level0=level0, form3d=2)
         # one streaming launch per level, one shell launch when the level has groups cut by a face
         cut = sum(1 for lev in range(level0, level0 + steps) if lev % 2 == 1 or nx % 2 or ny % 2 or nz % 2)
         assert info["kernel"] == "per_step" and info["launches"] == steps + cut
+        auto, ainfo = run_gpu(cfg, steps, level0=level0)
+        assert ainfo["launches"] == (steps + cut if vec else steps), ainfo
+        np.testing.assert_array_equal(got, auto)
         ref = run_oracle(oracle, cfg, steps, level0=level0)
         assert rel_err(got, ref) <= (5e-14 if dtype == "f64" else 5e-6), (nx, ny, nz, level0, steps)
         same, _ = run_gpu(cfg, steps, level0=level0, form3d=0)
