@@ -179,7 +179,8 @@ int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStre
     constexpr int V = 4;                               // columns per thread: one float4, two double2
     const bool aligned = (((uintptr_t)uin | (uintptr_t)uout) % 16 == 0);
     const int v = aligned && p->nx % V == 0 ? V : (aligned && p->nx % NV == 0 ? NV : 1);
-    const int64_t nvec = p->nx / v;
+    // rows that are not whole aligned vectors: V columns per thread all the same, element by element
+    const int64_t nvec = v == 1 ? (p->nx + V - 1) / V : p->nx / v;
     const int64_t npair = (p->ny + phase) / 2 + 1;      // anchor rows -phase, 2-phase, ... <= ny-1
     dim3 grid((unsigned)((nvec + ge::kLevel2dBx - 1) / ge::kLevel2dBx),
               (unsigned)((npair + ge::kLevel2dBy - 1) / ge::kLevel2dBy));
@@ -194,8 +195,8 @@ int launch_level_2d(ge_plan* p, const void* uin, void* uout, int phase, cudaStre
         if (phase == 0) ge::ge2d_level_kernel<T, NV, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
         else            ge::ge2d_level_kernel<T, NV, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
     } else {
-        if (phase == 0) ge::ge2d_level_kernel<T, 1, 0><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
-        else            ge::ge2d_level_kernel<T, 1, 1><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+        if (phase == 0) ge::ge2d_level_kernel<T, V, 0, false><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
+        else            ge::ge2d_level_kernel<T, V, 1, false><<<grid, block, 0, s>>>(in, out, p->nx, p->ny, c);
     }
     GE_CUDA(cudaGetLastError());
     p->launches += 1;

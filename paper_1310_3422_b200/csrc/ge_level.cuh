@@ -135,7 +135,9 @@ __device__ __forceinline__ void group_update(const T (&w)[4][4], const Coef2<T>&
 
 constexpr int kLevel2dBx = 32, kLevel2dBy = 8;
 
-template <typename T, int V, int PH>
+// AL = false: rows of any length at any alignment -- the thread still owns V columns of a group row (so every group is
+// computed once), read and written element by element; the last thread of a row may own fewer than V.
+template <typename T, int V, int PH, bool AL = true>
 __global__ void __launch_bounds__(kLevel2dBx * kLevel2dBy)
 ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, int64_t ny,
                   const Coef2<T>* __restrict__ coef) {
@@ -150,7 +152,7 @@ ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, i
     for (int rr = 0; rr < 4; ++rr) {
         const int64_t y = j0 - 1 + rr;
         const bool yin = y >= 0 && y < ny;
-        if constexpr (V > 1) {
+        if constexpr (V > 1 && AL) {
             constexpr int NV = VecOf<T>::V;            // native 16-byte vector; V is a multiple of it
             T t[NV];
             if (yin) {
@@ -201,7 +203,7 @@ ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, i
     for (int rr = 0; rr < 2; ++rr) {
         const int64_t y = j0 + rr;
         if (y < 0 || y >= ny) continue;
-        if constexpr (V > 1) {
+        if constexpr (V > 1 && AL) {
             constexpr int NV = VecOf<T>::V;
 #pragma unroll
             for (int c = 0; c < V / NV; ++c) {
@@ -211,7 +213,9 @@ ge2d_level_kernel(const T* __restrict__ uin, T* __restrict__ uout, int64_t nx, i
                 st_vec(uout + y * nx + e0 + c * NV, t);
             }
         } else {
-            uout[y * nx + e0] = o[rr][0];
+#pragma unroll
+            for (int j = 0; j < V; ++j)
+                if (e0 + j < nx) uout[y * nx + e0 + j] = o[rr][j];
         }
     }
 }
