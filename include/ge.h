@@ -54,7 +54,8 @@ typedef struct CUstream_st *ge_stream_t;        /* == cudaStream_t              
 typedef enum { GE_F32 = 0, GE_F64 = 1 } ge_dtype;
 
 typedef enum {
-    GE_KERNEL_AUTO = 0,       /* library picks per shape                  */
+    GE_KERNEL_AUTO = 0,       /* library picks per shape; 2-D grids below 24 MB of
+                                 state: PER_STEP (a blocked launch has a latency floor a small grid does not repay) */
     GE_KERNEL_PER_STEP = 1,   /* A: one launch per level, one HBM round trip per level              */
     GE_KERNEL_TEMPORAL = 2,   /* B: tb levels per launch in registers/SMEM, halo-redundant tiles    */
     GE_KERNEL_PERSISTENT = 3  /* C: state stays in registers for the whole run, one launch (1-D): a rod
@@ -187,7 +188,8 @@ enum {
                                   default for rods of >= 4 tiles (needs nx >= 32 * value)                   */
     GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
                                   2-D: one of the compiled-in block lengths 4, 6, 8; 6 needs the strip kernel)                            */
-    GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64) */
+    GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64; fewer, down to
+                                  16, on grids that would not give every SM its 16 warps)                              */
     GE_TUNE_RESIDENT_C = 3,    /* strategy C: values per lane (f64: 2..64, f32: 4..128, powers of two; one
                                   long rod: 16, 32, 64 (f64) / 32, 64, 128 (f32)); may synchronise and reallocate      */
     GE_TUNE_HALO_LANES = 4,    /* path 2: halo lanes per side, 1..8, default 2 (tb <= lanes * C); may synchronise */

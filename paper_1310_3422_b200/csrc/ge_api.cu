@@ -859,6 +859,12 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
         if (rc != GE_OK) { cudaFree(p->coef); cudaFree(p->scratch); cudaFree(p->res_xbuf); cudaFree(p->res_flags); cudaGetLastError(); delete p; return rc; }
         kernel = p->res_path ? GE_KERNEL_PERSISTENT : GE_KERNEL_TEMPORAL;
     }
+    // 2-D, AUTO: a blocked launch has a latency floor of 60 - 75 us (a warp marches its segment row pair by row pair
+    // through tb stages) whatever the grid, a per-level launch costs 4 us or its HBM time: below 24 MB of state one
+    // launch per level is faster (measured: fp32 2048^2 0.99 against 1.24 ms for 120 levels, 3072^2 1.63 against
+    // 1.54; fp64 1024^2 0.86 against 1.22, 2048^2 1.85 against 1.40)
+    if (d->dim == 2 && d->kernel == GE_KERNEL_AUTO && (int64_t)p->count * (int64_t)elem_size(p->dtype) < ((int64_t)24 << 20))
+        kernel = GE_KERNEL_PER_STEP;
     p->kernel = kernel;
     const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
     // measured on C4: the TMA-staged kernel is fp64-bound from tb ~ 12 on, best near 20
@@ -867,6 +873,16 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
         if (!temporal2d_tb_ok(p, p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
+        // segments: the C5 optimum (67 / 56 row pairs) leaves a smaller grid with too few warps -- 32 strips x 31
+        // segments on 4096^2 fp32 --, so segments shrink until strips x segments fill the chip's 16 warps per SM,
+        // down to 16 pairs (4096^2 fp32: 2.30 -> 1.88 ms for 120 levels at 16); GE_TUNE_SEG_PAIRS overrides
+        if (strip2d_ok(p)) {
+            const int64_t strips = (p->nx + 32 * ge::strip2d_columns_per_lane(p->dtype) - 1) / (32 * ge::strip2d_columns_per_lane(p->dtype));
+            const int64_t want = (int64_t)16 * p->sm_count;
+            int64_t hp = (p->ny / 2) * strips / want;
+            if (hp < 16) hp = 16;
+            if (hp < p->hp) p->hp = (int32_t)hp;
+        }
     }
     *out = p;
     return GE_OK;
