@@ -842,6 +842,20 @@ def run_src(args):
         gbs = 3.0 * es * glups
         roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
                 "traffic": traffic_of("%s/%s" % (cfg["name"], kname)), "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * n}
+    elif n % (16 // es) == 0 and n >= 32 * (128 // es):
+        # stationary source on rows of whole vectors: the register form (ge_temporal_src.cuh), bound by the fp pipes --
+        # the factored form's 5 flops per update + the source added to each right-hand side
+        lv = levels * args.steps / max(launches, 1)
+        kname = "ge1d_temporal_%s_kernel<%s>" % (what, cfg["dtype"])
+        alu = fma_peaks(dev, stream_obj)
+        tfl = (5.0 if args.var else 6.0) * glups / 1e3
+        peak = alu[cfg["dtype"] + "_tflops"]
+        roof = {"kernel": kname, "bound": "alu", "achieved": tfl, "peak": peak, "unit": "TFLOP/s", "frac": tfl / peak,
+                "traffic": None, "peak_source": "measured (in-run FMA microbenchmark, ge_fma_probe)", "levels_per_launch": lv,
+                "algorithmic_bytes_per_launch": 3.0 * es * n, "effective_gbs": 2.0 * es * glups,
+                "effective_frac_of_hbm": 2.0 * es * glups / peaks["hbm_gbs"],
+                "note": "flops per update: 4 FMA + 2 ADD per pair of the factored form (5 per node), + 1 ADD per node for tau*f "
+                        "(source); variable diffusivity: the same 5 with per-link coefficients from registers"}
     else:
         # blocked: HBM sees (2 u + 1 data) * sizeof(T) per node and launch of <= 16 levels; the kernel is bound by shared memory
         lv = levels * args.steps / max(launches, 1)

@@ -122,16 +122,19 @@ int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f,
  *   rl: device pointer, nx + 1 elements of dtype: rl[j] = tau * a(x_{j+1/2}) / h^2 > 0 for the link between nodes j
  *       and j+1, j = 0 .. N (the plan's own r is not used; the boundary values are the plan's).
  * Otherwise as ge_step_1d (batch == 1).  ge_run_var: `steps` such levels in place, temporally blocked (16 levels per HBM
- * round trip, the window and its link numbers resident in shared memory; ge_window.cuh), batched rods included: rl is
- * then [batch][nx + 1].  GE_EINVAL for dim != 1 or a null / misaligned pointer (ge_step_1d_var: also batch > 1),
+ * round trip: a tile's state, link numbers and pair factors in registers, ge_temporal_src.cuh -- rows of whole
+ * 16-byte vectors holding a tile --, else the window and its link numbers in shared memory, ge_window.cuh;
+ * GE_TUNE_SRC_FORM), batched rods included: rl is then [batch][nx + 1].  GE_EINVAL for dim != 1 or a null / misaligned pointer (ge_step_1d_var: also batch > 1),
  * GE_EUNSUPPORTED for group_k >= 2. */
 int ge_step_1d_var(ge_plan *p, const void *u_in, void *u_out, const void *rl, ge_stream_t stream);
 int ge_run_var(ge_plan *p, void *u, int64_t steps, const void *rl, ge_stream_t stream);
 
 /* `steps` >= 0 levels with a source term and moving boundary values in place (group_k == 1; result in u, level += steps):
  *   tau_f:          device pointer or NULL.  f_level_stride == 0: ONE STATIONARY source, [batch][nx] elements, used at
- *                   every level -- the run is temporally blocked (16 levels per HBM round trip, the source and the
- *                   window resident in shared memory; ge_window.cuh), batched rods included (per-rod r);
+ *                   every level -- the run is temporally blocked (16 levels per HBM round trip: a tile's state and
+ *                   source in registers, ge_temporal_src.cuh -- rows of whole 16-byte vectors holding a tile --, else
+ *                   the window and its source in shared memory, ge_window.cuh; GE_TUNE_SRC_FORM), batched rods
+ *                   included (per-rod r);
  *                   f_level_stride >= nx: level n of the run reads tau_f + n * f_level_stride (`steps` rows) -- one
  *                   launch of ge_step_1d_src per level, batch must be 1;
  *   bc_lo_t, bc_hi_t: HOST arrays, [batch][steps + 1] entries: the values of nodes 0 and N+1 of every rod at the run's
@@ -201,6 +204,9 @@ enum {
                                   for the groups cut by a face (one or two launches per level) where rows are a multiple
                                   of 16 bytes and the buffers aligned, a thread per group elsewhere; 0 = a thread per
                                   group always; 2 = the streaming kernel always (its scalar form on other rows)           */
+    GE_TUNE_SRC_FORM = 9,      /* ge_run_src with a stationary source, ge_run_var: 1 = the state and tau*f / the links of a tile in registers (default;
+                                  rows of whole aligned vectors holding at least one tile of 512 / 1024 nodes), 0 = windows in
+                                  shared memory (any row)                                                                  */
     GE_TUNE_K_FORM = 8,        /* group_k >= 2, TEMPORAL: 1 = units of 2k nodes held in registers for tb levels + the two ends of the
                                   rod recomputed by the shared-memory kernel (default where compiled: k = 2, 4, 8, 16, fp32 also 32),
                                   0 = windows in shared memory throughout                                                  */

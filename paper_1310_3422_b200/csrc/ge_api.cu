@@ -15,6 +15,7 @@
 
 #include "ge_common.cuh"
 #include "ge_level.cuh"
+#include "ge_temporal_src.cuh"
 #include "ge_temporal.cuh"
 #include "ge_temporal2d.cuh"
 #include "ge_resident.cuh"
@@ -86,6 +87,7 @@ struct ge_plan {
     int32_t strip_attr_tb;    // strip-kernel instantiation (tb*16 + coop) whose function attributes are set on this device (0: none)
     cudaStream_t aux3d;       // 3-D: side stream of the shell kernel, with its fork / join events (lazy)
     cudaEvent_t ev3d[2];
+    int32_t src_form;         // ge_run_src, stationary source: 1 registers (ge_temporal_src.cuh, default), 0 shared-memory windows
     int32_t kform;            // k >= 2 blocked kernel: 1 register-resident units + end windows (default), 0 shared-memory windows
     int32_t form3d;           // 3-D per-level form: 1 streaming + shell kernels (default), 0 a thread per group
     int32_t strip_coop;       // warps that share one strip of the 2-D strip kernel (0: a warp per strip)
@@ -840,6 +842,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->hp = p->dtype == GE_F64 ? 56 : 67;   // measured on C5 (the rate depends on the segment count, and sharply)
     p->form3d = 1;
     p->kform = 1;
+    p->src_form = 1;
     p->res_hl = 2;                 // measured on C2: 2 halo lanes, grid-wide meetings
     p->res_sync = ge::kSyncGrid;
     int kernel = d->kernel;
@@ -952,12 +955,30 @@ int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t s
     void* cur = u;
     void* oth = p->scratch;
     int64_t left = steps;
+    // rows of whole aligned vectors that hold a tile: the register form (ge_temporal_src.cuh); anything else: windows in
+    // shared memory (ge_window.cuh)
+    const int V = p->dtype == GE_F64 ? 2 : 4, cvar = p->dtype == GE_F64 ? 16 : 32;
+    const bool regs = p->nx % V == 0 && p->nx >= 32 * (int64_t)cvar && (uintptr_t)u % 16 == 0 && (uintptr_t)p->scratch % 16 == 0 &&
+                      p->src_form != 0;
     while (left > 0) {
-        // equal-sized blocks of at most kWindowTb levels, the link numbers resident in shared memory beside the window
+        // equal-sized blocks of at most kWindowTb levels, the link numbers resident beside the state
         const int64_t nl = (left + kWindowTb - 1) / kWindowTb;
         const int lv = (int)((left + nl - 1) / nl);
-        const int rc = p->dtype == GE_F64 ? launch_window<double, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s)
-                                          : launch_window<float, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s);
+        int rc;
+        if (regs) {
+            const int phase = (int)(p->level & 1);
+            const cudaError_t e = p->dtype == GE_F64
+                ? ge::temporal1d_var_launch<double, 16>((const double*)cur, (double*)oth, (const double*)rl, p->nx, p->batch,
+                                                        (const ge::Coef1<double>*)p->coef, lv, phase, s)
+                : ge::temporal1d_var_launch<float, 32>((const float*)cur, (float*)oth, (const float*)rl, p->nx, p->batch,
+                                                       (const ge::Coef1<float>*)p->coef, lv, phase, s);
+            if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+            p->launches += 1;
+            p->level += lv;
+            rc = GE_OK;
+        } else
+        rc = p->dtype == GE_F64 ? launch_window<double, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s)
+                                : launch_window<float, false, true>(p, cur, oth, nullptr, rl, nullptr, 0, 0, lv, s);
         if (rc != GE_OK) return rc;
         left -= lv;
         void* t = cur; cur = oth; oth = t;
@@ -1011,12 +1032,32 @@ int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_
             GE_CUDA(cudaMemcpyAsync(p->bc_dev, h.data(), bytes, cudaMemcpyHostToDevice, s));
             GE_CUDA(cudaStreamSynchronize(s));
         }
+        // rows of whole aligned vectors that hold a tile: the register form (ge_temporal_src.cuh); anything else: windows
+        // in shared memory (ge_window.cuh)
+        constexpr int kSrcTb = 16;
+        const int V = p->dtype == GE_F64 ? 2 : 4, csrc = p->dtype == GE_F64 ? 16 : 32;
+        const bool regs = p->nx % V == 0 && p->nx >= 32 * (int64_t)csrc && (uintptr_t)u % 16 == 0 && (uintptr_t)p->scratch % 16 == 0 &&
+                          (uintptr_t)tau_f % 16 == 0 && p->src_form != 0;
         int64_t left = steps, done = 0;
         while (left > 0) {
-            const int64_t nl = (left + kWindowTb - 1) / kWindowTb;
+            const int tbmax = regs ? kSrcTb : kWindowTb;
+            const int64_t nl = (left + tbmax - 1) / tbmax;
             const int lv = (int)((left + nl - 1) / nl);
-            const int rc = p->dtype == GE_F64 ? launch_window<double, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s)
-                                              : launch_window<float, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s);
+            int rc;
+            if (regs) {
+                const int phase = (int)(p->level & 1);
+                const cudaError_t e = p->dtype == GE_F64
+                    ? ge::temporal1d_src_launch<double, 16>((const double*)cur, (double*)oth, (const double*)tau_f, (const double*)p->bc_dev, done, steps + 1,
+                                                            p->nx, p->batch, (const ge::Coef1<double>*)p->coef, lv, phase, s)
+                    : ge::temporal1d_src_launch<float, 32>((const float*)cur, (float*)oth, (const float*)tau_f, (const float*)p->bc_dev, done, steps + 1,
+                                                           p->nx, p->batch, (const ge::Coef1<float>*)p->coef, lv, phase, s);
+                if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
+                p->launches += 1;
+                p->level += lv;
+                rc = GE_OK;
+            } else
+            rc = p->dtype == GE_F64 ? launch_window<double, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s)
+                                    : launch_window<float, true, false>(p, cur, oth, tau_f, nullptr, p->bc_dev, done, steps + 1, lv, s);
             if (rc != GE_OK) return rc;
             left -= lv; done += lv;
             void* t = cur; cur = oth; oth = t;
@@ -1396,6 +1437,10 @@ int ge_plan_tune(ge_plan* p, int32_t what, int64_t value) {
         case GE_TUNE_K_FORM:
             if (p->group_k < 2 || (value != 0 && value != 1)) return GE_EINVAL;
             p->kform = (int32_t)value;
+            return GE_OK;
+        case GE_TUNE_SRC_FORM:
+            if (p->dim != 1 || (value != 0 && value != 1)) return GE_EINVAL;
+            p->src_form = (int32_t)value;
             return GE_OK;
         case GE_TUNE_FORM_3D:
             if (p->dim != 3 || value < 0 || value > 2) return GE_EINVAL;

@@ -26,6 +26,7 @@ GE_INFO_KERNEL, GE_INFO_TB, GE_INFO_LAUNCHES, GE_INFO_TILE_VALID, GE_INFO_TILE_L
  GE_INFO_RESIDENT_TB, GE_INFO_MEETINGS, GE_INFO_SYNC_FAULT, GE_INFO_TEMPORAL_C) = 5, 6, 7, 8, 9, 10, 11, 12
 GE_TUNE_TEMPORAL_C, GE_TUNE_TB, GE_TUNE_SEG_PAIRS = 0, 1, 2
 GE_TUNE_RESIDENT_C, GE_TUNE_HALO_LANES, GE_TUNE_SYNC_MODE, GE_TUNE_STRIP_COOP, GE_TUNE_FORM_3D, GE_TUNE_K_FORM = 3, 4, 5, 6, 7, 8
+GE_TUNE_SRC_FORM = 9
 GE_SYNC_FLAGS, GE_SYNC_GRID, GE_SYNC_LINES, GE_SYNC_STAGGER = 0, 1, 2, 3
 GE_SYNC_CLUSTER2, GE_SYNC_CLUSTER4, GE_SYNC_CLUSTER8, GE_SYNC_CLUSTER16 = 4, 5, 6, 7
 

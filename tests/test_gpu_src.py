@@ -147,14 +147,17 @@ def test_run_src_argument_errors():
         assert plan.level == 0
 
 
+@pytest.mark.parametrize("form", [1, 0])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("batch,n,steps,level0", [(1, 100000, 203, 0), (5, 4099, 77, 1), (3, 1980, 40, 0), (2, 7, 33, 1),
-                                                  (64, 4096, 50, 0)])
-def test_run_src_blocked_with_a_stationary_source(oracle, dtype, batch, n, steps, level0):
-    """ge_run_src with one stationary source array: temporally blocked (windows of the rods with their source values in
-    shared memory, 16 levels per launch), batched rods with per-rod r, boundary values that move every level and
-    differ from rod to rod; several windows per rod, ragged last window, odd and tiny N, both starting phases.
-    Against the oracle marched level by level."""
+                                                  (64, 4096, 50, 0), (3, 1024, 35, 1), (2, 2 ** 16, 64, 1), (1, 2 ** 16 + 4, 17, 0)])
+def test_run_src_blocked_with_a_stationary_source(oracle, dtype, batch, n, steps, level0, form):
+    """ge_run_src with one stationary source array: temporally blocked, 16 levels per launch -- form 1 (default): the
+    state and the source values of a tile in registers (rows of whole aligned vectors that hold a tile), form 0 and
+    every other row: windows of the rods with their source values in shared memory; batched rods with per-rod r,
+    boundary values that move every level and differ from rod to rod; several tiles / windows per rod, ragged last
+    one, odd and tiny N, both starting phases, odd level counts.  Against the oracle marched level by level, and the
+    two forms bit for bit against each other."""
     import torch
     from paper_1310_3422_b200 import libge
     dt = _NP[dtype]
@@ -167,10 +170,18 @@ def test_run_src_blocked_with_a_stationary_source(oracle, dtype, batch, n, steps
     d_src = torch.from_numpy(src).to(dev)
     s = torch.cuda.current_stream(dev).cuda_stream
     with libge.Plan(cfg, stream=s) as plan:
+        plan.tune(libge.GE_TUNE_SRC_FORM, form)
         plan.level = level0
         plan.run_src(u.data_ptr(), steps, d_src.data_ptr(), 0, walk[:, :, 0].reshape(-1), walk[:, :, 1].reshape(-1), s)
         torch.cuda.synchronize(dev)
         assert plan.level == level0 + steps and plan.info()["launches"] == -(-steps // 16)
+        if form == 1:                       # the other form from the same start: the same bits
+            v = torch.from_numpy(cfg["u0"].copy()).to(dev)
+            plan.tune(libge.GE_TUNE_SRC_FORM, 0)
+            plan.level = level0
+            plan.run_src(v.data_ptr(), steps, d_src.data_ptr(), 0, walk[:, :, 0].reshape(-1), walk[:, :, 1].reshape(-1), s)
+            torch.cuda.synchronize(dev)
+            assert torch.equal(u, v)
     got = u.cpu().numpy().astype(np.float64)
     for b in range(batch):
         ref = cfg["u0"][b].astype(np.float64)

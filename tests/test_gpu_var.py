@@ -92,12 +92,16 @@ def test_var_argument_errors():
             plan.run_var(u.data_ptr(), -1, u.data_ptr() + 8 * 128)
 
 
+@pytest.mark.parametrize("form", [1, 0])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("batch,n,steps,level0", [(1, 100000, 203, 0), (5, 4099, 77, 1), (3, 1980, 40, 0), (2, 7, 33, 1)])
-def test_run_var_blocked_and_batched(oracle, dtype, batch, n, steps, level0):
-    """ge_run_var: windows of the rods with their link numbers in shared memory, 16 levels per launch, batched rods each
-    with its own links and boundary values; several windows per rod, odd and tiny N.  Against the oracle, and against
-    the per-level kernel (same expressions: to rounding of the in-kernel division only -- identical here)."""
+@pytest.mark.parametrize("batch,n,steps,level0", [(1, 100000, 203, 0), (5, 4099, 77, 1), (3, 1980, 40, 0), (2, 7, 33, 1),
+                                                  (4, 4096, 50, 1), (3, 1024, 35, 0), (1, 2 ** 16 + 4, 17, 1)])
+def test_run_var_blocked_and_batched(oracle, dtype, batch, n, steps, level0, form):
+    """ge_run_var, 16 levels per launch -- form 1 (default): the state, the link numbers and the pair factors of a tile
+    in registers (rows of whole aligned vectors that hold a tile); form 0 and every other row: windows of the rods
+    with their link numbers in shared memory; batched rods each with its own links and boundary values; several tiles
+    / windows per rod, odd and tiny N.  Against the oracle, against the per-level kernel (same expressions: bit for
+    bit) and form against form."""
     import torch
     from paper_1310_3422_b200 import libge
     dt = _NP[dtype]
@@ -108,10 +112,18 @@ def test_run_var_blocked_and_batched(oracle, dtype, batch, n, steps, level0):
     d_rl = torch.from_numpy(rl).to(dev)
     s = torch.cuda.current_stream(dev).cuda_stream
     with libge.Plan(cfg, stream=s) as plan:
+        plan.tune(libge.GE_TUNE_SRC_FORM, form)
         plan.level = level0
         plan.run_var(u.data_ptr(), steps, d_rl.data_ptr(), s)
         torch.cuda.synchronize(dev)
         assert plan.info()["launches"] == -(-steps // 16)
+        if form == 1:
+            v2 = torch.from_numpy(cfg["u0"].copy()).to(dev)
+            plan.tune(libge.GE_TUNE_SRC_FORM, 0)
+            plan.level = level0
+            plan.run_var(v2.data_ptr(), steps, d_rl.data_ptr(), s)
+            torch.cuda.synchronize(dev)
+            assert torch.equal(u, v2)
     got = u.cpu().numpy().astype(np.float64)
     for b in range(batch):
         ref = oracle.run_1d_var(cfg["u0"][b].astype(np.float64), rl[b].astype(np.float64), steps, cfg["bc_lo"][b],
