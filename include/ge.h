@@ -216,7 +216,7 @@ enum {
                                   every tb/2 levels and consumed every other time, the CTAs that share an SM
                                   taking opposite turns (needs tb >= 8); 4, 5, 6, 7 = thread-block CLUSTERS of 2, 4, 8,
                                   16 CTAs: shared memory (the CTA's own or, through distributed shared memory, the
-                                  adjacent CTA's) and the cluster's hardware barrier inside a cluster, mode 0's flags
+                                  adjacent CTA's) and the cluster's hardware barrier inside a cluster, mode 2's lines
                                   between clusters; GE_EINVAL when the rod cannot stay resident with clusters of that
                                   size; default 1, the fastest measured                                              */
 };

@@ -287,7 +287,7 @@ constexpr int kSyncFlags = 0, kSyncGrid = 1, kSyncLL = 2, kSyncStagger = 3;
 // 4 .. 7 = thread-block CLUSTERS of 2 / 4 / 8 / 16 CTAs (kernel instantiation CL = true): the tiles of a cluster
 // publish into their CTA's shared memory, meet at the cluster's hardware barrier and read their neighbours' sides
 // from shared memory -- their own CTA's or, through distributed shared memory, the adjacent CTA's; only the two
-// tiles at the ends of a cluster exchange through L2 with a flag, as in mode 0
+// tiles at the ends of a cluster exchange through L2, with flag-in-data lines as in mode 2
 constexpr int kSyncCluster2 = 4, kSyncCluster16 = 7;
 inline int sync_cluster_size(int mode) { return mode >= kSyncCluster2 && mode <= kSyncCluster16 ? 2 << (mode - kSyncCluster2) : 1; }
 constexpr int kLineSlots = 4;          // exchange slots of the flag-in-data modes (2 are used by kSyncLL)
@@ -510,40 +510,39 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
             if (active && (own_l || own_r)) {
                 T* dst = xs + ((size_t)(parity * kGridWarps + warp) * 2 + (own_l ? 0 : 1)) * side +
                          (size_t)(own_l ? lane - hl : lane - (32 - 2 * hl)) * C;
-                T* gdst = nullptr;
-                if ((own_l && cross_l) || (own_r && cross_r))
-                    gdst = xbuf + ((size_t)parity * a.ntiles + tile) * 2 * side +
-                           (own_l ? (size_t)(lane - hl) * C : side + (size_t)(lane - (32 - 2 * hl)) * C);
 #pragma unroll
                 for (int j = 0; j < C / V; ++j) {
                     T t[V];
 #pragma unroll
                     for (int i = 0; i < V; ++i) t[i] = v[j * V + i];
                     st_vec(dst + j * V, t);
-                    if (gdst) st_vec_cg(gdst + j * V, t);
+                }
+                // the side that faces another cluster also goes to L2 as flag-in-data lines (mode 2's exchange: payload
+                // and meeting number in one 8-byte unit, no fence, no separate flag)
+                if ((own_l && cross_l) || (own_r && cross_r)) {
+                    uint4* xl = reinterpret_cast<uint4*>(xbuf);
+                    const size_t lside = (size_t)hl * NQ;
+                    uint4* ldst = xl + ((size_t)parity * a.ntiles + tile) * 2 * lside +
+                                  (own_l ? (size_t)(lane - hl) * NQ : lside + (size_t)(lane - (32 - 2 * hl)) * NQ);
+#pragma unroll
+                    for (int j = 0; j < NQ; ++j) Line<T>::put(ldst + j, &v[j * Line<T>::per], stage);
                 }
             }
-            if (active && (cross_l || cross_r)) {
-                __syncwarp();
-                if (lane == 0) { __threadfence(); st_relaxed_u32(flags + tile, stage); }
-            }
             cluster.sync();
-            if (active && (cross_l || cross_r)) {
-                if (lane == 0) wait_flags(cross_l ? flags + tile - 1 : nullptr, cross_r ? flags + tile + 1 : nullptr, stage, fault);
-                __syncwarp();
-            }
             if (active) {
                 const T* src = nullptr;
-                bool global = false;
+                const uint4* lsrc = nullptr;
                 if (halo_l && has_l) {
-                    if (cross_l) { src = xbuf + ((size_t)parity * a.ntiles + tile - 1) * 2 * side + side + (size_t)lane * C; global = true; }
+                    if (cross_l) lsrc = reinterpret_cast<const uint4*>(xbuf) + ((size_t)parity * a.ntiles + tile - 1) * 2 * ((size_t)hl * NQ) +
+                                        (size_t)hl * NQ + (size_t)lane * NQ;
                     else {
                         const T* base = warp > 0 ? xs : cluster.map_shared_rank(xs, crank - 1);
                         const int w = warp > 0 ? warp - 1 : kGridWarps - 1;
                         src = base + ((size_t)(parity * kGridWarps + w) * 2 + 1) * side + (size_t)lane * C;
                     }
                 } else if (halo_r && has_r) {
-                    if (cross_r) { src = xbuf + ((size_t)parity * a.ntiles + tile + 1) * 2 * side + (size_t)(lane - (32 - hl)) * C; global = true; }
+                    if (cross_r) lsrc = reinterpret_cast<const uint4*>(xbuf) + ((size_t)parity * a.ntiles + tile + 1) * 2 * ((size_t)hl * NQ) +
+                                        (size_t)(lane - (32 - hl)) * NQ;
                     else {
                         const T* base = warp < kGridWarps - 1 ? xs : cluster.map_shared_rank(xs, crank + 1);
                         const int w = warp < kGridWarps - 1 ? warp + 1 : 0;
@@ -554,11 +553,32 @@ ge1d_grid_resident_kernel(T* u, T* xbuf, const Coef1<T>* __restrict__ coef, unsi
 #pragma unroll
                     for (int j = 0; j < C / V; ++j) {
                         T t[V];
-                        if (global) ld_vec_cg(src + j * V, t); else ld_vec_plain(src + j * V, t);
+                        ld_vec_plain(src + j * V, t);
 #pragma unroll
                         for (int i = 0; i < V; ++i) v[j * V + i] = t[i];
                     }
                 }
+                if (lsrc) {                       // poll the other cluster's lines until every tag is this meeting's
+                    uint4 q[NQ];
+                    bool ok = false;
+                    for (unsigned it = 0; it < (1u << 22); ++it) {
+                        const uint4 w = ld_line(lsrc + NQ - 1);
+                        if (w.y == stage && w.w == stage) break;
+                        __nanosleep(it < 64 ? 20 : 200);
+                    }
+                    for (unsigned it = 0; it < (1u << 20) && !ok; ++it) {
+#pragma unroll
+                        for (int j = 0; j < NQ; ++j) q[j] = ld_line(lsrc + j);
+                        ok = true;
+#pragma unroll
+                        for (int j = 0; j < NQ; ++j) ok = ok && q[j].y == stage && q[j].w == stage;
+                        if (!ok) __nanosleep(100);
+                    }
+                    if (!ok) atomicExch(fault, 1u);
+#pragma unroll
+                    for (int j = 0; j < NQ; ++j) Line<T>::get(q[j], &v[j * Line<T>::per]);
+                }
+                __syncwarp();
             }
             parity ^= 1;
         }
