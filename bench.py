@@ -842,7 +842,7 @@ def run_src(args):
         gbs = 3.0 * es * glups
         roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
                 "traffic": traffic_of("%s/%s" % (cfg["name"], kname)), "peak_source": srcp, "algorithmic_bytes_per_launch": 3.0 * es * n}
-    elif n % (16 // es) == 0 and n >= 32 * (128 // es):
+    elif n % (16 // es) == 0 and n >= 32 * (64 // es):
         # stationary source on rows of whole vectors: the register form (ge_temporal_src.cuh), bound by the fp pipes --
         # the factored form's 5 flops per update + the source added to each right-hand side
         lv = levels * args.steps / max(launches, 1)

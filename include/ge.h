@@ -205,7 +205,7 @@ enum {
                                   of 16 bytes and the buffers aligned, a thread per group elsewhere; 0 = a thread per
                                   group always; 2 = the streaming kernel always (its scalar form on other rows)           */
     GE_TUNE_SRC_FORM = 9,      /* ge_run_src with a stationary source, ge_run_var: 1 = the state and tau*f / the links of a tile in registers (default;
-                                  rows of whole aligned vectors holding at least one tile of 512 / 1024 nodes), 0 = windows in
+                                  rows of whole aligned vectors holding at least one tile of 256 / 512 nodes), 0 = windows in
                                   shared memory (any row)                                                                  */
     GE_TUNE_K_FORM = 8,        /* group_k >= 2, TEMPORAL: 1 = units of 2k nodes held in registers for tb levels + the two ends of the
                                   rod recomputed by the shared-memory kernel (default where compiled: k = 2, 4, 8, 16, fp32 also 32),

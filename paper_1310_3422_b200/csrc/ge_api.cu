@@ -28,6 +28,15 @@
 #include "ge_level_var.cuh"
 #include "ge_window.cuh"
 
+// (measured on a 2^27 rod, GLUPS source / variable diffusivity: fp64 C = 16 2326 / 1793, C = 8 2943 / 2455;
+// fp32 C = 32 4584 / 2781, C = 16 4794 / 4737, C = 8 4436 / 4359)
+#ifndef GE_SRC_C_F64
+#define GE_SRC_C_F64 8
+#endif
+#ifndef GE_SRC_C_F32
+#define GE_SRC_C_F32 16          // values per lane of the fp32 register kernels for non-constant data
+#endif
+
 namespace {
 
 thread_local char g_errbuf[512];
@@ -958,7 +967,7 @@ int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t s
     int64_t left = steps;
     // rows of whole aligned vectors that hold a tile: the register form (ge_temporal_src.cuh); anything else: windows in
     // shared memory (ge_window.cuh)
-    const int V = p->dtype == GE_F64 ? 2 : 4, cvar = p->dtype == GE_F64 ? 16 : 32;
+    const int V = p->dtype == GE_F64 ? 2 : 4, cvar = p->dtype == GE_F64 ? GE_SRC_C_F64 : GE_SRC_C_F32;
     const bool regs = p->nx % V == 0 && p->nx >= 32 * (int64_t)cvar && (uintptr_t)u % 16 == 0 && (uintptr_t)p->scratch % 16 == 0 &&
                       p->src_form != 0;
     while (left > 0) {
@@ -969,9 +978,9 @@ int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t s
         if (regs) {
             const int phase = (int)(p->level & 1);
             const cudaError_t e = p->dtype == GE_F64
-                ? ge::temporal1d_var_launch<double, 16>((const double*)cur, (double*)oth, (const double*)rl, p->nx, p->batch,
+                ? ge::temporal1d_var_launch<double, GE_SRC_C_F64>((const double*)cur, (double*)oth, (const double*)rl, p->nx, p->batch,
                                                         (const ge::Coef1<double>*)p->coef, lv, phase, s)
-                : ge::temporal1d_var_launch<float, 32>((const float*)cur, (float*)oth, (const float*)rl, p->nx, p->batch,
+                : ge::temporal1d_var_launch<float, GE_SRC_C_F32>((const float*)cur, (float*)oth, (const float*)rl, p->nx, p->batch,
                                                        (const ge::Coef1<float>*)p->coef, lv, phase, s);
             if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
             p->launches += 1;
@@ -1036,7 +1045,7 @@ int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_
         // rows of whole aligned vectors that hold a tile: the register form (ge_temporal_src.cuh); anything else: windows
         // in shared memory (ge_window.cuh)
         constexpr int kSrcTb = 16;
-        const int V = p->dtype == GE_F64 ? 2 : 4, csrc = p->dtype == GE_F64 ? 16 : 32;
+        const int V = p->dtype == GE_F64 ? 2 : 4, csrc = p->dtype == GE_F64 ? GE_SRC_C_F64 : GE_SRC_C_F32;
         const bool regs = p->nx % V == 0 && p->nx >= 32 * (int64_t)csrc && (uintptr_t)u % 16 == 0 && (uintptr_t)p->scratch % 16 == 0 &&
                           (uintptr_t)tau_f % 16 == 0 && p->src_form != 0;
         int64_t left = steps, done = 0;
@@ -1048,9 +1057,9 @@ int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_
             if (regs) {
                 const int phase = (int)(p->level & 1);
                 const cudaError_t e = p->dtype == GE_F64
-                    ? ge::temporal1d_src_launch<double, 16>((const double*)cur, (double*)oth, (const double*)tau_f, (const double*)p->bc_dev, done, steps + 1,
+                    ? ge::temporal1d_src_launch<double, GE_SRC_C_F64>((const double*)cur, (double*)oth, (const double*)tau_f, (const double*)p->bc_dev, done, steps + 1,
                                                             p->nx, p->batch, (const ge::Coef1<double>*)p->coef, lv, phase, s)
-                    : ge::temporal1d_src_launch<float, 32>((const float*)cur, (float*)oth, (const float*)tau_f, (const float*)p->bc_dev, done, steps + 1,
+                    : ge::temporal1d_src_launch<float, GE_SRC_C_F32>((const float*)cur, (float*)oth, (const float*)tau_f, (const float*)p->bc_dev, done, steps + 1,
                                                            p->nx, p->batch, (const ge::Coef1<float>*)p->coef, lv, phase, s);
                 if (e != cudaSuccess) { g_last_cuda = e; return GE_ECUDA; }
                 p->launches += 1;
