@@ -188,7 +188,7 @@ int ge_plan_info(const ge_plan *p, int32_t what, int64_t *value);
 enum {
     GE_TUNE_TEMPORAL_C = 0,    /* values per lane of the 1-D temporal kernel: 8, 16, 32 (f64) / 16, 32, 64 (f32):
                                   warp-per-tile kernel; 18, 22, 26 (f64) / 36, 44, 52 (f32): TMA-staged persistent kernel, 22 / 52 the
-                                  default for rods of >= 4 tiles (needs nx >= 32 * value)                   */
+                                  default for rods of >= 2 tiles, 8 / 16 for shorter rods (needs nx >= 32 * value)          */
     GE_TUNE_TB = 1,            /* levels per launch, or between meetings on path 2 (1-D: >= 1, clamped to the largest the tile allows;
                                   2-D: one of the compiled-in block lengths 4, 6, 8; 6 needs the strip kernel)                            */
     GE_TUNE_SEG_PAIRS = 2,     /* 2-D temporal kernel: output row pairs per warp segment (default 67 f32, 56 f64; fewer, down to
