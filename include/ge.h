@@ -121,9 +121,9 @@ int ge_step_1d_src(ge_plan *p, const void *u_in, void *u_out, const void *tau_f,
  * reading R-VAR; the paper's coefficient is constant): u_t = (a(x) u_x)_x in flux form.
  *   rl: device pointer, nx + 1 elements of dtype: rl[j] = tau * a(x_{j+1/2}) / h^2 > 0 for the link between nodes j
  *       and j+1, j = 0 .. N (the plan's own r is not used; the boundary values are the plan's).
- * Otherwise as ge_step_1d (batch == 1).  ge_run_var: `steps` such levels in place, temporally blocked (16 levels per HBM
+ * Otherwise as ge_step_1d (batch == 1).  ge_run_var: `steps` such levels in place, temporally blocked (20 levels per HBM
  * round trip: a tile's state, link numbers and pair factors in registers, ge_temporal_src.cuh -- rows of whole
- * 16-byte vectors holding a tile --, else the window and its link numbers in shared memory, ge_window.cuh;
+ * 16-byte vectors holding a tile --, else the window and its link numbers in shared memory, 16 levels, ge_window.cuh;
  * GE_TUNE_SRC_FORM), batched rods included: rl is then [batch][nx + 1].  GE_EINVAL for dim != 1 or a null / misaligned pointer (ge_step_1d_var: also batch > 1),
  * GE_EUNSUPPORTED for group_k >= 2. */
 int ge_step_1d_var(ge_plan *p, const void *u_in, void *u_out, const void *rl, ge_stream_t stream);
@@ -131,9 +131,9 @@ int ge_run_var(ge_plan *p, void *u, int64_t steps, const void *rl, ge_stream_t s
 
 /* `steps` >= 0 levels with a source term and moving boundary values in place (group_k == 1; result in u, level += steps):
  *   tau_f:          device pointer or NULL.  f_level_stride == 0: ONE STATIONARY source, [batch][nx] elements, used at
- *                   every level -- the run is temporally blocked (16 levels per HBM round trip: a tile's state and
+ *                   every level -- the run is temporally blocked (20 levels per HBM round trip: a tile's state and
  *                   source in registers, ge_temporal_src.cuh -- rows of whole 16-byte vectors holding a tile --, else
- *                   the window and its source in shared memory, ge_window.cuh; GE_TUNE_SRC_FORM), batched rods
+ *                   the window and its source in shared memory, 16 levels, ge_window.cuh; GE_TUNE_SRC_FORM), batched rods
  *                   included (per-rod r);
  *                   f_level_stride >= nx: level n of the run reads tau_f + n * f_level_stride (`steps` rows) -- one
  *                   launch of ge_step_1d_src per level, batch must be 1;

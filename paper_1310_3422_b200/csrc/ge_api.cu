@@ -756,6 +756,12 @@ bool resident_ok(const ge_plan* p, const void* u) {
 
 // ---- strategy B with non-constant data (ge_window.cuh): `levels` <= kWindowTb levels per launch ----
 constexpr int kWindowTb = 16;
+// (2^27 rod, GLUPS source / variable diffusivity at 8 / 12 / 16 / 20 / 24 levels per launch: fp64 2085 / 2735 / 2941 /
+// 2933 / 2816 and 1546 / 2019 / 2449 / 2668 / 2693; fp32 3698 / 4293 / 4775 / 4998 / 4958 and 2485 / 3454 / 4739 / 5610 / 5747)
+#ifndef GE_SRC_TB
+#define GE_SRC_TB 20
+#endif
+constexpr int kSrcTb = GE_SRC_TB;        // levels per launch of the register kernels for non-constant data
 template <typename T, bool SRC, bool VAR>
 int launch_window(ge_plan* p, const void* uin, void* uout, const void* src, const void* rl, const void* bc, int64_t bc_lev,
                   int64_t bc_stride, int levels, cudaStream_t s) {
@@ -974,7 +980,8 @@ int ge_run_var(ge_plan* p, void* u, int64_t steps, const void* rl, ge_stream_t s
                       p->src_form != 0;
     while (left > 0) {
         // equal-sized blocks of at most kWindowTb levels, the link numbers resident beside the state
-        const int64_t nl = (left + kWindowTb - 1) / kWindowTb;
+        const int tbmax = regs ? kSrcTb : kWindowTb;
+        const int64_t nl = (left + tbmax - 1) / tbmax;
         const int lv = (int)((left + nl - 1) / nl);
         int rc;
         if (regs) {
@@ -1046,7 +1053,6 @@ int ge_run_src(ge_plan* p, void* u, int64_t steps, const void* tau_f, int64_t f_
         }
         // rows of whole aligned vectors that hold a tile: the register form (ge_temporal_src.cuh); anything else: windows
         // in shared memory (ge_window.cuh)
-        constexpr int kSrcTb = 16;
         const int V = p->dtype == GE_F64 ? 2 : 4, csrc = p->dtype == GE_F64 ? GE_SRC_C_F64 : GE_SRC_C_F32;
         const bool regs = p->nx % V == 0 && p->nx >= 32 * (int64_t)csrc && (uintptr_t)u % 16 == 0 && (uintptr_t)p->scratch % 16 == 0 &&
                           (uintptr_t)tau_f % 16 == 0 && p->src_form != 0;

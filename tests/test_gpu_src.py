@@ -174,7 +174,9 @@ def test_run_src_blocked_with_a_stationary_source(oracle, dtype, batch, n, steps
         plan.level = level0
         plan.run_src(u.data_ptr(), steps, d_src.data_ptr(), 0, walk[:, :, 0].reshape(-1), walk[:, :, 1].reshape(-1), s)
         torch.cuda.synchronize(dev)
-        assert plan.level == level0 + steps and plan.info()["launches"] == -(-steps // 16)
+        # 20 levels per launch in registers (rows of whole vectors that hold a tile), 16 in shared memory
+        regs = form == 1 and n % (2 if dtype == "f64" else 4) == 0 and n >= (256 if dtype == "f64" else 512)
+        assert plan.level == level0 + steps and plan.info()["launches"] == -(-steps // (20 if regs else 16))
         if form == 1:                       # the other form from the same start: the same bits
             v = torch.from_numpy(cfg["u0"].copy()).to(dev)
             plan.tune(libge.GE_TUNE_SRC_FORM, 0)
