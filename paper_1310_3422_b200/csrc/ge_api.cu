@@ -889,7 +889,7 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
     p->kernel = kernel;
     const bool temporal_like = kernel == GE_KERNEL_TEMPORAL || kernel == GE_KERNEL_PERSISTENT;   // C falls back to B
     // measured on C4: the TMA-staged kernel is fp64-bound from tb ~ 12 on, best near 20
-    if (temporal_like && d->dim == 1 && d->group_k == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (is_stream_tc(p->dtype, p->tc) ? 20 : 16));
+    if (temporal_like && d->dim == 1 && d->group_k == 1) p->tb = clamp_tb(p, d->tb > 0 ? d->tb : (is_stream_tc(p->dtype, p->tc) ? 20 : 24));   // (warp-per-tile, 65536 rods of 1032 nodes: fp64 3278 / 3348 / 3420 GLUPS at 16 / 20 / 24, fp32 5137 / 5255 / 5388)
     if (temporal_like && d->dim == 2) {
         p->tc = 4;
         p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
