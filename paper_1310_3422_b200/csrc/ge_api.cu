@@ -895,14 +895,16 @@ int ge_plan_create(ge_plan** out, const ge_desc* d, ge_stream_t stream) {
         p->tb = d->tb > 0 ? d->tb : (strip2d_ok(p) ? 6 : 8);   // measured on C5
         if (!temporal2d_tb_ok(p, p->tb)) { cudaFree(p->coef); cudaFree(p->scratch); delete p; return GE_EINVAL; }
         // segments: the C5 optimum (67 / 56 row pairs) leaves a smaller grid with too few warps -- 32 strips x 31
-        // segments on 4096^2 fp32 --, so segments shrink until strips x segments fill the chip's 16 warps per SM,
-        // down to 16 pairs (4096^2 fp32: 2.30 -> 1.88 ms for 120 levels at 16); GE_TUNE_SEG_PAIRS overrides
+        // segments on 4096^2 fp32 --, so segments shrink until strips x segments give every SM ~28 warps, down to 16
+        // pairs; GE_TUNE_SEG_PAIRS overrides
         if (strip2d_ok(p)) {
             const int64_t strips = (p->nx + 32 * ge::strip2d_columns_per_lane(p->dtype) - 1) / (32 * ge::strip2d_columns_per_lane(p->dtype));
-            const int64_t want = (int64_t)16 * p->sm_count;
+            // (4096^2, 120 levels: fp32 2.30 / 2.16 / 1.88 ms at 67 / 32 / 16 pairs, fp64 2.56 / 2.42 / 2.62 at 56 / 32 / 16:
+            // both optima hold ~28 warps per SM)
+            const int64_t want = (int64_t)28 * p->sm_count;
             int64_t hp = (p->ny / 2) * strips / want;
             if (hp < 16) hp = 16;
-            if (hp < p->hp) p->hp = (int32_t)hp;
+            if (4 * hp < 3 * p->hp) p->hp = (int32_t)hp;         // (near the C5 optimum the rate is too sensitive to move)
         }
     }
     *out = p;
