@@ -75,3 +75,21 @@ def test_product_does_not_import_oracle():
                 assert "ge_oracle" not in txt and "ge_ref" not in txt, f
     o = open(os.path.join(ROOT, "oracle", "ge_oracle.py")).read()
     assert not re.search(r"^\s*(import|from)\s+paper_1310_3422_b200", o, flags=re.M)
+
+
+def test_static_entry_point_validates_without_a_gpu(lib):
+    """ge_run_1d_static rejects what it cannot take before any CUDA call, with a message that names the limit."""
+    from paper_1310_3422_b200 import libge
+    assert libge.GE_STATIC_MAX_BYTES == 4 * 1024 * 1024
+    for dtype, nmax in ((libge.GE_F64, libge.GE_STATIC_MAX_BYTES // 8), (libge.GE_F32, libge.GE_STATIC_MAX_BYTES // 4)):
+        rc = lib.ge_run_1d_static(dtype, 4096, 1 << 30, nmax + 1, 1, 0, 1.0, 0.0, 0.0, None)
+        assert rc == libge.GE_EINVAL
+        msg = libge.ge_static_error()
+        assert "exceeds the static scratch array" in msg and str(nmax) in msg, msg
+    for args in ((7, 4096, 8192, 16, 1, 0, 1.0, 0.0, 0.0), (libge.GE_F64, 0, 8192, 16, 1, 0, 1.0, 0.0, 0.0),
+                 (libge.GE_F64, 4096, 4096 + 64, 16, 1, 0, 1.0, 0.0, 0.0), (libge.GE_F64, 4096, 8192, 16, -1, 0, 1.0, 0.0, 0.0),
+                 (libge.GE_F64, 4096, 8192, 16, 1, 0, 0.0, 0.0, 0.0), (libge.GE_F64, 4096, 8192, 16, 1, 0, 1.0, float("nan"), 0.0),
+                 (libge.GE_F64, 4100, 8192, 16, 1, 0, 1.0, 0.0, 0.0)):
+        assert lib.ge_run_1d_static(*args, None) == libge.GE_EINVAL, args
+        assert libge.ge_static_error() != "ok"
+    assert lib.ge_static_error(None, 10) == libge.GE_EINVAL
